@@ -1,0 +1,204 @@
+/* prr.h — C ABI of the B200-native PRR (Predict, Reuse, Repair) decode hot path.
+ *
+ * Source of the operations: /root/reference/PAPER.md (arxiv 2606.30389).  "PAPER.md:n" below is a
+ * line of that file; Q1..Q15 are the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every call returns an int32 status (PRR_OK = 0).  No exceptions, no abort(), no I/O.
+ *   - "dev" pointers are CUDA device memory owned by the CALLER, 16-byte aligned; "host" pointers
+ *     are ordinary host memory.  The library owns only what lives in the prr_ctx (EMA state, theta,
+ *     scores, block sets, partial attention states, streams/events) and frees it in prr_destroy.
+ *     It never allocates on the per-step path.
+ *   - Every call that takes `stream` (a cudaStream_t passed as void*) only ENQUEUES work on it and
+ *     returns; results are valid after the caller synchronises that stream.  Calls that fill a host
+ *     output (prr_calibrate with theta_out/H_out, prr_get_stats, prr_decode_step_host) synchronise
+ *     the stream themselves.  All calls may be issued while `stream` is being captured into a CUDA
+ *     graph (prr_graph_begin/end or the caller's own capture) except those that synchronise.
+ *   - Errors: bad arguments -> PRR_E_INVALID before any launch; unsupported shape/dtype ->
+ *     PRR_E_UNSUPPORTED; decode before theta/EMA state exists is NOT an error (P is empty and the
+ *     step degenerates to repair over all of A, Q5); CUDA failures -> PRR_E_CUDA; prr_last_error
+ *     gives the text.  No partial output on an argument error.  There is no CPU fallback.
+ *   - Layouts (row-major, innermost last):
+ *       K/V pages   bf16  [n_pages, n_kv_heads, block_size, head_dim]
+ *       block_table int32 [batch, max_blocks_per_seq]     logical block -> physical page
+ *       seq_lens    int32 [batch]                         tokens in the cache
+ *       summaries   bf16  [batch, n_kv_heads, max_blocks_per_seq, head_dim]   (one buffer per layer)
+ *       q           bf16  [batch, n_q_heads, head_dim]; query head g belongs to KV head g / G
+ *       scores      fp32  [batch, n_kv_heads, max_blocks_per_seq]
+ *       block lists int32 [batch, n_kv_heads, width] ascending block index, padded with -1
+ *       partials    fp32  O [batch, n_q_heads, width, head_dim] unnormalised, m and l
+ *                   [batch, n_q_heads, width]; m in natural-log units of the scaled logit,
+ *                   relative to which O and l are accumulated (block-local maximum)
+ *       out         fp32  [batch, n_q_heads, head_dim]
+ */
+#ifndef PRR_H_
+#define PRR_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { PRR_OK = 0, PRR_E_INVALID = 1, PRR_E_UNSUPPORTED = 2, PRR_E_STATE = 3, PRR_E_CUDA = 4,
+       PRR_E_NOMEM = 5 };
+enum { PRR_BF16 = 0 };
+/* What happens to over-predicted blocks P\A at merge (Q7).  PRR_DROP: the output is attention
+ * over exactly A (BASELINE.json north_star).  PRR_RETAIN: P\A is "retained as additional
+ * low-priority context", the output is attention over A u P. */
+enum { PRR_DROP = 0, PRR_RETAIN = 1 };
+
+typedef struct prr_ctx prr_ctx; /* opaque, library-owned */
+
+typedef struct {
+  int32_t n_q_heads, n_kv_heads; /* n_q_heads % n_kv_heads == 0, group G = ratio, G <= 16 */
+  int32_t head_dim;              /* 64 or 128 */
+  int32_t max_batch;             /* >= 1 */
+  int32_t max_blocks_per_seq;    /* row stride of block_table / summaries / scores; <= 32768 */
+  int32_t n_layers;              /* EMA state is kept per (layer, sequence, KV head, block) */
+  int32_t kv_dtype;              /* PRR_BF16 */
+  int32_t overpredict_policy;    /* PRR_DROP | PRR_RETAIN */
+  float sm_scale;                /* softmax scale of the attention logits; 0 -> 1/sqrt(head_dim) */
+} prr_layout;
+
+typedef struct {
+  const void* k_pages;        /* dev bf16 */
+  const void* v_pages;        /* dev bf16 */
+  const int32_t* block_table; /* dev */
+  int32_t* seq_lens;          /* dev; read-only for every call except prr_append */
+  int32_t batch;              /* 1..max_batch */
+  int32_t layer;              /* 0..n_layers-1 */
+} prr_paged_kv;
+
+/* Problem statement (PAPER.md:109 Eq. 1, :135): block size, top-K of the DSA, speculation budget
+ * |P| <= budget = delta*K.  block_size in {16,32,64,128}; 1 <= K <= 512; 0 <= budget <= 1024. */
+int32_t prr_create(const prr_layout* layout, int32_t block_size, int32_t K, int32_t budget,
+                   prr_ctx** out);
+int32_t prr_destroy(prr_ctx* ctx);
+/* Text of the last error of this ctx (or of the last failed prr_create if ctx == NULL). */
+const char* prr_last_error(const prr_ctx* ctx);
+const char* prr_version(void);
+
+/* --- cache maintenance (a0) ------------------------------------------------------------------ */
+
+/* Mean-pooled key summary of every block of every sequence ("compresses each block
+ * (e.g., mean)"): kbar = bf16_rne(exact mean over the valid tokens), Q2.  Also seeds the running
+ * sum of the open block that prr_append continues.  The prefill-side counterpart of prr_append. */
+int32_t prr_build_summaries(prr_ctx* ctx, const prr_paged_kv* kv, void* summaries /*dev bf16*/,
+                            void* stream);
+
+/* Append one token per sequence: writes k_new/v_new (dev bf16 [batch, n_kv_heads, head_dim]) at
+ * position seq_lens[b] of the paged cache (the page must already be mapped in block_table),
+ * refreshes the summary row of that block, then INCREMENTS seq_lens[b] on the device (Q10: the
+ * decode step that follows sees its own token).  k_pages/v_pages are written through the const
+ * pointers of `kv`. */
+int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* k_new, const void* v_new,
+                   void* summaries, void* stream);
+
+/* --- predictor ------------------------------------------------------------ */
+
+/* Set theta = (alpha, beta, gamma) of Eq. 2-3 for one (layer, sequence) without calibration.
+ * seq = -1: all sequences.  Enqueued on `stream`. */
+int32_t prr_set_ema_params(prr_ctx* ctx, int32_t layer, int32_t seq, double alpha, double beta,
+                           double gamma, void* stream);
+/* Forget the EMA state of a layer (no block has state; next prediction is empty). */
+int32_t prr_reset_ema(prr_ctx* ctx, int32_t layer, void* stream);
+
+/* Per-prompt calibration: simulate Eq. 2-3 over the prefill score trajectory
+ * for the 80 grid points (alpha {.2,.4,.6,.8} x beta {.1,..,.5} x gamma {0,.25,.5,.75}, alpha-major),
+ * score-weighted hit rate H (Eq. 4) with |P| = min(budget, #stateful), theta* = first argmax
+ * (Eq. 5), Q8.  prefill_scores: dev fp32 [n_kv_heads, T, N] (row phi = score vector at prefill
+ * token phi); n_valid: dev int32 [T] non-decreasing number of valid blocks per row, or NULL = N.
+ * Stores theta*, seeds the EMA state of (layer, seq) with the state after the last row and
+ * predicts the first decode step's P (Q5).  theta_out (host double[3]), H_out (host double),
+ * H_all_out (host double[80]) may be NULL; if any is given the call synchronises `stream`. */
+int32_t prr_calibrate(prr_ctx* ctx, int32_t layer, int32_t seq, const float* prefill_scores,
+                      int32_t T, int32_t N, const int32_t* n_valid, double* theta_out,
+                      double* H_out, double* H_all_out, void* stream);
+
+/* Eq. 2: predicted scores from the current state, P = top-min(budget, #stateful) blocks, ties ->
+ * lower index.  P_out dev int32 [batch, n_kv_heads, budget]; count_out dev [batch, n_kv_heads]
+ * or NULL. */
+int32_t prr_predict(prr_ctx* ctx, int32_t layer, int32_t batch, int32_t* P_out,
+                    int32_t* count_out, void* stream);
+/* Eq. 3 with this step's scores (dev fp32 [batch, n_kv_heads, max_blocks]); blocks seen for the
+ * first time get l = IS, v = 0.  Also refreshes the library's stored prediction
+ * for the next decode step of this layer.  n_blocks: dev int32 [batch]. */
+int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, const float* scores,
+                       const int32_t* n_blocks, void* stream);
+
+/* --- selection (a1, a2) ---------------------------------------------------------------------- */
+
+/* Block importance (PAPER.md:66 compressed attention; group aggregated as in A.1 PAPER.md:372):
+ * IS[b,h,i] = fp32( (sum_{g in group h} sum_j q[b,g,j] kbar[b,h,i,j]) / (G sqrt(head_dim)) ),
+ * accumulated exactly (fp64 over exact bf16 products), rounded once, -0 -> +0 (Q1).  Writes the
+ * first ceil(seq_len/block_size) entries of each row. */
+int32_t prr_score(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                  float* scores_out, void* stream);
+/* Top-k of the first n_blocks[b] scores of each (b, KV head) row (row stride max_blocks_per_seq);
+ * order (value desc, index asc), selects min(k, n); idx_out dev int32 [batch, n_kv_heads, k]
+ * ascending, -1 padded; count_out dev [batch, n_kv_heads] or NULL.  1 <= k <= 1024. */
+int32_t prr_topk(prr_ctx* ctx, const float* scores, const int32_t* n_blocks, int32_t batch,
+                 int32_t k, int32_t* idx_out, int32_t* count_out, void* stream);
+
+/* --- attention (a4-a7) ----------------------------------------------------------------------- */
+
+/* Per-block partial states (the forward also writes l and m) for every block of
+ * the list P (dev int32 [batch, n_kv_heads, budget], -1 padded) and every query head:
+ * m_p = max_j s_j, l_p = sum_j e^{s_j - m_p}, O_p = sum_j e^{s_j - m_p} v_j, s_j = sm_scale q.k_j,
+ * tokens >= seq_len masked.  Slots holding -1 are left untouched. */
+int32_t prr_speculate(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* P,
+                      float* O_part, float* m_part, float* l_part, void* stream);
+/* Incremental repair (Eq. 6-8): given the true set A (dev int32 [batch,
+ * n_kv_heads, K]), the predicted set P and its partial states, attends only to M = A\P and folds
+ * hits u M (PRR_DROP) or P u M (PRR_RETAIN) in ascending block order into out; m_out/l_out (dev
+ * fp32 [batch, n_q_heads], natural-log max and denominator of the final state) may be NULL. */
+int32_t prr_repair(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* A,
+                   const int32_t* P, const float* O_part, const float* m_part,
+                   const float* l_part, float* out, float* m_out, float* l_out, void* stream);
+
+/* Sequential select-then-attend (the serial DSA PRR is compared with): score ->
+ * top-K -> attention over A, one stream.  Updates the EMA state like prr_decode_step. */
+int32_t prr_attend(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                   float* out, void* stream);
+/* One PRR layer-step (Fig. 1): speculative attention over the stored prediction P
+ * on a second stream, concurrently score -> top-K -> diff -> repair of A\P, then merge; EMA update
+ * and the next step's prediction run off the critical path.  Call prr_append first. */
+int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                        float* out, void* stream);
+/* prr_append + prr_decode_step with HOST q/k_new/v_new/out (pinned or pageable): copies the
+ * inputs to library staging buffers, runs the step, copies out back and synchronises. */
+int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_host,
+                             const void* k_new_host, const void* v_new_host, void* summaries,
+                             float* out_host, void* stream);
+
+/* --- introspection --------------------------------------------------------------------------- */
+
+/* Block sets of the last step of `layer` (any of the dev outputs may be NULL): A [batch,n_kv,K],
+ * P [batch,n_kv,budget] (the prediction that step used), M [batch,n_kv,K], counts
+ * [batch,n_kv,3] = |A|, |P|, |M|. */
+int32_t prr_get_sets(prr_ctx* ctx, int32_t layer, int32_t batch, int32_t* A, int32_t* P,
+                     int32_t* M, int32_t* counts, void* stream);
+/* Last scores of `layer`: dev fp32 [batch, n_kv_heads, max_blocks_per_seq]. */
+int32_t prr_get_scores(prr_ctx* ctx, int32_t layer, int32_t batch, float* scores, void* stream);
+/* EMA state of one (layer, seq): dev double [n_kv_heads, max_blocks] each, n_state dev int32
+ * [n_kv_heads], theta host double[3] (any may be NULL; theta synchronises). */
+int32_t prr_get_ema(prr_ctx* ctx, int32_t layer, int32_t seq, double* level, double* trend,
+                    int32_t* n_state, double* theta, void* stream);
+/* Cumulative counters since create / last reset: host int64[4] = sum|A|, sum|A n P|, sum|M|,
+ * sum|P| over all (layer, seq, KV head, step).  Synchronises `stream`.  reset != 0 clears them. */
+int32_t prr_get_stats(prr_ctx* ctx, int64_t* stats_out, int32_t reset, void* stream);
+/* Number of kernels this ctx has launched (or captured) so far. */
+int64_t prr_launch_count(const prr_ctx* ctx);
+
+/* --- CUDA-graph helpers (so callers need no CUDA runtime of their own) ------------------------ */
+typedef struct prr_graph prr_graph;
+int32_t prr_graph_begin(prr_ctx* ctx, void* stream);               /* start capturing `stream` */
+int32_t prr_graph_end(prr_ctx* ctx, void* stream, prr_graph** out); /* end capture, instantiate */
+int32_t prr_graph_launch(prr_graph* g, void* stream);
+int32_t prr_graph_destroy(prr_graph* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PRR_H_ */

@@ -1,0 +1,579 @@
+// C-ABI entry points of libprr (include/prr.h): argument validation, state allocation and the
+// two-stream, event-ordered orchestration of one PRR layer-step (Fig. 1, :38-42).
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "prr_internal.h"
+
+using namespace prr;
+
+static thread_local std::string g_create_err;
+
+#define PRR_FAIL(ctx, code, ...)                      \
+  do {                                                \
+    char _b[512];                                     \
+    snprintf(_b, sizeof(_b), __VA_ARGS__);            \
+    if (ctx) (ctx)->err = _b; else g_create_err = _b; \
+    return (code);                                    \
+  } while (0)
+
+#define PRR_CUDA(ctx, expr)                                                            \
+  do {                                                                                 \
+    cudaError_t _e = (expr);                                                           \
+    if (_e != cudaSuccess) PRR_FAIL(ctx, PRR_E_CUDA, "%s: %s", #expr, cudaGetErrorString(_e)); \
+  } while (0)
+
+static int check_launch(prr_ctx* c, const char* what) {
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    PRR_FAIL(c, PRR_E_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  }
+  return PRR_OK;
+}
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <typename T>
+static cudaError_t dalloc(prr_ctx* c, T** p, size_t n, bool zero = true) {
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, n * sizeof(T) + 16);
+  if (e != cudaSuccess) return e;
+  c->allocs.push_back(q);
+  if (zero) e = cudaMemset(q, 0, n * sizeof(T) + 16);
+  *p = reinterpret_cast<T*>(q);
+  return e;
+}
+
+extern "C" const char* prr_version(void) { return "prr-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* prr_last_error(const prr_ctx* ctx) {
+  return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" int64_t prr_launch_count(const prr_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t K, int32_t budget,
+                              prr_ctx** out) {
+  prr_ctx* none = nullptr;
+  if (!lay || !out) PRR_FAIL(none, PRR_E_INVALID, "prr_create: null argument");
+  *out = nullptr;
+  if (lay->n_q_heads <= 0 || lay->n_kv_heads <= 0 || lay->n_q_heads % lay->n_kv_heads)
+    PRR_FAIL(none, PRR_E_INVALID, "prr_create: n_q_heads must be a positive multiple of n_kv_heads");
+  if (lay->max_batch < 1 || lay->n_layers < 1 || lay->max_blocks_per_seq < 1)
+    PRR_FAIL(none, PRR_E_INVALID, "prr_create: max_batch, n_layers, max_blocks_per_seq must be >= 1");
+  if (K < 1 || budget < 0) PRR_FAIL(none, PRR_E_INVALID, "prr_create: need K >= 1 and budget >= 0");
+  if (lay->overpredict_policy != PRR_DROP && lay->overpredict_policy != PRR_RETAIN)
+    PRR_FAIL(none, PRR_E_INVALID, "prr_create: unknown overpredict_policy");
+  if (lay->sm_scale < 0.f || lay->sm_scale != lay->sm_scale)
+    PRR_FAIL(none, PRR_E_INVALID, "prr_create: sm_scale must be >= 0");
+  const int G = lay->n_q_heads / lay->n_kv_heads;
+  if (lay->head_dim != 64 && lay->head_dim != 128)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: head_dim must be 64 or 128");
+  if (block_size != 16 && block_size != 32 && block_size != 64 && block_size != 128)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: block_size must be 16, 32, 64 or 128");
+  if (G > 16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: GQA group > 16 unsupported");
+  if (lay->kv_dtype != PRR_BF16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: kv_dtype must be PRR_BF16");
+  if (lay->max_blocks_per_seq > 32768 || K > 512 || budget > 1024)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: max_blocks_per_seq <= 32768, K <= 512, budget <= 1024");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    PRR_FAIL(none, PRR_E_CUDA, "prr_create: no CUDA device (this library has no CPU fallback)");
+  }
+  prr_ctx* c = new prr_ctx();
+  c->lay = *lay;
+  c->bs = block_size; c->K = K; c->Bud = budget; c->G = G; c->D = lay->head_dim;
+  c->Hq = lay->n_q_heads; c->Hkv = lay->n_kv_heads; c->MB = lay->max_blocks_per_seq;
+  c->NL = lay->n_layers; c->maxB = lay->max_batch;
+  c->sm_scale = lay->sm_scale > 0.f ? lay->sm_scale : (float)(1.0 / std::sqrt((double)c->D));
+  c->score_c = 1.0 / ((double)G * std::sqrt((double)c->D));
+
+  const size_t rows = (size_t)c->NL * c->maxB * c->Hkv;
+  const size_t srows = (size_t)c->maxB * c->Hkv;
+  cudaError_t e = cudaSuccess;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  A(dalloc(c, &c->ema_l, rows * c->MB));
+  A(dalloc(c, &c->ema_v, rows * c->MB));
+  A(dalloc(c, &c->n_state, rows));
+  A(dalloc(c, &c->theta, (size_t)c->NL * c->maxB * 3));
+  A(dalloc(c, &c->open_sum, rows * c->D));
+  A(dalloc(c, &c->scores, rows * c->MB));
+  A(dalloc(c, &c->setA, rows * c->K));
+  A(dalloc(c, &c->setM, rows * c->K));
+  A(dalloc(c, &c->P_next, rows * (size_t)(c->Bud + 1)));
+  A(dalloc(c, &c->P_used, rows * (size_t)(c->Bud + 1)));
+  A(dalloc(c, &c->counts, rows * 3));
+  A(dalloc(c, &c->merge_src, srows * (c->Bud + c->K)));
+  A(dalloc(c, &c->merge_n, srows));
+  A(dalloc(c, &c->nblk, (size_t)c->maxB));
+  const size_t qrows = (size_t)c->maxB * c->Hq;
+  A(dalloc(c, &c->O_spec, qrows * (size_t)(c->Bud + 1) * c->D, false));
+  A(dalloc(c, &c->m_spec, qrows * (size_t)(c->Bud + 1), false));
+  A(dalloc(c, &c->l_spec, qrows * (size_t)(c->Bud + 1), false));
+  A(dalloc(c, &c->O_rep, qrows * c->K * c->D, false));
+  A(dalloc(c, &c->m_rep, qrows * c->K, false));
+  A(dalloc(c, &c->l_rep, qrows * c->K, false));
+  A(dalloc(c, &c->stats, (size_t)4));
+  A(dalloc(c, &c->cal_acc, (size_t)2 * 80 * c->Hkv + 80 + 2));
+  uint16_t *sq = nullptr, *sk = nullptr, *sv = nullptr;
+  A(dalloc(c, &sq, qrows * c->D));
+  A(dalloc(c, &sk, srows * c->D));
+  A(dalloc(c, &sv, srows * c->D));
+  A(dalloc(c, &c->st_out, qrows * c->D));
+  c->st_q = sq; c->st_k = sk; c->st_v = sv;
+  if (e == cudaSuccess) {
+    // P lists start empty (-1); theta defaults to (1, 1, 0): "reuse the last step's top-K" (S1)
+    e = cudaMemset(c->P_next, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->P_used, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
+    std::vector<double> th((size_t)c->NL * c->maxB * 3);
+    for (size_t i = 0; i < th.size(); i += 3) { th[i] = 1.0; th[i + 1] = 1.0; th[i + 2] = 0.0; }
+    if (e == cudaSuccess) e = cudaMemcpy(c->theta, th.data(), th.size() * sizeof(double), cudaMemcpyHostToDevice);
+  }
+  A(cudaStreamCreateWithFlags(&c->side_spec, cudaStreamNonBlocking));
+  A(cudaStreamCreateWithFlags(&c->side_ema, cudaStreamNonBlocking));
+  A(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+  A(cudaEventCreateWithFlags(&c->ev_spec, cudaEventDisableTiming));
+  A(cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
+  c->ev_upd.assign(c->NL, nullptr);
+  c->upd_pending.assign(c->NL, 0);
+  for (int l = 0; l < c->NL; ++l) A(cudaEventCreateWithFlags(&c->ev_upd[l], cudaEventDisableTiming));
+  if (e != cudaSuccess) {
+    g_create_err = std::string("prr_create: ") + cudaGetErrorString(e);
+    const bool nomem = e == cudaErrorMemoryAllocation;
+    cudaGetLastError();
+    prr_destroy(c);
+    return nomem ? PRR_E_NOMEM : PRR_E_CUDA;
+  }
+  *out = c;
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_destroy(prr_ctx* c) {
+  if (!c) return PRR_E_INVALID;
+  cudaDeviceSynchronize();
+  for (void* p : c->allocs) cudaFree(p);
+  if (c->cal_state) cudaFree(c->cal_state);
+  if (c->cal_mask) cudaFree(c->cal_mask);
+  if (c->cal_den) cudaFree(c->cal_den);
+  if (c->side_spec) cudaStreamDestroy(c->side_spec);
+  if (c->side_ema) cudaStreamDestroy(c->side_ema);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_spec) cudaEventDestroy(c->ev_spec);
+  if (c->ev_sel) cudaEventDestroy(c->ev_sel);
+  for (cudaEvent_t ev : c->ev_upd) if (ev) cudaEventDestroy(ev);
+  cudaGetLastError();
+  delete c;
+  return PRR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+static int check_kv(prr_ctx* c, const prr_paged_kv* kv, const char* fn) {
+  if (!c) return PRR_E_INVALID;
+  if (!kv) PRR_FAIL(c, PRR_E_INVALID, "%s: null prr_paged_kv", fn);
+  if (!kv->k_pages || !kv->v_pages || !kv->block_table || !kv->seq_lens)
+    PRR_FAIL(c, PRR_E_INVALID, "%s: null pointer in prr_paged_kv", fn);
+  if (!aligned16(kv->k_pages) || !aligned16(kv->v_pages))
+    PRR_FAIL(c, PRR_E_INVALID, "%s: k_pages / v_pages must be 16-byte aligned", fn);
+  if (kv->batch < 1 || kv->batch > c->maxB) PRR_FAIL(c, PRR_E_INVALID, "%s: batch out of range", fn);
+  if (kv->layer < 0 || kv->layer >= c->NL) PRR_FAIL(c, PRR_E_INVALID, "%s: layer out of range", fn);
+  return PRR_OK;
+}
+#define CHECK_KV(fn) do { int _r = check_kv(ctx, kv, fn); if (_r) return _r; } while (0)
+#define CHECK_PTR(p, fn) do { if (!(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: null %s", fn, #p); \
+    if (!aligned16(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: %s must be 16-byte aligned", fn, #p); } while (0)
+
+static size_t layer_rows(const prr_ctx* c, int layer) { return (size_t)layer * c->maxB * c->Hkv; }
+
+// Make `s` wait for every EMA update still running on the side stream.
+static void join_updates(prr_ctx* c, cudaStream_t s) {
+  for (int l = 0; l < c->NL; ++l)
+    if (c->upd_pending[l]) { cudaStreamWaitEvent(s, c->ev_upd[l], 0); c->upd_pending[l] = 0; }
+}
+static void join_layer(prr_ctx* c, int layer, cudaStream_t s) {
+  if (c->upd_pending[layer]) { cudaStreamWaitEvent(s, c->ev_upd[layer], 0); c->upd_pending[layer] = 0; }
+}
+
+extern "C" int32_t prr_build_summaries(prr_ctx* ctx, const prr_paged_kv* kv, void* summaries, void* stream) {
+  CHECK_KV("prr_build_summaries");
+  CHECK_PTR(summaries, "prr_build_summaries");
+  launch_build_summaries(ctx, kv, summaries, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_build_summaries");
+}
+
+extern "C" int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* k_new, const void* v_new,
+                              void* summaries, void* stream) {
+  CHECK_KV("prr_append");
+  CHECK_PTR(k_new, "prr_append"); CHECK_PTR(v_new, "prr_append"); CHECK_PTR(summaries, "prr_append");
+  launch_append(ctx, kv, k_new, v_new, summaries, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_append");
+}
+
+// ---------------------------------------------------------------------------------------------
+__global__ void k_set_theta(double* theta, int n, double a, double b, double g) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { theta[i * 3] = a; theta[i * 3 + 1] = b; theta[i * 3 + 2] = g; }
+}
+__global__ void k_fill_i32(int32_t* p, size_t n, int32_t v) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
+}
+
+extern "C" int32_t prr_set_ema_params(prr_ctx* ctx, int32_t layer, int32_t seq, double alpha, double beta,
+                                      double gamma, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || seq < -1 || seq >= ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_ema_params: layer/seq out of range");
+  if (!(alpha > 0.0 && alpha <= 1.0 && beta > 0.0 && beta <= 1.0 && gamma >= 0.0 && gamma <= 1.0))
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_ema_params: need alpha,beta in (0,1], gamma in [0,1] (PAPER.md:149,156)");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  const int n = seq < 0 ? ctx->maxB : 1;
+  double* th = ctx->theta + ((size_t)layer * ctx->maxB + (seq < 0 ? 0 : seq)) * 3;
+  k_set_theta<<<(n + 63) / 64, 64, 0, s>>>(th, n, alpha, beta, gamma);
+  ctx->launches++;
+  return check_launch(ctx, "prr_set_ema_params");
+}
+
+extern "C" int32_t prr_reset_ema(prr_ctx* ctx, int32_t layer, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL) PRR_FAIL(ctx, PRR_E_INVALID, "prr_reset_ema: layer out of range");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  const size_t r = layer_rows(ctx, layer), n = (size_t)ctx->maxB * ctx->Hkv;
+  PRR_CUDA(ctx, cudaMemsetAsync(ctx->n_state + r, 0, n * sizeof(int32_t), s));
+  if (ctx->Bud > 0)
+    PRR_CUDA(ctx, cudaMemsetAsync(ctx->P_next + r * ctx->Bud, 0xff, n * ctx->Bud * sizeof(int32_t), s));
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_calibrate(prr_ctx* ctx, int32_t layer, int32_t seq, const float* prefill_scores,
+                                 int32_t T, int32_t N, const int32_t* n_valid, double* theta_out,
+                                 double* H_out, double* H_all_out, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || seq < 0 || seq >= ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_calibrate: layer/seq out of range");
+  if (!prefill_scores) PRR_FAIL(ctx, PRR_E_INVALID, "prr_calibrate: null prefill_scores");
+  if (T < 1 || N < 1 || N > ctx->MB) PRR_FAIL(ctx, PRR_E_INVALID, "prr_calibrate: need T >= 1 and 1 <= N <= max_blocks_per_seq");
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(s, &cap);
+  if (cap != cudaStreamCaptureStatusNone) PRR_FAIL(ctx, PRR_E_STATE, "prr_calibrate: cannot run inside a stream capture");
+  join_layer(ctx, layer, s);
+  int r = launch_calibrate(ctx, layer, seq, prefill_scores, T, N, n_valid, s);
+  if (r) return r;
+  if ((r = check_launch(ctx, "prr_calibrate"))) return r;
+  if (ctx->Bud > 0) {  // first decode step's prediction (Q5)
+    EmaArgs e{};
+    e.layer = layer; e.batch = 1; e.seq0 = seq;
+    const size_t rows = layer_rows(ctx, layer) + (size_t)seq * ctx->Hkv;
+    e.P_out = ctx->P_next + rows * ctx->Bud;
+    launch_ema(ctx, e, s);
+    if ((r = check_launch(ctx, "prr_calibrate(predict)"))) return r;
+  }
+  if (theta_out || H_out || H_all_out) {
+    double H[80];
+    int32_t best = 0;
+    double* dH = ctx->cal_acc + 2 * 80 * ctx->Hkv;
+    PRR_CUDA(ctx, cudaMemcpyAsync(H, dH, sizeof(H), cudaMemcpyDeviceToHost, s));
+    PRR_CUDA(ctx, cudaMemcpyAsync(&best, dH + 80, sizeof(best), cudaMemcpyDeviceToHost, s));
+    double th[3];
+    PRR_CUDA(ctx, cudaMemcpyAsync(th, ctx->theta + ((size_t)layer * ctx->maxB + seq) * 3, sizeof(th),
+                                  cudaMemcpyDeviceToHost, s));
+    PRR_CUDA(ctx, cudaStreamSynchronize(s));
+    if (theta_out) memcpy(theta_out, th, sizeof(th));
+    if (H_out) *H_out = H[best];
+    if (H_all_out) memcpy(H_all_out, H, sizeof(H));
+  }
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_predict(prr_ctx* ctx, int32_t layer, int32_t batch, int32_t* P_out,
+                               int32_t* count_out, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || batch < 1 || batch > ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_predict: layer/batch out of range");
+  if (!P_out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_predict: null P_out");
+  if (ctx->Bud < 1) PRR_FAIL(ctx, PRR_E_STATE, "prr_predict: ctx was created with budget 0");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  EmaArgs e{};
+  e.layer = layer; e.batch = batch; e.seq0 = 0;
+  e.P_out = P_out; e.P_count = count_out;
+  launch_ema(ctx, e, s);
+  return check_launch(ctx, "prr_predict");
+}
+
+extern "C" int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, const float* scores,
+                                  const int32_t* n_blocks, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || batch < 1 || batch > ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_ema_update: layer/batch out of range");
+  if (!scores || !n_blocks) PRR_FAIL(ctx, PRR_E_INVALID, "prr_ema_update: null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  EmaArgs e{};
+  e.layer = layer; e.batch = batch; e.seq0 = 0;
+  e.scores = scores; e.n_blocks = n_blocks;
+  e.P_out = ctx->P_next + layer_rows(ctx, layer) * ctx->Bud;
+  launch_ema(ctx, e, s);
+  return check_launch(ctx, "prr_ema_update");
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int32_t prr_score(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                             float* scores_out, void* stream) {
+  CHECK_KV("prr_score");
+  CHECK_PTR(q, "prr_score"); CHECK_PTR(summaries, "prr_score");
+  if (!scores_out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_score: null scores_out");
+  launch_score(ctx, kv, q, summaries, scores_out, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_score");
+}
+
+extern "C" int32_t prr_topk(prr_ctx* ctx, const float* scores, const int32_t* n_blocks, int32_t batch,
+                            int32_t k, int32_t* idx_out, int32_t* count_out, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (!scores || !n_blocks || !idx_out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_topk: null argument");
+  if (batch < 1 || batch > ctx->maxB || k < 1 || k > 1024)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_topk: need 1 <= batch <= max_batch, 1 <= k <= 1024");
+  SelectArgs a{};
+  a.scores = scores; a.row_stride = ctx->MB; a.n_blocks = n_blocks; a.bs = ctx->bs;
+  a.batch = batch; a.Hkv = ctx->Hkv; a.k = k; a.A_out = idx_out; a.A_count = count_out;
+  launch_select(ctx, a, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_topk");
+}
+
+extern "C" int32_t prr_speculate(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* P,
+                                 float* O_part, float* m_part, float* l_part, void* stream) {
+  CHECK_KV("prr_speculate");
+  CHECK_PTR(q, "prr_speculate");
+  if (!P || !O_part || !m_part || !l_part) PRR_FAIL(ctx, PRR_E_INVALID, "prr_speculate: null argument");
+  if (ctx->Bud < 1) PRR_FAIL(ctx, PRR_E_STATE, "prr_speculate: ctx was created with budget 0");
+  launch_partial(ctx, kv, q, P, ctx->Bud, O_part, m_part, l_part, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_speculate");
+}
+
+extern "C" int32_t prr_repair(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* A,
+                              const int32_t* P, const float* O_part, const float* m_part,
+                              const float* l_part, float* out, float* m_out, float* l_out, void* stream) {
+  CHECK_KV("prr_repair");
+  CHECK_PTR(q, "prr_repair");
+  if (!A || !out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_repair: null argument");
+  if (P && (!O_part || !m_part || !l_part)) PRR_FAIL(ctx, PRR_E_INVALID, "prr_repair: P given without its partial states");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t r = layer_rows(ctx, kv->layer);
+  SelectArgs a{};
+  a.scores = nullptr; a.row_stride = ctx->MB; a.seq_lens = kv->seq_lens; a.bs = ctx->bs;
+  a.batch = kv->batch; a.Hkv = ctx->Hkv; a.k = ctx->K;
+  a.A_out = const_cast<int32_t*>(A);  // read-only in this mode
+  a.P = P; a.Bud = ctx->Bud;
+  a.M_out = ctx->setM + r * ctx->K;
+  a.merge_src = ctx->merge_src; a.merge_n = ctx->merge_n;
+  a.counts = ctx->counts + r * 3;
+  a.retain = ctx->lay.overpredict_policy == PRR_RETAIN;
+  launch_select(ctx, a, s);
+  launch_partial(ctx, kv, q, a.M_out, ctx->K, ctx->O_rep, ctx->m_rep, ctx->l_rep, s);
+  launch_merge(ctx, kv->batch, ctx->merge_src, ctx->merge_n, O_part, m_part, l_part, ctx->Bud,
+               ctx->O_rep, ctx->m_rep, ctx->l_rep, ctx->K, out, m_out, l_out, s);
+  return check_launch(ctx, "prr_repair");
+}
+
+// ---------------------------------------------------------------------------------------------
+static void enqueue_ema(prr_ctx* c, const prr_paged_kv* kv, cudaStream_t main, bool wait_spec) {
+  // Off the critical path: Eq. 3 update with this step's scores, then the next step's P.  It must
+  // not overwrite P while the speculative launch and the diff still read it.
+  const size_t r = layer_rows(c, kv->layer);
+  cudaEventRecord(c->ev_sel, main);
+  cudaStreamWaitEvent(c->side_ema, c->ev_sel, 0);
+  if (wait_spec) cudaStreamWaitEvent(c->side_ema, c->ev_spec, 0);
+  EmaArgs e{};
+  e.layer = kv->layer; e.batch = kv->batch; e.seq0 = 0;
+  e.scores = c->scores + r * c->MB;
+  e.seq_lens = kv->seq_lens;
+  e.P_out = c->P_next + r * c->Bud;
+  e.P_save = c->Bud > 0 ? c->P_used + r * c->Bud : nullptr;
+  launch_ema(c, e, c->side_ema);
+  cudaEventRecord(c->ev_upd[kv->layer], c->side_ema);
+  c->upd_pending[kv->layer] = 1;
+}
+
+extern "C" int32_t prr_attend(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                              float* out, void* stream) {
+  CHECK_KV("prr_attend");
+  CHECK_PTR(q, "prr_attend"); CHECK_PTR(summaries, "prr_attend");
+  if (!out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_attend: null out");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t r = layer_rows(ctx, kv->layer);
+  join_layer(ctx, kv->layer, s);
+  float* sc = ctx->scores + r * ctx->MB;
+  launch_score(ctx, kv, q, summaries, sc, s);
+  SelectArgs a{};
+  a.scores = sc; a.row_stride = ctx->MB; a.seq_lens = kv->seq_lens; a.bs = ctx->bs;
+  a.batch = kv->batch; a.Hkv = ctx->Hkv; a.k = ctx->K;
+  a.A_out = ctx->setA + r * ctx->K;
+  a.P = nullptr; a.Bud = ctx->Bud;
+  a.M_out = ctx->setM + r * ctx->K;
+  a.merge_src = ctx->merge_src; a.merge_n = ctx->merge_n;
+  a.counts = ctx->counts + r * 3;
+  a.retain = 0;
+  launch_select(ctx, a, s);
+  enqueue_ema(ctx, kv, s, false);
+  launch_partial(ctx, kv, q, a.M_out, ctx->K, ctx->O_rep, ctx->m_rep, ctx->l_rep, s);
+  launch_merge(ctx, kv->batch, ctx->merge_src, ctx->merge_n, ctx->O_spec, ctx->m_spec, ctx->l_spec,
+               ctx->Bud, ctx->O_rep, ctx->m_rep, ctx->l_rep, ctx->K, out, nullptr, nullptr, s);
+  return check_launch(ctx, "prr_attend");
+}
+
+extern "C" int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
+                                   float* out, void* stream) {
+  CHECK_KV("prr_decode_step");
+  CHECK_PTR(q, "prr_decode_step"); CHECK_PTR(summaries, "prr_decode_step");
+  if (!out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_decode_step: null out");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t r = layer_rows(ctx, kv->layer);
+  const bool spec = ctx->Bud > 0;
+  join_layer(ctx, kv->layer, s);  // this layer's previous EMA update / prediction must be complete
+  const int32_t* P = spec ? ctx->P_next + r * ctx->Bud : nullptr;
+  if (spec) {
+    // speculation branch: attention over the predicted blocks while selection is in flight
+    cudaEventRecord(ctx->ev_fork, s);
+    cudaStreamWaitEvent(ctx->side_spec, ctx->ev_fork, 0);
+    launch_partial(ctx, kv, q, P, ctx->Bud, ctx->O_spec, ctx->m_spec, ctx->l_spec, ctx->side_spec);
+    cudaEventRecord(ctx->ev_spec, ctx->side_spec);
+  }
+  // selection branch (critical path): score -> top-K + diff -> repair partials of A\P
+  float* sc = ctx->scores + r * ctx->MB;
+  launch_score(ctx, kv, q, summaries, sc, s);
+  SelectArgs a{};
+  a.scores = sc; a.row_stride = ctx->MB; a.seq_lens = kv->seq_lens; a.bs = ctx->bs;
+  a.batch = kv->batch; a.Hkv = ctx->Hkv; a.k = ctx->K;
+  a.A_out = ctx->setA + r * ctx->K;
+  a.P = P; a.Bud = ctx->Bud;
+  a.M_out = ctx->setM + r * ctx->K;
+  a.merge_src = ctx->merge_src; a.merge_n = ctx->merge_n;
+  a.counts = ctx->counts + r * 3;
+  a.stats = ctx->stats;
+  a.retain = ctx->lay.overpredict_policy == PRR_RETAIN;
+  launch_select(ctx, a, s);
+  enqueue_ema(ctx, kv, s, spec);
+  launch_partial(ctx, kv, q, a.M_out, ctx->K, ctx->O_rep, ctx->m_rep, ctx->l_rep, s);
+  if (spec) cudaStreamWaitEvent(s, ctx->ev_spec, 0);  // join
+  launch_merge(ctx, kv->batch, ctx->merge_src, ctx->merge_n, ctx->O_spec, ctx->m_spec, ctx->l_spec,
+               ctx->Bud, ctx->O_rep, ctx->m_rep, ctx->l_rep, ctx->K, out, nullptr, nullptr, s);
+  return check_launch(ctx, "prr_decode_step");
+}
+
+extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_host,
+                                        const void* k_new_host, const void* v_new_host, void* summaries,
+                                        float* out_host, void* stream) {
+  CHECK_KV("prr_decode_step_host");
+  if (!q_host || !k_new_host || !v_new_host || !out_host || !summaries)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_decode_step_host: null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t qb = (size_t)kv->batch * ctx->Hq * ctx->D, kb = (size_t)kv->batch * ctx->Hkv * ctx->D;
+  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_q, q_host, qb * 2, cudaMemcpyHostToDevice, s));
+  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_k, k_new_host, kb * 2, cudaMemcpyHostToDevice, s));
+  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_v, v_new_host, kb * 2, cudaMemcpyHostToDevice, s));
+  int r = prr_append(ctx, kv, ctx->st_k, ctx->st_v, summaries, stream);
+  if (r) return r;
+  r = prr_decode_step(ctx, kv, ctx->st_q, summaries, ctx->st_out, stream);
+  if (r) return r;
+  PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));
+  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  return PRR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int32_t prr_get_sets(prr_ctx* ctx, int32_t layer, int32_t batch, int32_t* A, int32_t* P,
+                                int32_t* M, int32_t* counts, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || batch < 1 || batch > ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_get_sets: layer/batch out of range");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  const size_t r = layer_rows(ctx, layer), n = (size_t)batch * ctx->Hkv;
+  if (A) PRR_CUDA(ctx, cudaMemcpyAsync(A, ctx->setA + r * ctx->K, n * ctx->K * 4, cudaMemcpyDeviceToDevice, s));
+  if (M) PRR_CUDA(ctx, cudaMemcpyAsync(M, ctx->setM + r * ctx->K, n * ctx->K * 4, cudaMemcpyDeviceToDevice, s));
+  if (P && ctx->Bud > 0)
+    PRR_CUDA(ctx, cudaMemcpyAsync(P, ctx->P_used + r * ctx->Bud, n * ctx->Bud * 4, cudaMemcpyDeviceToDevice, s));
+  if (counts) PRR_CUDA(ctx, cudaMemcpyAsync(counts, ctx->counts + r * 3, n * 3 * 4, cudaMemcpyDeviceToDevice, s));
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_get_scores(prr_ctx* ctx, int32_t layer, int32_t batch, float* scores, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || batch < 1 || batch > ctx->maxB || !scores)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_get_scores: bad argument");
+  const size_t r = layer_rows(ctx, layer), n = (size_t)batch * ctx->Hkv * ctx->MB;
+  PRR_CUDA(ctx, cudaMemcpyAsync(scores, ctx->scores + r * ctx->MB, n * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_get_ema(prr_ctx* ctx, int32_t layer, int32_t seq, double* level, double* trend,
+                               int32_t* n_state, double* theta, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || seq < 0 || seq >= ctx->maxB)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_get_ema: layer/seq out of range");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  const size_t sq = (size_t)layer * ctx->maxB + seq, n = (size_t)ctx->Hkv * ctx->MB;
+  if (level) PRR_CUDA(ctx, cudaMemcpyAsync(level, ctx->ema_l + sq * n, n * 8, cudaMemcpyDeviceToDevice, s));
+  if (trend) PRR_CUDA(ctx, cudaMemcpyAsync(trend, ctx->ema_v + sq * n, n * 8, cudaMemcpyDeviceToDevice, s));
+  if (n_state) PRR_CUDA(ctx, cudaMemcpyAsync(n_state, ctx->n_state + sq * ctx->Hkv, ctx->Hkv * 4, cudaMemcpyDeviceToDevice, s));
+  if (theta) {
+    PRR_CUDA(ctx, cudaMemcpyAsync(theta, ctx->theta + sq * 3, 24, cudaMemcpyDeviceToHost, s));
+    PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  }
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_get_stats(prr_ctx* ctx, int64_t* stats_out, int32_t reset, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  join_updates(ctx, s);
+  if (stats_out) PRR_CUDA(ctx, cudaMemcpyAsync(stats_out, ctx->stats, 32, cudaMemcpyDeviceToHost, s));
+  if (reset) PRR_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, 32, s));
+  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  return PRR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+extern "C" int32_t prr_graph_begin(prr_ctx* ctx, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  join_updates(ctx, s);  // side work issued before the capture must not be waited on inside it
+  PRR_CUDA(ctx, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_graph_end(prr_ctx* ctx, void* stream, prr_graph** out) {
+  if (!ctx || !out) return PRR_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  join_updates(ctx, s);  // every forked branch rejoins the origin stream before the capture ends
+  prr_graph* g = new prr_graph();
+  cudaError_t e = cudaStreamEndCapture(s, &g->graph);
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+  if (e != cudaSuccess) {
+    if (g->graph) cudaGraphDestroy(g->graph);
+    delete g;
+    cudaGetLastError();
+    PRR_FAIL(ctx, PRR_E_CUDA, "prr_graph_end: %s", cudaGetErrorString(e));
+  }
+  *out = g;
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_graph_launch(prr_graph* g, void* stream) {
+  if (!g || !g->exec) return PRR_E_INVALID;
+  return cudaGraphLaunch(g->exec, (cudaStream_t)stream) == cudaSuccess ? PRR_OK : PRR_E_CUDA;
+}
+
+extern "C" int32_t prr_graph_destroy(prr_graph* g) {
+  if (!g) return PRR_E_INVALID;
+  if (g->exec) cudaGraphExecDestroy(g->exec);
+  if (g->graph) cudaGraphDestroy(g->graph);
+  delete g;
+  return PRR_OK;
+}

@@ -1,0 +1,104 @@
+// Host-side internals of libprr: the context and the kernel launchers (one per .cu file).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/prr.h"
+
+struct prr_ctx {
+  prr_layout lay;
+  int bs, K, Bud, G, D, Hq, Hkv, MB, NL, maxB;
+  float sm_scale;
+  double score_c;  // 1 / (G sqrt(d)), computed once on the host in fp64
+
+  // ---- per-layer state, device ----
+  double* ema_l = nullptr;    // [NL, maxB, Hkv, MB]
+  double* ema_v = nullptr;    // [NL, maxB, Hkv, MB]
+  int32_t* n_state = nullptr; // [NL, maxB, Hkv]
+  double* theta = nullptr;    // [NL, maxB, 3]
+  double* open_sum = nullptr; // [NL, maxB, Hkv, D] running fp64 sum of the open block's keys
+  float* scores = nullptr;    // [NL, maxB, Hkv, MB]
+  int32_t* setA = nullptr;    // [NL, maxB, Hkv, K]
+  int32_t* setM = nullptr;    // [NL, maxB, Hkv, K]
+  int32_t* P_next = nullptr;  // [NL, maxB, Hkv, Bud]  prediction for the next step of the layer
+  int32_t* P_used = nullptr;  // [NL, maxB, Hkv, Bud]  prediction the last step used
+  int32_t* counts = nullptr;  // [NL, maxB, Hkv, 3]    |A|, |P|, |M| of the last step
+  // ---- per-step scratch, device (shared by all layers; steps are ordered on the main stream) ----
+  int32_t* merge_src = nullptr; // [maxB, Hkv, Bud+K] slot codes, ascending block order
+  int32_t* merge_n = nullptr;   // [maxB, Hkv]
+  int32_t* nblk = nullptr;      // [maxB] scratch for n_blocks derived from seq_lens
+  float *O_spec = nullptr, *m_spec = nullptr, *l_spec = nullptr; // [maxB, Hq, Bud, D] / [.., Bud]
+  float *O_rep = nullptr, *m_rep = nullptr, *l_rep = nullptr;    // [maxB, Hq, K, D]   / [.., K]
+  unsigned long long* stats = nullptr; // [4]
+  // ---- calibration scratch (allocated on first prr_calibrate) ----
+  double* cal_state = nullptr; size_t cal_state_elems = 0; // [80, Hkv, N, 2]
+  uint32_t* cal_mask = nullptr; size_t cal_mask_words = 0; // [Hkv, T, ceil(N/32)]
+  double* cal_den = nullptr; size_t cal_den_elems = 0;     // [Hkv, T]
+  double* cal_acc = nullptr;  // [80, Hkv] + counts [80, Hkv] + H [80] + best[1]
+  // ---- host staging for prr_decode_step_host ----
+  void *st_q = nullptr, *st_k = nullptr, *st_v = nullptr; float* st_out = nullptr;
+
+  cudaStream_t side_spec = nullptr, side_ema = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_spec = nullptr, ev_sel = nullptr;
+  std::vector<cudaEvent_t> ev_upd; // per layer: EMA update of the last step of that layer done
+  std::vector<char> upd_pending;
+  std::vector<void*> allocs;
+  int64_t launches = 0;
+  std::string err;
+};
+
+struct prr_graph {
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+};
+
+namespace prr {
+
+// k_cache.cu
+void launch_build_summaries(prr_ctx* c, const prr_paged_kv* kv, void* summaries, cudaStream_t s);
+void launch_append(prr_ctx* c, const prr_paged_kv* kv, const void* k_new, const void* v_new,
+                   void* summaries, cudaStream_t s);
+void launch_nblocks(prr_ctx* c, const int32_t* seq_lens, int batch, int32_t* nblk, cudaStream_t s);
+// k_score.cu
+void launch_score(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries,
+                  float* scores, cudaStream_t s);
+// k_select.cu
+// Top-k of each row (+ optional diff against P and merge list).  n per row comes from
+// seq_lens (if non-null: ceil(len/bs)) else n_blocks.
+struct SelectArgs {
+  const float* scores; int row_stride;
+  const int32_t* seq_lens; const int32_t* n_blocks; int bs;
+  int batch, Hkv, k;
+  int32_t* A_out; int32_t* A_count;      // [rows,k], [rows] (count may be null)
+  const int32_t* P; int Bud;             // null -> empty prediction
+  int32_t* M_out;                        // [rows,k] or null
+  int32_t* merge_src; int32_t* merge_n;  // [rows,Bud+k], [rows] or null
+  int32_t* counts;                       // [rows,3] or null
+  unsigned long long* stats;             // [4] or null
+  int retain;
+};
+void launch_select(prr_ctx* c, const SelectArgs& a, cudaStream_t s);
+// EMA update (optional) + prediction of the next P.
+struct EmaArgs {
+  int layer, batch, seq0;                // rows cover sequences [seq0, seq0+batch)
+  const float* scores;                   // null -> predict only from the current state
+  const int32_t* seq_lens; const int32_t* n_blocks; // n per sequence when updating
+  int32_t* P_out; int32_t* P_count;      // [batch,Hkv,Bud], [batch,Hkv] or null
+  int32_t* P_save;                       // old contents of P_out copied here first, or null
+};
+void launch_ema(prr_ctx* c, const EmaArgs& a, cudaStream_t s);
+// k_attn.cu
+void launch_partial(prr_ctx* c, const prr_paged_kv* kv, const void* q, const int32_t* list,
+                    int width, float* O, float* m, float* l, cudaStream_t s);
+void launch_merge(prr_ctx* c, int batch, const int32_t* merge_src, const int32_t* merge_n,
+                  const float* O_spec, const float* m_spec, const float* l_spec, int w_spec,
+                  const float* O_rep, const float* m_rep, const float* l_rep, int w_rep,
+                  float* out, float* m_out, float* l_out, cudaStream_t s);
+// k_calib.cu
+int launch_calibrate(prr_ctx* c, int layer, int seq, const float* IS, int T, int N,
+                     const int32_t* n_valid, cudaStream_t s);
+
+}  // namespace prr

@@ -1,0 +1,391 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the oracle, element by element, on the
+same seeded inputs.  Integer / index work is compared bit-exactly; scores bit-exactly; attention
+outputs within the tolerance BASELINE.json states (harness.check_out)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import prr_oracle as O
+from paper_2606_30389_b200 import prr, synth
+import prr_harness as H
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+# small shapes that still span several tiles and ragged tails
+TINY = synth.CONFIGS["C0"].scaled(ctx_lo=700, ctx_hi=1000, B=3, T_cal=16, steps=8)          # d=64, bs=64, G=4
+T128 = synth.Config("T128", B=2, L=1, Hq=14, Hkv=2, d=128, ctx_lo=900, ctx_hi=1300, bs=32, K=8, Bud=11,
+                    rho=0.8, steps=8, T_cal=16)                                            # G=7, bs=32
+T16 = synth.Config("T16", B=2, L=1, Hq=4, Hkv=4, d=128, ctx_lo=300, ctx_hi=333, bs=16, K=6, Bud=9,
+                   rho=0.9, steps=20, T_cal=12)                                            # G=1, bs=16
+TB128 = synth.Config("TB128", B=1, L=1, Hq=16, Hkv=1, d=64, ctx_lo=2000, ctx_hi=2000, bs=128, K=5, Bud=7,
+                     rho=0.9, steps=6, T_cal=12)                                           # G=16, bs=128
+SHAPES = [TINY, T128, T16, TB128]
+
+
+def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None):
+    cfg = cfg if seed is None else cfg.scaled(seed=seed)
+    inp = synth.make_layer(cfg, 0, device=DEV, steps=steps)
+    gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget)
+    ol = H.oracle_layer(cfg, inp, policy=policy, budget=budget)
+    return cfg, inp, gl, ol
+
+
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_summaries_and_append_bit_exact(cfg):
+    cfg, inp, gl, ol = make(cfg)
+    torch.cuda.synchronize()
+    assert np.array_equal(synth.bits(gl.summ), ol.summ)
+    for t in range(cfg.steps):
+        gl.append(t)
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+    torch.cuda.synchronize()
+    assert np.array_equal(gl.seq_lens.cpu().numpy(), ol.lens)
+    assert np.array_equal(synth.bits(gl.summ), ol.summ)
+    for b in range(cfg.B):
+        nb = ol.n_blocks()[b]
+        pg = ol.table[b, :nb]
+        n_last = ol.lens[b] - (nb - 1) * cfg.bs
+        assert np.array_equal(synth.bits(gl.k_pages)[pg[:-1]], ol.k[pg[:-1]])
+        assert np.array_equal(synth.bits(gl.v_pages)[pg[-1], :, :n_last], ol.v[pg[-1], :, :n_last])
+
+
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_score_bit_exact(cfg):
+    cfg, inp, gl, ol = make(cfg)
+    sc = torch.full((cfg.B, cfg.Hkv, gl.MB), 7.0, dtype=torch.float32, device=DEV)
+    for t in range(3):
+        gl.ctx.score(gl.kv, inp.q_dec[t].contiguous(), gl.summ, sc)
+        torch.cuda.synchronize()
+        want = ol.scores(synth.bits(inp.q_dec[t]))
+        got = sc.cpu().numpy()
+        for b in range(cfg.B):
+            nb = ol.n_blocks()[b]
+            assert np.array_equal(got[b, :, :nb].view(np.uint32), want[b, :, :nb].view(np.uint32))
+            assert (got[b, :, nb:] == 7.0).all()          # rows beyond NB are not written
+
+
+@pytest.mark.parametrize("n,k", [(1, 1), (5, 8), (64, 8), (257, 64), (2048, 64), (4096, 128), (1000, 1000)])
+def test_topk_bit_exact_with_ties(n, k):
+    rng = np.random.default_rng(n + k)
+    Hkv, B, MB = 4, 3, 4100
+    ctx = prr.Context(4, Hkv, 64, 64, min(k, 512), 4, max_batch=B, max_blocks_per_seq=MB)
+    vals = rng.standard_normal((B, Hkv, MB)).astype(np.float32)
+    vals[0] = np.round(vals[0] * 2) / 2                       # heavy ties
+    vals[1, :, ::3] = 0.0
+    vals[1, :, 1::3] = -0.0                                   # +-0 mix
+    vals[2, 0] = 1.25                                         # all equal
+    vals[2, 1, : n // 2] = np.inf
+    nbs = np.array([n, max(1, n - 3), n], dtype=np.int32)
+    idx = torch.full((B, Hkv, k), -7, dtype=torch.int32, device=DEV)
+    cnt = torch.zeros(B, Hkv, dtype=torch.int32, device=DEV)
+    ctx.topk(torch.from_numpy(vals).to(DEV), torch.from_numpy(nbs).to(DEV), B, k, idx, cnt)
+    torch.cuda.synchronize()
+    got, gc = idx.cpu().numpy(), cnt.cpu().numpy()
+    for b in range(B):
+        for h in range(Hkv):
+            want = O.topk(vals[b, h, :nbs[b]], k)
+            assert gc[b, h] == len(want)
+            assert np.array_equal(got[b, h, :len(want)], want), (b, h)
+            assert (got[b, h, len(want):] == -1).all()
+
+
+@pytest.mark.parametrize("cfg", [TINY, T16], ids=lambda c: c.name)
+def test_ema_update_predict_bit_exact(cfg):
+    cfg, inp, gl, ol = make(cfg)
+    rng = np.random.default_rng(3)
+    theta = (0.6, 0.3, 0.75)
+    gl.ctx.set_ema_params(0, -1, *theta)
+    nb0 = ol.n_blocks()
+    P = torch.empty(cfg.B, cfg.Hkv, cfg.Bud, dtype=torch.int32, device=DEV)
+    Pc = torch.empty(cfg.B, cfg.Hkv, dtype=torch.int32, device=DEV)
+    L = torch.empty(cfg.Hkv, gl.MB, dtype=torch.float64, device=DEV)
+    V = torch.empty_like(L)
+    for step in range(6):
+        nb = np.minimum(nb0 - 3 + step, gl.MB).astype(np.int32)   # blocks enter over time
+        sc = (rng.standard_normal((cfg.B, cfg.Hkv, gl.MB)) * 0.07).astype(np.float32)
+        gl.ctx.predict(0, cfg.B, P, Pc)
+        torch.cuda.synchronize()
+        for b in range(cfg.B):
+            for h in range(cfg.Hkv):
+                want = O.ema_predict_set(ol.ema[b][h], theta[2], cfg.Bud)
+                assert Pc[b, h].item() == len(want)
+                assert np.array_equal(P[b, h, :len(want)].cpu().numpy(), want), (step, b, h)
+        gl.ctx.ema_update(0, cfg.B, torch.from_numpy(sc).to(DEV), torch.from_numpy(nb).to(DEV))
+        for b in range(cfg.B):
+            for h in range(cfg.Hkv):
+                O.ema_update(ol.ema[b][h], sc[b, h, :nb[b]], theta[0], theta[1])
+        for b in range(cfg.B):
+            gl.ctx.get_ema(0, b, L, V)
+            torch.cuda.synchronize()
+            for h in range(cfg.Hkv):
+                n = ol.ema[b][h].n
+                assert np.array_equal(L[h, :n].cpu().numpy(), ol.ema[b][h].l[:n])
+                assert np.array_equal(V[h, :n].cpu().numpy(), ol.ema[b][h].v[:n])
+
+
+@pytest.mark.parametrize("cfg", [TINY, T128], ids=lambda c: c.name)
+def test_calibrate_matches_oracle(cfg):
+    cfg, inp, gl, ol = make(cfg)
+    gres = gl.calibrate(inp.q_cal)
+    ores = ol.calibrate(synth.bits(inp.q_cal))
+    P = torch.empty(cfg.B, cfg.Hkv, cfg.Bud, dtype=torch.int32, device=DEV)
+    gl.ctx.predict(0, cfg.B, P)
+    torch.cuda.synchronize()
+    for b in range(cfg.B):
+        (theta, Hs, H_all), traj = gres[b]
+        otheta, oH, oH_all, oIS = ores[b]
+        assert np.array_equal(traj.cpu().numpy().view(np.uint32), oIS.view(np.uint32))
+        assert np.array_equal(np.array(H_all), oH_all), np.abs(np.array(H_all) - oH_all).max()
+        assert theta == otheta and Hs == oH
+        for h in range(cfg.Hkv):
+            want = O.ema_predict_set(ol.ema[b][h], otheta[2], cfg.Bud)
+            assert np.array_equal(H.unpad(P[b, h].cpu().numpy()), want)
+
+
+def test_calibrate_causal_staircase():
+    cfg, inp, gl, ol = make(TINY)
+    b = 1
+    nb = int(ol.n_blocks()[b])
+    traj = gl.trajectory(inp.q_cal, b).contiguous()
+    nv = np.minimum(np.arange(1, cfg.T_cal + 1) * 2, nb).astype(np.int32)
+    theta, Hs, H_all = gl.ctx.calibrate(0, b, traj, n_valid=torch.from_numpy(nv).to(DEV))
+    otheta, oH, ostates, oH_all = O.calibrate(traj.cpu().numpy(), cfg.K, cfg.Bud, nv)
+    assert np.array_equal(np.array(H_all), oH_all) and theta == otheta
+    ns = torch.empty(cfg.Hkv, dtype=torch.int32, device=DEV)
+    gl.ctx.get_ema(0, b, n_state=ns)
+    torch.cuda.synchronize()
+    assert ns.tolist() == [ostates[0].n] * cfg.Hkv
+
+
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_block_partials_against_eq6_8_states(cfg):
+    """prr_speculate: per-block (m, l, O) of an arbitrary list incl. the open block and -1 holes."""
+    cfg, inp, gl, ol = make(cfg)
+    gl.append(0); ol.append(synth.bits(inp.k_new[0]), synth.bits(inp.v_new[0]))   # open block is ragged
+    rng = np.random.default_rng(5)
+    nb = ol.n_blocks()
+    P = np.full((cfg.B, cfg.Hkv, cfg.Bud), -1, dtype=np.int32)
+    for b in range(cfg.B):
+        for h in range(cfg.Hkv):
+            pick = np.sort(rng.choice(nb[b] - 1, size=cfg.Bud - 3, replace=False))
+            P[b, h, :cfg.Bud - 3] = pick
+            P[b, h, cfg.Bud - 2] = nb[b] - 1                      # after a -1 hole: the open block
+    Op = torch.full((cfg.B, cfg.Hq, cfg.Bud, cfg.d), 9.0, dtype=torch.float32, device=DEV)
+    mp = torch.full((cfg.B, cfg.Hq, cfg.Bud), 9.0, dtype=torch.float32, device=DEV)
+    lp = torch.full((cfg.B, cfg.Hq, cfg.Bud), 9.0, dtype=torch.float32, device=DEV)
+    q = inp.q_dec[0].contiguous()
+    gl.ctx.speculate(gl.kv, q, torch.from_numpy(P).to(DEV), Op, mp, lp)
+    torch.cuda.synchronize()
+    Op, mp, lp = Op.cpu().numpy(), mp.cpu().numpy(), lp.cpu().numpy()
+    qb = synth.bits(q)
+    for b in range(cfg.B):
+        for h in range(cfg.Hkv):
+            for s in range(cfg.Bud):
+                for g in range(cfg.G):
+                    hq = h * cfg.G + g
+                    if P[b, h, s] < 0:
+                        assert (Op[b, hq, s] == 9.0).all() and mp[b, hq, s] == 9.0   # untouched
+                        continue
+                    st = O.fold(qb[b], ol.k, ol.v, ol.table[b], ol.lens[b],
+                                [[P[b, h, s]] if hh == h else [] for hh in range(cfg.Hkv)], cfg.bs)[hq]
+                    m, l, On = st
+                    assert abs(mp[b, hq, s] - m) <= 1e-5 * max(1.0, abs(m))
+                    assert abs(lp[b, hq, s] - l) <= 4e-3 * l
+                    H.check_out(Op[b, hq, s] / lp[b, hq, s], On, f"partial b{b} hq{hq} s{s}")
+
+
+@pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_repair_stage_matches_attention_over_true_set(cfg, policy):
+    cfg, inp, gl, ol = make(cfg, policy=policy)
+    rng = np.random.default_rng(6)
+    nb = ol.n_blocks()
+    A = np.full((cfg.B, cfg.Hkv, cfg.K), -1, dtype=np.int32)
+    P = np.full((cfg.B, cfg.Hkv, cfg.Bud), -1, dtype=np.int32)
+    for b in range(cfg.B):
+        for h in range(cfg.Hkv):
+            A[b, h] = np.sort(rng.choice(nb[b], size=cfg.K, replace=False))
+            npred = [cfg.Bud, 0, cfg.Bud - 2][(b + h) % 3]
+            keep = rng.choice(A[b, h], size=min(npred, cfg.K) // 2, replace=False)
+            rest = np.setdiff1d(np.arange(nb[b]), A[b, h])
+            extra = rng.choice(rest, size=npred - len(keep), replace=False) if npred else []
+            pp = np.sort(np.concatenate([keep, extra]).astype(np.int32))
+            P[b, h, :len(pp)] = pp
+    q = inp.q_dec[1].contiguous()
+    Op = torch.zeros(cfg.B, cfg.Hq, cfg.Bud, cfg.d, dtype=torch.float32, device=DEV)
+    mp = torch.zeros(cfg.B, cfg.Hq, cfg.Bud, dtype=torch.float32, device=DEV)
+    lp = torch.zeros_like(mp)
+    out = torch.zeros(cfg.B, cfg.Hq, cfg.d, dtype=torch.float32, device=DEV)
+    mo = torch.zeros(cfg.B, cfg.Hq, dtype=torch.float32, device=DEV)
+    lo = torch.zeros_like(mo)
+    Pd, Ad = torch.from_numpy(P).to(DEV), torch.from_numpy(A).to(DEV)
+    gl.ctx.speculate(gl.kv, q, Pd, Op, mp, lp)
+    gl.ctx.repair(gl.kv, q, Ad, Pd, Op, mp, lp, out, mo, lo)
+    torch.cuda.synchronize()
+    qb = synth.bits(q)
+    for b in range(cfg.B):
+        S = [np.union1d(A[b, h], H.unpad(P[b, h])) if policy == prr.RETAIN else A[b, h] for h in range(cfg.Hkv)]
+        want = O.attend(qb[b], ol.k, ol.v, ol.table[b], ol.lens[b], S, cfg.bs)
+        H.check_out(out[b].cpu().numpy(), want, f"repair b{b}")
+        st = O.fold(qb[b], ol.k, ol.v, ol.table[b], ol.lens[b], S, cfg.bs)
+        for hq in range(cfg.Hq):
+            assert abs(mo[b, hq].item() - st[hq][0]) <= 1e-5 * max(1.0, abs(st[hq][0]))
+            assert abs(lo[b, hq].item() - st[hq][1]) <= 4e-3 * st[hq][1]
+    _, _, M, cnt = gl.sets()
+    for b in range(cfg.B):
+        for h in range(cfg.Hkv):
+            assert np.array_equal(H.unpad(M[b, h]), np.setdiff1d(A[b, h], P[b, h]))
+
+
+def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True):
+    steps = cfg.steps if steps is None else steps
+    cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps)
+    twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget) if seq_check else None
+    if calibrate:
+        gres = gl.calibrate(inp.q_cal)
+        ores = ol.calibrate(synth.bits(inp.q_cal))
+        if twin:
+            twin.calibrate(inp.q_cal)
+        for b in range(cfg.B):
+            assert gres[b][0][0] == ores[b][0], "theta*"
+    worst = (0.0, 0.0)
+    hits = tot = 0
+    for t in range(steps):
+        gl.append(t)
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        out = gl.step(t)
+        torch.cuda.synchronize()
+        r = ol.step(synth.bits(inp.q_dec[t]))
+        sc = gl.scores()
+        for b in range(cfg.B):
+            nb = ol.n_blocks()[b]
+            assert np.array_equal(sc[b, :, :nb].view(np.uint32), r["scores"][b, :, :nb].view(np.uint32)), f"scores t{t}"
+        H.compare_sets(gl, r, f"t{t}")
+        e = H.check_out(out.cpu().numpy(), r["out"], f"out t{t}")
+        worst = (max(worst[0], e[0]), max(worst[1], e[1]))
+        if twin:   # the library's own sequential select-then-attend path
+            twin.append(t)
+            o2 = twin.step(t, sequential=True)
+            torch.cuda.synchronize()
+            if policy == prr.DROP:
+                assert (out - o2).abs().max().item() <= 1e-5, f"PRR vs sequential t{t}"
+        for b in range(cfg.B):
+            for h in range(cfg.Hkv):
+                hits += len(r["A"][b][h]) - len(r["M"][b][h]); tot += len(r["A"][b][h])
+    st = gl.ctx.get_stats()
+    assert st[0] == tot and st[1] == hits and st[2] == tot - hits
+    return worst, hits / max(tot, 1)
+
+
+@pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_decode_steps_small_shapes(cfg, policy):
+    run_decode(cfg, policy=policy)
+
+
+def test_decode_c0_full():
+    """BASELINE.json configs[0]: every one of the 32 steps, all outputs."""
+    worst, hit = run_decode(synth.CONFIGS["C0"])
+    assert hit > 0.5
+
+
+def test_decode_without_calibration_and_zero_budget():
+    run_decode(TINY, calibrate=False)                 # first step: no state -> P = {} -> repair all of A
+    run_decode(TINY, budget=0, seq_check=False)       # no speculation at all
+    run_decode(T16.scaled(K=40), steps=4)             # K > number of blocks
+
+
+def test_decode_c1_sampled_steps():
+    """BASELINE.json configs[1] at full size (32768 ctx, 512 blocks), first 12 steps."""
+    run_decode(synth.CONFIGS["C1"].scaled(T_cal=32), steps=12, seq_check=True)
+
+
+def test_decode_c2_full_size_sampled_steps():
+    """configs[2], the headline 128K case, at full size: 6 steps, every output compared."""
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=6)
+
+
+def test_decode_c4_full_size_sampled_steps():
+    """configs[4]: batch 4, GQA 7, block 32, 4096 blocks, K=128, budget 160, rho 0.7."""
+    worst, hit = run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=3, seq_check=False)
+
+
+def test_decode_c3_shape_two_layers():
+    """configs[3] shape (batch 16, ragged lengths in [16384, 32768]) on 2 of its 32 layers."""
+    cfg = synth.CONFIGS["C3"].scaled(T_cal=8)
+    steps = 3
+    MB = (cfg.ctx_hi + steps + cfg.bs - 1) // cfg.bs + 1
+    ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B, max_blocks_per_seq=MB,
+                      n_layers=2)
+    layers = []
+    for l in range(2):
+        inp = synth.make_layer(cfg, l, device=DEV, steps=steps)
+        gl = H.GpuLayer(cfg, inp, ctx=ctx, layer=l, n_layers=2)
+        ol = H.oracle_layer(cfg, inp)
+        gl.ctx.set_ema_params(l, -1, 0.6, 0.2, 0.5)
+        ol.theta = [(0.6, 0.2, 0.5)] * cfg.B
+        layers.append((inp, gl, ol))
+    for t in range(steps):
+        for inp, gl, ol in layers:          # layers interleave like a model's forward pass
+            gl.append(t)
+            gl.step(t)
+        torch.cuda.synchronize()
+        for inp, gl, ol in layers:          # every layer keeps its own out buffer
+            ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+            r = ol.step(synth.bits(inp.q_dec[t]))
+            H.compare_sets(gl, r, f"t{t} L{gl.layer}")
+            H.check_out(gl.out.cpu().numpy(), r["out"], f"C3 t{t} L{gl.layer}")
+
+
+def test_graph_replay_matches_eager():
+    cfg, inp, gl, ol = make(TINY)
+    _, _, g2, _ = make(TINY)
+    gl.calibrate(inp.q_cal); g2.calibrate(inp.q_cal)
+    outs_e = []
+    for t in range(4):
+        gl.append(t); outs_e.append(gl.step(t).clone())
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    outs_g = [torch.zeros_like(g2.out) for _ in range(4)]
+    with torch.cuda.stream(s):
+        g2.ctx.graph_begin(s)
+        for t in range(4):
+            g2.ctx.append(g2.kv, inp.k_new[t].contiguous(), inp.v_new[t].contiguous(), g2.summ, stream=s)
+            g2.ctx.decode_step(g2.kv, inp.q_dec[t].contiguous(), g2.summ, outs_g[t], stream=s)
+        graph = g2.ctx.graph_end(s)
+        graph.launch(s)
+    s.synchronize()
+    for t in range(4):
+        assert torch.equal(outs_e[t], outs_g[t]), t
+    assert g2.seq_lens.tolist() == gl.seq_lens.tolist()
+    graph.destroy()
+
+
+def test_host_buffer_step_matches_device_step():
+    cfg, inp, gl, ol = make(TINY)
+    _, _, g2, _ = make(TINY)
+    out_h = torch.zeros(cfg.B, cfg.Hq, cfg.d, dtype=torch.float32).pin_memory()
+    for t in range(3):
+        gl.append(t); o = gl.step(t)
+        g2.ctx.decode_step_host(g2.kv, inp.q_dec[t].cpu().contiguous().pin_memory(),
+                                inp.k_new[t].cpu().contiguous().pin_memory(),
+                                inp.v_new[t].cpu().contiguous().pin_memory(), g2.summ, out_h)
+        torch.cuda.synchronize()
+        assert torch.equal(o.cpu(), out_h)
+
+
+def test_errors_are_reported_not_raised_in_c():
+    with pytest.raises(prr.PrrError) as e:
+        prr.Context(30, 8, 128, 64, 8, 8)
+    assert e.value.code == prr.E_INVALID
+    with pytest.raises(prr.PrrError) as e:
+        prr.Context(32, 8, 96, 64, 8, 8)
+    assert e.value.code == prr.E_UNSUPPORTED
+    cfg, inp, gl, ol = make(TINY)
+    with pytest.raises(prr.PrrError) as e:
+        gl.ctx.score(gl.kv, None, gl.summ, gl.out)
+    assert e.value.code == prr.E_INVALID and "null" in str(e.value)
+    bad = gl.ctx.kv(gl.k_pages, gl.v_pages, inp.block_table, gl.seq_lens, layer=3)
+    with pytest.raises(prr.PrrError):
+        gl.ctx.decode_step(bad, inp.q_dec[0].contiguous(), gl.summ, gl.out)
