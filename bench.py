@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py — per-layer DSA decode critical path of PRR on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--layers R] [--impl reference]
+
+A "step" is ONE LAYER-STEP: one pass of the whole hot path (append + summary refresh, score, top-K,
+diff, EMA predict/update, speculative attention over P on a second stream, repair of A\\P, merge)
+for one layer of the named config.  R independent seeded layer caches are visited round-robin, as a
+model's forward pass does, so every step reads a cache that left L2 long ago ("inputs larger than
+L2": R x ~30 MB touched per visit vs the 126 MB L2).  Consecutive steps are ordered on one stream:
+the time per step in steady state IS the critical path; EMA update/predict overlap later steps.
+Steps are captured into CUDA graphs (chunks of 4R steps) and the K timed steps are launched back
+to back between two CUDA events.  One JSON line is printed by rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for _p in (ROOT, os.path.join(ROOT, "tests")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
+
+import numpy as np
+import torch
+
+from paper_2606_30389_b200 import synth
+
+METRIC = "per_layer_dsa_decode_critical_path"
+UNIT = "us"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.12)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0, t1):
+        inside = [r for (t, r) in self.rows if t0 - 0.06 <= t <= t1 + 0.06 and len(r) >= 6] or \
+                 [r for (_, r) in self.rows if len(r) >= 6]
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm = sorted(float(r[0]) for r in inside)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in inside)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(inside[0][1]), "reasons": reasons,
+                "samples": len(inside)}
+
+
+def algorithmic_bytes(cfg, mean_len):
+    """summaries + selected KV per layer-step."""
+    nb = mean_len / cfg.bs
+    return cfg.B * nb * cfg.Hkv * cfg.d * 2 + cfg.B * cfg.Hkv * cfg.K * cfg.bs * cfg.d * 4
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_run(cfg, steps, warmup, budget_s=None):
+    """The oracle, as it stands, on layer 0 of the workload: returns (us per layer-step, cores, n)."""
+    import psutil
+    from oracle import prr_oracle as O
+    inp = synth.make_layer(cfg, 0, device="cpu", steps=steps + warmup)
+    lay = O.OracleLayer(synth.bits(inp.k_pages), synth.bits(inp.v_pages), inp.block_table.numpy(),
+                        inp.seq_lens.numpy(), cfg.bs, cfg.K, cfg.Bud, cfg.Hq)
+    lay.theta = [(0.8, 0.1, 0.0)] * cfg.B          # fixed theta: the timed sample is the decode step
+    kb, vb, qb = synth.bits(inp.k_new), synth.bits(inp.v_new), synth.bits(inp.q_dec)
+    for t in range(warmup):
+        lay.append(kb[t], vb[t]); lay.step(qb[t])
+    proc = psutil.Process()
+    c0 = proc.cpu_times(); w0 = time.perf_counter()
+    n = 0
+    for t in range(warmup, warmup + steps):
+        lay.append(kb[t], vb[t]); lay.step(qb[t])
+        n += 1
+        if budget_s and time.perf_counter() - w0 > budget_s:
+            break
+    w1 = time.perf_counter(); c1 = proc.cpu_times()
+    cpu = (c1.user + c1.system) - (c0.user + c0.system)
+    cores = max(1, int(round(cpu / max(w1 - w0, 1e-9))))
+    return (w1 - w0) / n * 1e6, cores, n
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    us, cores, n = oracle_run(cfg, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": n, "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, 1), "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": us, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{n} layer-steps of layer 0 (numpy fp64 oracle, fixed theta, no calibration)"},
+            "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg, R):
+    return (f"{cfg.name}: batch {cfg.B}, {cfg.Hq}q/{cfg.Hkv}kv heads, d={cfg.d}, ctx {cfg.ctx_lo}"
+            + (f"-{cfg.ctx_hi}" if cfg.ctx_hi != cfg.ctx_lo else "") +
+            f", block {cfg.bs}, top-K {cfg.K}, budget {cfg.Bud}, rho {cfg.rho}; {R} independent seeded layer "
+            f"caches visited round-robin")
+
+
+# ------------------------------------------------------------------------------------------------
+class Stack:
+    """R layers of the workload resident in HBM + the library context."""
+
+    def __init__(self, cfg, R, tokens, dev, seed_off=0):
+        from paper_2606_30389_b200 import prr
+        self.prr, self.cfg, self.R, self.dev = prr, cfg, R, dev
+        self.inps = [synth.make_layer(cfg.scaled(seed=cfg.seed + seed_off), l, device=dev, steps=tokens,
+                                      poison=False) for l in range(R)]
+        self.MB = self.inps[0].block_table.shape[1]
+        self.ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B,
+                               max_blocks_per_seq=self.MB, n_layers=R)
+        self.kvs, self.summ = [], []
+        for l, inp in enumerate(self.inps):
+            kv = self.ctx.kv(inp.k_pages, inp.v_pages, inp.block_table, inp.seq_lens, l)
+            s = torch.zeros(cfg.B, cfg.Hkv, self.MB, cfg.d, dtype=torch.bfloat16, device=dev)
+            self.ctx.build_summaries(kv, s)
+            self.kvs.append(kv); self.summ.append(s)
+        self.out = [torch.zeros(cfg.B, cfg.Hq, cfg.d, dtype=torch.float32, device=dev) for _ in range(R)]
+        self.pos = 0                                        # global layer-step counter
+
+    def calibrate(self):
+        cfg = self.cfg
+        sc = torch.zeros(cfg.B, cfg.Hkv, self.MB, dtype=torch.float32, device=self.dev)
+        t0 = time.perf_counter()
+        for l, inp in enumerate(self.inps):
+            nb = ((inp.seq_lens.cpu().numpy() + cfg.bs - 1) // cfg.bs)
+            trajs = [torch.empty(cfg.Hkv, cfg.T_cal, int(nb[b]), dtype=torch.float32, device=self.dev)
+                     for b in range(cfg.B)]
+            for t in range(cfg.T_cal):
+                self.ctx.score(self.kvs[l], inp.q_cal[t], self.summ[l], sc)
+                for b in range(cfg.B):
+                    trajs[b][:, t, :] = sc[b, :, :int(nb[b])]
+            for b in range(cfg.B):
+                self.ctx.calibrate(l, b, trajs[b].contiguous(), want_host=False)
+        torch.cuda.synchronize()
+        return time.perf_counter() - t0
+
+    def enqueue(self, n, stream, sequential=False):
+        """Enqueue the next n layer-steps (append + PRR step) on `stream`."""
+        for _ in range(n):
+            l, t = self.pos % self.R, self.pos // self.R
+            inp = self.inps[l]
+            self.ctx.append(self.kvs[l], inp.k_new[t], inp.v_new[t], self.summ[l], stream=stream)
+            fn = self.ctx.attend if sequential else self.ctx.decode_step
+            fn(self.kvs[l], inp.q_dec[t], self.summ[l], self.out[l], stream=stream)
+            self.pos += 1
+
+    def capture(self, n, stream, sequential=False, chunk=None):
+        chunk = chunk or 4 * self.R
+        graphs = []
+        with torch.cuda.stream(stream):
+            while n > 0:
+                c = min(chunk, n)
+                self.ctx.graph_begin(stream)
+                self.enqueue(c, stream, sequential)
+                graphs.append(self.ctx.graph_end(stream))
+                n -= c
+        return graphs
+
+
+def timed_launch(graphs, stream):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for g in graphs:
+            g.launch(stream)
+        e1.record(stream)
+    e1.synchronize()
+    return e0.elapsed_time(e1)            # ms
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=16384)
+    ap.add_argument("--warmup", type=int, default=256)
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--layers", type=int, default=16, help="independent layer caches visited round-robin")
+    ap.add_argument("--impl", default="prr", choices=["prr", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=512)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-seq", action="store_true", help="skip the sequential select-then-attend leg")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = synth.CONFIGS[args.config]
+    if args.impl == "reference":
+        if args.steps == 16384:
+            args.steps, args.warmup = 12, 3
+        run_reference(args, cfg, rank, world)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    R = args.layers
+    K, W = args.steps, args.warmup
+    E = args.e2e_steps
+    seq_steps = 0 if args.no_seq else min(K, 4096)
+    total = 3 * W + K + seq_steps + E
+    tokens = (total + R - 1) // R + 2
+    st = Stack(cfg, R, tokens, dev, seed_off=rank)          # weak scaling: every rank its own sequences
+    cal_s = st.calibrate()
+    stream = torch.cuda.Stream(device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- PRR: warm-up (eager), capture K steps, time them ---------------------------------------
+    with torch.cuda.stream(stream):
+        st.enqueue(W, stream)
+    torch.cuda.synchronize()
+    st.ctx.get_stats(reset=True)
+    l0 = st.ctx.launch_count()
+    graphs = st.capture(K, stream)
+    launches = st.ctx.launch_count() - l0
+    barrier()
+    with ClockSampler(local) as cs:
+        t0 = time.time()
+        ms = timed_launch(graphs, stream)
+        barrier()
+        t1 = time.time()
+    clocks = cs.summary(t0, t1)
+    for g in graphs:
+        g.destroy()
+    stats = st.ctx.get_stats(reset=True)
+    if world > 1:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    us_step = ms * 1e3 / K
+
+    # ---- in-library sequential select-then-attend, same protocol --------------------------------
+    seq_us = None
+    if seq_steps:
+        with torch.cuda.stream(stream):
+            st.enqueue(W, stream, sequential=True)
+        torch.cuda.synchronize()
+        g2 = st.capture(seq_steps, stream, sequential=True)
+        barrier()
+        seq_us = timed_launch(g2, stream) * 1e3 / seq_steps
+        for g in g2:
+            g.destroy()
+
+    # ---- dominant kernel alone (speculative per-block attention), rotating layers, CUDA events ---
+    Bud = cfg.Bud
+    P = torch.empty(cfg.B, cfg.Hkv, Bud, dtype=torch.int32, device=dev)
+    Op = torch.empty(cfg.B, cfg.Hq, Bud, cfg.d, dtype=torch.float32, device=dev)
+    mp = torch.empty(cfg.B, cfg.Hq, Bud, dtype=torch.float32, device=dev)
+    lp = torch.empty_like(mp)
+    Ps = []
+    for l in range(R):
+        st.ctx.predict(l, cfg.B, P)
+        Ps.append(P.clone())
+    torch.cuda.synchronize()
+    units = float(sum((p >= 0).sum().item() for p in Ps)) / R          # (block, KV head) units per launch
+    reps = max(3, min(40, 2000 // R))
+    k_ms = []
+    with torch.cuda.stream(stream):
+        for rep in range(reps + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for l in range(R):
+                st.ctx.speculate(st.kvs[l], st.inps[l].q_dec[0], Ps[l], Op, mp, lp, stream=stream)
+            e1.record(stream)
+            e1.synchronize()
+            if rep:
+                k_ms.append(e0.elapsed_time(e1) / R)
+    k_us = float(np.median(k_ms)) * 1e3
+    unit_bytes = 4 * cfg.bs * cfg.d                                     # K and V tile of one block, bf16
+    peak, peak_src = peaks()
+    achieved = units * unit_bytes / (k_us * 1e-6) / 1e9
+
+    # ---- end to end through the C-ABI with HOST buffers -----------------------------------------
+    e2e = None
+    if E:
+        qh = [st.inps[l].q_dec.cpu().pin_memory() for l in range(R)]
+        kh = [st.inps[l].k_new.cpu().pin_memory() for l in range(R)]
+        vh = [st.inps[l].v_new.cpu().pin_memory() for l in range(R)]
+        oh = torch.zeros(cfg.B, cfg.Hq, cfg.d, dtype=torch.float32).pin_memory()
+        with torch.cuda.stream(stream):
+            st.enqueue(W, stream)
+        barrier()
+        w0 = time.perf_counter()
+        for i in range(E):
+            l, t = st.pos % R, st.pos // R
+            st.ctx.decode_step_host(st.kvs[l], qh[l][t], kh[l][t], vh[l][t], st.summ[l], oh, stream=stream)
+            st.pos += 1
+        e_us = (time.perf_counter() - w0) / E * 1e6
+        if world > 1:
+            t = torch.tensor([e_us], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_us = float(t.item())
+        e2e = {"value": e_us, "unit": UNIT,
+               "h2d_bytes_per_step": int(cfg.B * (cfg.Hq + 2 * cfg.Hkv) * cfg.d * 2),
+               "d2h_bytes_per_step": int(cfg.B * cfg.Hq * cfg.d * 4)}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    mean_len = float(np.mean([inp.seq_lens.float().mean().item() for inp in st.inps]))
+    abytes = algorithmic_bytes(cfg, mean_len)
+    cpu_us, cores, n_cpu = oracle_run(cfg, 64, 2, budget_s=args.cpu_seconds)
+    line = {
+        "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16 KV / fp32 softmax+accumulate (mma.sync bf16), fp64 exact scoring + EMA", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, R), "l2": "inputs larger than L2 (round-robin over "
+                   f"{R} layer caches, ~{R * abytes * 1.4 / 1e6:.0f} MB touched between reuses)",
+                   "timing": "CUDA events around K graph-captured layer-steps on one stream; max over ranks",
+                   "calibration_s": round(cal_s, 3)},
+        "layer_steps_per_s": world * 1e6 / us_step,
+        "path_roofline": {"algorithmic_bytes_per_step": int(abytes), "achieved": abytes / (us_step * 1e-6) / 1e9,
+                          "peak": peak, "unit": "GB/s", "frac": abytes / (us_step * 1e-6) / 1e9 / peak,
+                          "frac_of_nominal_8TBs": abytes / (us_step * 1e-6) / 1e9 / 8000.0, "peak_source": peak_src},
+        "sequential_us": seq_us, "speedup_vs_sequential": (seq_us / us_step) if seq_us else None,
+        "hit_rate": stats[1] / max(stats[0], 1), "mean_missed_per_row": stats[2] * K and stats[2] / (K * cfg.B * cfg.Hkv),
+        "roofline": {"kernel": "k_partial (speculative per-block attention over P)", "bound": "hbm",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "us_per_launch": k_us, "units_per_launch": units,
+                     "bytes_per_unit": unit_bytes, "peak_source": peak_src,
+                     "how": "kernel alone, CUDA events on its launch stream, round-robin over the layer caches"},
+        "cpu_baseline": {"value": cpu_us, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{n_cpu} layer-steps of layer 0 (numpy fp64 oracle, fixed theta, no calibration)"},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "paper_context": "PAPER.md reports only end-to-end ratios on H100 (1.35-1.47x avg decode speedup); no absolute per-layer number",
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -118,16 +118,21 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
   const float sl2 = scale * LOG2E;
   const float off0 = mx0 == -CUDART_INF_F ? 0.f : m0 * LOG2E;
   const float off1 = mx1 == -CUDART_INF_F ? 0.f : m1 * LOG2E;
-  uint32_t pa[4];
+  // P is fed to the tensor core as a two-term bf16 split (hi + lo), so the PV product keeps
+  // ~16 significant bits of the fp32 probabilities instead of bf16's 8.
+  uint32_t pa[4], pb[4];
   float l0 = 0.f, l1 = 0.f;
 #pragma unroll
   for (int nt = 0; nt < 2; ++nt) {
-    const uint32_t p01 = pack_bf16x2(ex2(fmaf(s[nt][0], sl2, -off0)), ex2(fmaf(s[nt][1], sl2, -off0)));
-    const uint32_t p23 = pack_bf16x2(ex2(fmaf(s[nt][2], sl2, -off1)), ex2(fmaf(s[nt][3], sl2, -off1)));
-    pa[nt * 2 + 0] = p01;  // (row r0,   tokens nt*8 + 2tq..)
-    pa[nt * 2 + 1] = p23;  // (row r0+8, tokens nt*8 + 2tq..)
-    l0 += bf16_lo(p01) + bf16_hi(p01);  // the denominator uses the weights the PV product uses
-    l1 += bf16_lo(p23) + bf16_hi(p23);
+    const float p0 = ex2(fmaf(s[nt][0], sl2, -off0)), p1 = ex2(fmaf(s[nt][1], sl2, -off0));
+    const float p2 = ex2(fmaf(s[nt][2], sl2, -off1)), p3 = ex2(fmaf(s[nt][3], sl2, -off1));
+    const uint32_t h01 = pack_bf16x2(p0, p1), h23 = pack_bf16x2(p2, p3);
+    pa[nt * 2 + 0] = h01;  // (row r0,   tokens nt*8 + 2tq..)
+    pa[nt * 2 + 1] = h23;  // (row r0+8, tokens nt*8 + 2tq..)
+    pb[nt * 2 + 0] = pack_bf16x2(p0 - bf16_lo(h01), p1 - bf16_hi(h01));
+    pb[nt * 2 + 1] = pack_bf16x2(p2 - bf16_lo(h23), p3 - bf16_hi(h23));
+    l0 += p0 + p1;
+    l1 += p2 + p3;
   }
   l0 += __shfl_xor_sync(FULL, l0, 1);
   l0 += __shfl_xor_sync(FULL, l0, 2);
@@ -148,7 +153,9 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
     uint32_t b0, b1, b2, b3;
     ldmatrix_x4_trans(b0, b1, b2, b3, Vs + (tok0 + (mat & 1) * 8 + rr) * LD + d2 * 16 + (mat >> 1) * 8);
     mma_bf16_16816(o[2 * d2], pa, b0, b1);
+    mma_bf16_16816(o[2 * d2], pb, b0, b1);
     mma_bf16_16816(o[2 * d2 + 1], pa, b2, b3);
+    mma_bf16_16816(o[2 * d2 + 1], pb, b2, b3);
   }
 
   // combine the TW warps through shared memory (aliases the K/V tiles)

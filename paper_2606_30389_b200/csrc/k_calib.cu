@@ -109,10 +109,12 @@ k_calib_sim(const float* __restrict__ IS, const int32_t* __restrict__ n_valid, i
       for (int i = tid; i < n_st; i += CAL_NT)
         s.keys[i] = score_key(f64_to_score(__dadd_rn(L[i], __dmul_rn(gamma, V[i]))));
       __syncthreads();
-      uint32_t Tk;
-      int need;
-      radix_select<CAL_NT>(s.keys, n_st, min(Bud, n_st), s.hist, s.ctl, Tk, need);
-      ordered_select<CAL_NT>(s.keys, n_st, Tk, need, nullptr, s.mask, s.scan);
+      if (min(Bud, n_st) > 0) {
+        uint32_t Tk;
+        int need;
+        radix_select<CAL_NT>(s.keys, n_st, min(Bud, n_st), s.hist, s.ctl, Tk, need);
+        ordered_select<CAL_NT>(s.keys, n_st, Tk, need, nullptr, s.mask, s.scan);
+      }
       __syncthreads();
       const uint32_t* mA = maskA + ((size_t)h * T + phi) * words;
       double loc = 0.0;

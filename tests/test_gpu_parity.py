@@ -191,7 +191,7 @@ def test_block_partials_against_eq6_8_states(cfg):
                                 [[P[b, h, s]] if hh == h else [] for hh in range(cfg.Hkv)], cfg.bs)[hq]
                     m, l, On = st
                     assert abs(mp[b, hq, s] - m) <= 1e-5 * max(1.0, abs(m))
-                    assert abs(lp[b, hq, s] - l) <= 4e-3 * l
+                    assert abs(lp[b, hq, s] - l) <= 1e-4 * l
                     H.check_out(Op[b, hq, s] / lp[b, hq, s], On, f"partial b{b} hq{hq} s{s}")
 
 
@@ -209,7 +209,7 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
             npred = [cfg.Bud, 0, cfg.Bud - 2][(b + h) % 3]
             keep = rng.choice(A[b, h], size=min(npred, cfg.K) // 2, replace=False)
             rest = np.setdiff1d(np.arange(nb[b]), A[b, h])
-            extra = rng.choice(rest, size=npred - len(keep), replace=False) if npred else []
+            extra = rng.choice(rest, size=min(len(rest), npred - len(keep)), replace=False) if npred else []
             pp = np.sort(np.concatenate([keep, extra]).astype(np.int32))
             P[b, h, :len(pp)] = pp
     q = inp.q_dec[1].contiguous()
@@ -231,7 +231,7 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
         st = O.fold(qb[b], ol.k, ol.v, ol.table[b], ol.lens[b], S, cfg.bs)
         for hq in range(cfg.Hq):
             assert abs(mo[b, hq].item() - st[hq][0]) <= 1e-5 * max(1.0, abs(st[hq][0]))
-            assert abs(lo[b, hq].item() - st[hq][1]) <= 4e-3 * st[hq][1]
+            assert abs(lo[b, hq].item() - st[hq][1]) <= 1e-4 * st[hq][1]
     _, _, M, cnt = gl.sets()
     for b in range(cfg.B):
         for h in range(cfg.Hkv):
