@@ -47,6 +47,11 @@ enum { PRR_BF16 = 0 };
  * over exactly A (BASELINE.json north_star).  PRR_RETAIN: P\A is "retained as additional
  * low-priority context", the output is attention over A u P. */
 enum { PRR_DROP = 0, PRR_RETAIN = 1 };
+/* How a layer-step is orchestrated (Fig. 1: speculation overlaps selection).
+ * PRR_FUSED (default): ONE persistent cooperative launch; warps are the workers, selection,
+ * speculative attention, repair and merge are ordered by device-scope counters.
+ * PRR_STREAMS: the paper's orchestration, one kernel per stage on two event-ordered streams. */
+enum { PRR_FUSED = 0, PRR_STREAMS = 1 };
 
 typedef struct prr_ctx prr_ctx; /* opaque, library-owned */
 
@@ -59,6 +64,7 @@ typedef struct {
   int32_t kv_dtype;              /* PRR_BF16 */
   int32_t overpredict_policy;    /* PRR_DROP | PRR_RETAIN */
   float sm_scale;                /* softmax scale of the attention logits; 0 -> 1/sqrt(head_dim) */
+  int32_t orchestration;         /* PRR_FUSED | PRR_STREAMS */
 } prr_layout;
 
 typedef struct {
@@ -188,6 +194,10 @@ int32_t prr_get_ema(prr_ctx* ctx, int32_t layer, int32_t seq, double* level, dou
 /* Cumulative counters since create / last reset: host int64[4] = sum|A|, sum|A n P|, sum|M|,
  * sum|P| over all (layer, seq, KV head, step).  Synchronises `stream`.  reset != 0 clears them. */
 int32_t prr_get_stats(prr_ctx* ctx, int64_t* stats_out, int32_t reset, void* stream);
+/* Synchronises `stream` and reports whether a fused step ever gave up waiting on a dependency
+ * counter (PRR_E_STATE; cannot happen unless the device was shared with a kernel that never ends)
+ * or a CUDA error is pending (PRR_E_CUDA). */
+int32_t prr_check(prr_ctx* ctx, void* stream);
 /* Number of kernels this ctx has launched (or captured) so far. */
 int64_t prr_launch_count(const prr_ctx* ctx);
 

@@ -33,6 +33,8 @@ static int check_launch(prr_ctx* c, const char* what) {
   return PRR_OK;
 }
 
+static size_t layer_rows(const prr_ctx* c, int layer) { return (size_t)layer * c->maxB * c->Hkv; }
+
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 template <typename T>
@@ -66,6 +68,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   if (K < 1 || budget < 0) PRR_FAIL(none, PRR_E_INVALID, "prr_create: need K >= 1 and budget >= 0");
   if (lay->overpredict_policy != PRR_DROP && lay->overpredict_policy != PRR_RETAIN)
     PRR_FAIL(none, PRR_E_INVALID, "prr_create: unknown overpredict_policy");
+  if (lay->orchestration != PRR_FUSED && lay->orchestration != PRR_STREAMS)
+    PRR_FAIL(none, PRR_E_INVALID, "prr_create: unknown orchestration");
   if (lay->sm_scale < 0.f || lay->sm_scale != lay->sm_scale)
     PRR_FAIL(none, PRR_E_INVALID, "prr_create: sm_scale must be >= 0");
   const int G = lay->n_q_heads / lay->n_kv_heads;
@@ -90,6 +94,18 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   c->NL = lay->n_layers; c->maxB = lay->max_batch;
   c->sm_scale = lay->sm_scale > 0.f ? lay->sm_scale : (float)(1.0 / std::sqrt((double)c->D));
   c->score_c = 1.0 / ((double)G * std::sqrt((double)c->D));
+  c->fused = lay->orchestration == PRR_FUSED;
+  {
+    int dev = 0, coop = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (c->fused && (!coop || c->n_sm < 1)) {
+      delete c;
+      PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: PRR_FUSED needs cooperative launch support");
+    }
+  }
 
   const size_t rows = (size_t)c->NL * c->maxB * c->Hkv;
   const size_t srows = (size_t)c->maxB * c->Hkv;
@@ -106,6 +122,12 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->P_next, rows * (size_t)(c->Bud + 1)));
   A(dalloc(c, &c->P_used, rows * (size_t)(c->Bud + 1)));
   A(dalloc(c, &c->counts, rows * 3));
+  A(dalloc(c, &c->Pbuf[0], rows * (size_t)(c->Bud + 1)));
+  A(dalloc(c, &c->Pbuf[1], rows * (size_t)(c->Bud + 1)));
+  A(dalloc(c, &c->parity, (size_t)c->NL));
+  A(dalloc(c, &c->maskA, srows * (size_t)((c->MB + 31) / 32)));
+  A(dalloc(c, &c->pred, srows * (size_t)c->MB));
+  A(dalloc(c, &c->ctl, (size_t)8 + 5 * srows));
   A(dalloc(c, &c->merge_src, srows * (c->Bud + c->K)));
   A(dalloc(c, &c->merge_n, srows));
   A(dalloc(c, &c->nblk, (size_t)c->maxB));
@@ -128,6 +150,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
     // P lists start empty (-1); theta defaults to (1, 1, 0): "reuse the last step's top-K" (S1)
     e = cudaMemset(c->P_next, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemset(c->P_used, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->Pbuf[0], 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemset(c->Pbuf[1], 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
     std::vector<double> th((size_t)c->NL * c->maxB * 3);
     for (size_t i = 0; i < th.size(); i += 3) { th[i] = 1.0; th[i + 1] = 1.0; th[i + 2] = 0.0; }
     if (e == cudaSuccess) e = cudaMemcpy(c->theta, th.data(), th.size() * sizeof(double), cudaMemcpyHostToDevice);
@@ -185,8 +209,6 @@ static int check_kv(prr_ctx* c, const prr_paged_kv* kv, const char* fn) {
 #define CHECK_PTR(p, fn) do { if (!(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: null %s", fn, #p); \
     if (!aligned16(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: %s must be 16-byte aligned", fn, #p); } while (0)
 
-static size_t layer_rows(const prr_ctx* c, int layer) { return (size_t)layer * c->maxB * c->Hkv; }
-
 // Make `s` wait for every EMA update still running on the side stream.
 static void join_updates(prr_ctx* c, cudaStream_t s) {
   for (int l = 0; l < c->NL; ++l)
@@ -221,6 +243,24 @@ __global__ void k_fill_i32(int32_t* p, size_t n, int32_t v) {
   if (i < n) p[i] = v;
 }
 
+// Fused orchestration keeps the prediction in two buffers selected by a device-side parity.
+// which = 0: the buffer the NEXT step reads; which = 1: the buffer the LAST step read.
+__global__ void k_copy_P(int32_t* P0, int32_t* P1, const int32_t* parity, int which, int32_t* other,
+                         size_t n, int to_pbuf) {
+  int32_t* P = ((*parity ^ which) & 1) ? P1 : P0;
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { if (to_pbuf) P[i] = other[i]; else other[i] = P[i]; }
+}
+// After a stage-level prediction landed in P_next: make it the one the next fused step reads.
+static void sync_pred(prr_ctx* c, int layer, int seq0, int nseq, cudaStream_t s) {
+  if (!c->fused || c->Bud <= 0) return;
+  const size_t off = (layer_rows(c, layer) + (size_t)seq0 * c->Hkv) * c->Bud;
+  const size_t n = (size_t)nseq * c->Hkv * c->Bud;
+  k_copy_P<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(c->Pbuf[0] + off, c->Pbuf[1] + off,
+                                                       c->parity + layer, 0, c->P_next + off, n, 1);
+  c->launches++;
+}
+
 extern "C" int32_t prr_set_ema_params(prr_ctx* ctx, int32_t layer, int32_t seq, double alpha, double beta,
                                       double gamma, void* stream) {
   if (!ctx) return PRR_E_INVALID;
@@ -246,6 +286,10 @@ extern "C" int32_t prr_reset_ema(prr_ctx* ctx, int32_t layer, void* stream) {
   PRR_CUDA(ctx, cudaMemsetAsync(ctx->n_state + r, 0, n * sizeof(int32_t), s));
   if (ctx->Bud > 0)
     PRR_CUDA(ctx, cudaMemsetAsync(ctx->P_next + r * ctx->Bud, 0xff, n * ctx->Bud * sizeof(int32_t), s));
+  if (ctx->Bud > 0 && ctx->fused) {
+    PRR_CUDA(ctx, cudaMemsetAsync(ctx->Pbuf[0] + r * ctx->Bud, 0xff, n * ctx->Bud * sizeof(int32_t), s));
+    PRR_CUDA(ctx, cudaMemsetAsync(ctx->Pbuf[1] + r * ctx->Bud, 0xff, n * ctx->Bud * sizeof(int32_t), s));
+  }
   return PRR_OK;
 }
 
@@ -271,6 +315,7 @@ extern "C" int32_t prr_calibrate(prr_ctx* ctx, int32_t layer, int32_t seq, const
     const size_t rows = layer_rows(ctx, layer) + (size_t)seq * ctx->Hkv;
     e.P_out = ctx->P_next + rows * ctx->Bud;
     launch_ema(ctx, e, s);
+    sync_pred(ctx, layer, seq, 1, s);
     if ((r = check_launch(ctx, "prr_calibrate(predict)"))) return r;
   }
   if (theta_out || H_out || H_all_out) {
@@ -319,6 +364,7 @@ extern "C" int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, co
   e.scores = scores; e.n_blocks = n_blocks;
   e.P_out = ctx->P_next + layer_rows(ctx, layer) * ctx->Bud;
   launch_ema(ctx, e, s);
+  sync_pred(ctx, layer, 0, batch, s);
   return check_launch(ctx, "prr_ema_update");
 }
 
@@ -399,12 +445,23 @@ static void enqueue_ema(prr_ctx* c, const prr_paged_kv* kv, cudaStream_t main, b
   c->upd_pending[kv->layer] = 1;
 }
 
+static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries,
+                      float* out, int spec, cudaStream_t s, const char* fn) {
+  const int e = launch_step(c, kv, q, summaries, out, spec, s);
+  if (e) {
+    cudaGetLastError();
+    PRR_FAIL(c, PRR_E_CUDA, "%s: fused step launch: %s", fn, cudaGetErrorString((cudaError_t)e));
+  }
+  return check_launch(c, fn);
+}
+
 extern "C" int32_t prr_attend(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
                               float* out, void* stream) {
   CHECK_KV("prr_attend");
   CHECK_PTR(q, "prr_attend"); CHECK_PTR(summaries, "prr_attend");
   if (!out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_attend: null out");
   cudaStream_t s = (cudaStream_t)stream;
+  if (ctx->fused) return fused_step(ctx, kv, q, summaries, out, 0, s, "prr_attend");
   const size_t r = layer_rows(ctx, kv->layer);
   join_layer(ctx, kv->layer, s);
   float* sc = ctx->scores + r * ctx->MB;
@@ -432,6 +489,7 @@ extern "C" int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const v
   CHECK_PTR(q, "prr_decode_step"); CHECK_PTR(summaries, "prr_decode_step");
   if (!out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_decode_step: null out");
   cudaStream_t s = (cudaStream_t)stream;
+  if (ctx->fused) return fused_step(ctx, kv, q, summaries, out, 1, s, "prr_decode_step");
   const size_t r = layer_rows(ctx, kv->layer);
   const bool spec = ctx->Bud > 0;
   join_layer(ctx, kv->layer, s);  // this layer's previous EMA update / prediction must be complete
@@ -496,7 +554,12 @@ extern "C" int32_t prr_get_sets(prr_ctx* ctx, int32_t layer, int32_t batch, int3
   const size_t r = layer_rows(ctx, layer), n = (size_t)batch * ctx->Hkv;
   if (A) PRR_CUDA(ctx, cudaMemcpyAsync(A, ctx->setA + r * ctx->K, n * ctx->K * 4, cudaMemcpyDeviceToDevice, s));
   if (M) PRR_CUDA(ctx, cudaMemcpyAsync(M, ctx->setM + r * ctx->K, n * ctx->K * 4, cudaMemcpyDeviceToDevice, s));
-  if (P && ctx->Bud > 0)
+  if (P && ctx->Bud > 0 && ctx->fused) {
+    const size_t np = n * ctx->Bud;
+    k_copy_P<<<(unsigned)((np + 255) / 256), 256, 0, s>>>(ctx->Pbuf[0] + r * ctx->Bud, ctx->Pbuf[1] + r * ctx->Bud,
+                                                          ctx->parity + layer, 1, P, np, 0);
+    ctx->launches++;
+  } else if (P && ctx->Bud > 0)
     PRR_CUDA(ctx, cudaMemcpyAsync(P, ctx->P_used + r * ctx->Bud, n * ctx->Bud * 4, cudaMemcpyDeviceToDevice, s));
   if (counts) PRR_CUDA(ctx, cudaMemcpyAsync(counts, ctx->counts + r * 3, n * 3 * 4, cudaMemcpyDeviceToDevice, s));
   return PRR_OK;
@@ -537,6 +600,17 @@ extern "C" int32_t prr_get_stats(prr_ctx* ctx, int64_t* stats_out, int32_t reset
   if (reset) PRR_CUDA(ctx, cudaMemsetAsync(ctx->stats, 0, 32, s));
   PRR_CUDA(ctx, cudaStreamSynchronize(s));
   return PRR_OK;
+}
+
+extern "C" int32_t prr_check(prr_ctx* ctx, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  cudaStream_t s = (cudaStream_t)stream;
+  join_updates(ctx, s);
+  uint32_t err = 0;
+  PRR_CUDA(ctx, cudaMemcpyAsync(&err, ctx->ctl + 1, sizeof(err), cudaMemcpyDeviceToHost, s));
+  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  if (err) PRR_FAIL(ctx, PRR_E_STATE, "prr_check: a fused step gave up waiting on a dependency counter");
+  return check_launch(ctx, "prr_check");
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -25,6 +25,10 @@ struct prr_ctx {
   int32_t* setM = nullptr;    // [NL, maxB, Hkv, K]
   int32_t* P_next = nullptr;  // [NL, maxB, Hkv, Bud]  prediction for the next step of the layer
   int32_t* P_used = nullptr;  // [NL, maxB, Hkv, Bud]  prediction the last step used
+  // fused orchestration: the step reads Pbuf[parity[layer]] and writes the next prediction into
+  // the other buffer, then flips the parity (all on the device, so a captured graph replays)
+  int32_t* Pbuf[2] = {nullptr, nullptr};  // [NL, maxB, Hkv, Bud] each
+  int32_t* parity = nullptr;              // [NL]
   int32_t* counts = nullptr;  // [NL, maxB, Hkv, 3]    |A|, |P|, |M| of the last step
   // ---- per-step scratch, device (shared by all layers; steps are ordered on the main stream) ----
   int32_t* merge_src = nullptr; // [maxB, Hkv, Bud+K] slot codes, ascending block order
@@ -33,6 +37,10 @@ struct prr_ctx {
   float *O_spec = nullptr, *m_spec = nullptr, *l_spec = nullptr; // [maxB, Hq, Bud, D] / [.., Bud]
   float *O_rep = nullptr, *m_rep = nullptr, *l_rep = nullptr;    // [maxB, Hq, K, D]   / [.., K]
   unsigned long long* stats = nullptr; // [4]
+  uint32_t* maskA = nullptr;  // [maxB, Hkv, ceil(MB/32)] bitmask of A (fused step)
+  float* pred = nullptr;      // [maxB, Hkv, MB] Eq. 2 predictions of the row being ranked (fused step)
+  uint32_t* ctl = nullptr;    // fused step: exit counter, error flag, per-row dependency counters
+  int n_sm = 0, smem_optin = 0, fused = 1;
   // ---- calibration scratch (allocated on first prr_calibrate) ----
   double* cal_state = nullptr; size_t cal_state_elems = 0; // [80, Hkv, N, 2]
   uint32_t* cal_mask = nullptr; size_t cal_mask_words = 0; // [Hkv, T, ceil(N/32)]
@@ -97,6 +105,10 @@ void launch_merge(prr_ctx* c, int batch, const int32_t* merge_src, const int32_t
                   const float* O_spec, const float* m_spec, const float* l_spec, int w_spec,
                   const float* O_rep, const float* m_rep, const float* l_rep, int w_rep,
                   float* out, float* m_out, float* l_out, cudaStream_t s);
+// k_step.cu: one fused launch for a whole layer-step; spec = 0 is the sequential path.  Returns 0
+// or a cudaError_t.
+int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
+                int spec, cudaStream_t s);
 // k_calib.cu
 int launch_calibrate(prr_ctx* c, int layer, int seq, const float* IS, int T, int N,
                      const int32_t* n_valid, cudaStream_t s);

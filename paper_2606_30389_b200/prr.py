@@ -15,12 +15,13 @@ LIB_PATH = os.path.join(_HERE, "libprr.so")
 
 OK, E_INVALID, E_UNSUPPORTED, E_STATE, E_CUDA, E_NOMEM = range(6)
 DROP, RETAIN = 0, 1
+FUSED, STREAMS = 0, 1
 
 SYMBOLS = [
     "prr_create", "prr_destroy", "prr_last_error", "prr_version", "prr_build_summaries", "prr_append",
     "prr_set_ema_params", "prr_reset_ema", "prr_calibrate", "prr_predict", "prr_ema_update", "prr_score",
     "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_decode_step_host",
-    "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_launch_count",
+    "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
 ]
 
@@ -28,7 +29,8 @@ SYMBOLS = [
 class Layout(C.Structure):
     _fields_ = [("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("max_batch", C.c_int32), ("max_blocks_per_seq", C.c_int32), ("n_layers", C.c_int32),
-                ("kv_dtype", C.c_int32), ("overpredict_policy", C.c_int32), ("sm_scale", C.c_float)]
+                ("kv_dtype", C.c_int32), ("overpredict_policy", C.c_int32), ("sm_scale", C.c_float),
+                ("orchestration", C.c_int32)]
 
 
 class PagedKV(C.Structure):
@@ -99,9 +101,9 @@ class Context:
     """prr_ctx handle.  Methods take torch CUDA tensors with the layouts of include/prr.h."""
 
     def __init__(self, n_q_heads, n_kv_heads, head_dim, block_size, K, budget, max_batch=1,
-                 max_blocks_per_seq=1, n_layers=1, policy=DROP, sm_scale=0.0):
+                 max_blocks_per_seq=1, n_layers=1, policy=DROP, sm_scale=0.0, orchestration=FUSED):
         self.layout = Layout(n_q_heads, n_kv_heads, head_dim, max_batch, max_blocks_per_seq, n_layers,
-                             0, policy, sm_scale)
+                             0, policy, sm_scale, orchestration)
         self.block_size, self.K, self.budget = block_size, K, budget
         self._h = C.c_void_p()
         r = lib().prr_create(C.byref(self.layout), block_size, K, budget, C.byref(self._h))
@@ -226,6 +228,10 @@ class Context:
         st = (C.c_int64 * 4)()
         self._chk(lib().prr_get_stats(self._h, st, int(reset), C.c_void_p(_stream(stream))))
         return tuple(st)
+
+    def check(self, stream=None):
+        """Synchronises; raises if a fused step timed out on a dependency or a CUDA error is pending."""
+        self._chk(lib().prr_check(self._h, C.c_void_p(_stream(stream))))
 
     def launch_count(self) -> int:
         return int(lib().prr_launch_count(self._h))
