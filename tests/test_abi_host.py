@@ -30,12 +30,12 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_binding_structs_match_header_layout():
-    # field order and sizes of the two C structs (9 x 4 bytes; 4 pointers + 2 int32)
-    assert C.sizeof(prr.Layout) == 36
+    # field order and sizes of the two C structs (10 x 4 bytes; 4 pointers + 2 int32)
+    assert C.sizeof(prr.Layout) == 40
     assert C.sizeof(prr.PagedKV) == 4 * C.sizeof(C.c_void_p) + 8
     assert [f[0] for f in prr.Layout._fields_] == [
         "n_q_heads", "n_kv_heads", "head_dim", "max_batch", "max_blocks_per_seq", "n_layers", "kv_dtype",
-        "overpredict_policy", "sm_scale"]
+        "overpredict_policy", "sm_scale", "orchestration"]
 
 
 @pytest.mark.parametrize("args,code", [
