@@ -200,6 +200,15 @@ int32_t prr_get_stats(prr_ctx* ctx, int64_t* stats_out, int32_t reset, void* str
 int32_t prr_check(prr_ctx* ctx, void* stream);
 /* Number of kernels this ctx has launched (or captured) so far. */
 int64_t prr_launch_count(const prr_ctx* ctx);
+/* Profiling aid for the fused step (a9, Fig. 5 timeline).  While enabled, every warp of a
+ * fused step launched (or captured) afterwards stores %globaltimer (ns) at its phase boundaries:
+ * [0] start, [1] scores done, [2] row job done, [3] speculative units done, [4] repair units done,
+ * [5] merge done; words 6-15 are finer marks inside the prologue and the row jobs.  prr_timeline_read copies the stamps of the LAST step,
+ * uint64 [n_warps, 16] with warp index = cta * warps_per_cta + warp, to HOST memory and
+ * synchronises `stream`; n_warps_out (host, may be NULL) receives the rows copied (<= max_warps). */
+int32_t prr_timeline_enable(prr_ctx* ctx, int32_t on);
+int32_t prr_timeline_read(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps, int32_t* n_warps_out,
+                          void* stream);
 
 /* --- CUDA-graph helpers (so callers need no CUDA runtime of their own) ------------------------ */
 typedef struct prr_graph prr_graph;

@@ -9,23 +9,29 @@
 // targets an EARLIER phase of other warps, all CTAs are co-resident (cooperative launch), so the
 // schedule cannot deadlock; waits are bounded anyway and raise ctl[CTL_ERR].
 //
-//   phase 0  prefetch: cp.async of the warp's first speculative (block, KV head) tile -> all of
-//            the step's KV bytes are in flight before anything else happens
-//   phase 1  score chunks (a1): 16-byte loads of summary rows, exact fp64 accumulation (Q1)
-//   phase 2  row jobs, on the otherwise idle highest-numbered warps:
-//              select(row): wait for the row's scores -> exact top-K by range narrowing (a2),
-//                           ascending A / bitmask, diff against P (a5) -> M list, publish
+//   phase 1  score chunks (a1): the 16-byte loads of the summary rows are issued FIRST (they head
+//            the critical path), then the warp's first speculative tile is put in flight
+//            (cp.async), then the chunk is finished: exact fp64 accumulation (Q1)
+//   phase 2  row jobs.  When rows are few (2R <= #SM/4) a whole CTA is the team of one job: its
+//            threads hold the row's keys in shared memory and find the exact k-th key by range
+//            narrowing with private counters; otherwise one warp per job does the same.
+//              select(row): wait for the row's scores -> A ascending + bitmask (a2), diff against
+//                           P (a5) -> M list, publish
 //              ema(row):    wait for the row's scores -> Eq. 3 update, Eq. 2 prediction, top-Bud
 //                           -> P of the NEXT step into the other parity buffer (a8, a3)
 //   phase 3  speculative units (a4): per-block partial state (m, l, O) of every block of P
-//   phase 4  repair units (a6): wait for select(row), same partial-state code over M = A\P
-//   phase 5  merge items (a7): wait for the row's units, fold hits u M (DROP) or P u M (RETAIN)
-//            by Eq. 6-8 with one division at the end
+//   phase 4  repair units (a6), claimed dynamically by whichever warp is free: ticket -> (row,
+//            slot), wait for select(row), same partial-state code over M = A\P
+//   phase 5  merge items (a7), claimed dynamically: wait for the row's units, fold hits u M (DROP)
+//            or P u M (RETAIN) by Eq. 6-8 with one division at the end
 //   exit     last warp resets the counters and flips the layer's P parity
 //
 // spec = 0 runs the same kernel as the sequential select-then-attend path: P is
 // treated as empty, every block of A is a "repair" unit that can only start after selection.
+#include <cuda.h>
 #include <math_constants.h>
+
+#include <cstring>
 
 #include "prr_dev.cuh"
 #include "prr_internal.h"
@@ -35,13 +41,19 @@ namespace prr {
 constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr uint32_t SPIN_LIMIT = 1u << 22;  // ~0.1-0.5 s of polling, then give up loudly
 
-enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_HDR = 4 };  // then 5 arrays of Rmax words
-// ctl arrays: [0] score_done, [1] sel_flag, [2] units_done, [3] units_total, [4] nM
+// ctl header words, then 5 arrays of Rmax words:
+//   [0] score_done, [1] sel_flag, [2] units_done, [3] units_total, [4] nM
+enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_RTICKET = 2, CTL_MTICKET = 3, CTL_SELDONE = 4, CTL_MAXM = 5, CTL_HDR = 8 };
 
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
   return v;
+}
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
+  return t;
 }
 
 // Warp-collective wait until *p >= target.  Lane 0 polls; __syncwarp orders the other lanes.
@@ -49,7 +61,7 @@ __device__ __forceinline__ void wait_ge(const uint32_t* p, uint32_t target, uint
   if ((threadIdx.x & 31) == 0) {
     uint32_t it = 0;
     while (ld_acquire(p) < target) {
-      __nanosleep(40);
+      __nanosleep(20);
       if (++it > SPIN_LIMIT) { atomicExch(err, 1u); break; }
     }
   }
@@ -63,109 +75,149 @@ __device__ __forceinline__ void signal_add(uint32_t* p, uint32_t v) {
   if ((threadIdx.x & 31) == 0) atomicAdd(p, v);
 }
 
-__device__ __forceinline__ uint32_t key_at(const float* v, int i) { return score_key(__ldcg(v + i)); }
-
 struct Thr { uint32_t key; int idx; };  // selected(i) <=> key_i > key || (key_i == key && i <= idx)
+__device__ __forceinline__ bool selected(uint32_t key, int i, const Thr& t) {
+  return key > t.key || (key == t.key && i <= t.idx);
+}
 
 // ---------------------------------------------------------------------------------------------
-// Exact k-th largest of n fp32 values in global memory under the order (value desc, index asc),
-// by one warp, as a threshold pair.  Range narrowing on the order-preserving keys: the invariant
-// is "the threshold key lies in [lo, lo+span]; `need` of the keys in that range are selected, every
-// key above it is".  Each pass counts 16 sub-ranges in packed per-lane counters (no atomics);
-// <= 64 survivors are ranked directly; a range of one key value is resolved by index order.
-// Integer-only, hence order-independent and bit-exact (Q4).  Requires 1 <= k < n.
-// ---------------------------------------------------------------------------------------------
-__device__ Thr warp_kth(const float* v, int n, int k, uint32_t* candk, int32_t* candi) {
-  const int lane = threadIdx.x & 31;
-  const uint32_t lt = (1u << lane) - 1u;
-  uint32_t kmin = 0xffffffffu, kmax = 0u;
-  for (int i = lane; i < n; i += 32) {
-    const uint32_t key = key_at(v, i);
-    kmin = min(kmin, key);
-    kmax = max(kmax, key);
+// A team is the set of threads that works on one row job: a whole CTA or one warp.
+struct Team {
+  int tid, nt, wid, nw;
+  bool cta;
+  __device__ __forceinline__ void sync() const { if (cta) __syncthreads(); else __syncwarp(); }
+};
+// The team's shared memory: the row's keys (if they fit), bitmask / offset words, a histogram of
+// 2^hbits counters, reduction slots.
+struct TeamMem {
+  uint32_t* keys; int key_cap;
+  uint32_t *pmask, *amask, *offs;  // [MBw] each
+  uint32_t* hist; int hbits;       // [1 << hbits], zero on entry to and exit from team_kth
+  uint32_t* red;                   // [nw*16] per-warp slots, then 8 decision words
+  uint32_t* candk; int32_t* candi; // [64] each
+};
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void red_shared_add(uint32_t* p, uint32_t v) {
+  asm volatile("red.shared.add.u32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+struct Keys {  // the row's order-preserving keys: shared memory if they fit, else recomputed from global
+  uint32_t sm; const float* gl;  // sm: shared-window address of keys[0], 0 = not resident
+  __device__ __forceinline__ uint32_t get(int i) const {
+    return sm ? lds_u32(sm + 4u * (uint32_t)i) : score_key(__ldcg(gl + i));
   }
-  uint32_t lo = __reduce_min_sync(FULL, kmin);
-  uint32_t span = __reduce_max_sync(FULL, kmax) - lo;
+};
+
+// Highest bucket b of hist[0 .. NB) with  sum_{b' >= b} hist[b'] >= need  (1 <= need <= total);
+// `above` = the count in the buckets over b.  Thread t owns the buckets [NB-(t+1)per, NB-t*per), so
+// a prefix scan over threads is a suffix scan over buckets.  Every thread zeroes the buckets it
+// read; every thread returns the same triple.
+__device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, const TeamMem& m, int& bstar,
+                          int& cstar, int& above) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + tm.nw * 16;
+  const int per = (NB + tm.nt - 1) / tm.nt;
+  const int hi = NB - tm.tid * per, lo = max(0, hi - per);
+  uint32_t sum = 0;
+  for (int b = lo; b < hi; ++b) sum += hist[b];
+  uint32_t incl = sum;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const uint32_t x = __shfl_up_sync(FULL, incl, off);
+    if (lane >= off) incl += x;
+  }
+  if (tm.cta) {
+    if (lane == 31) m.red[tm.wid] = incl;
+    __syncthreads();
+    for (int w = 0; w < tm.wid; ++w) incl += m.red[w];
+  }
+  const uint32_t excl = incl - sum;
+  if ((int)excl < need && need <= (int)incl) {  // the crossing is in this thread's buckets (exactly one thread)
+    uint32_t acc = excl;
+    for (int b = hi - 1; b >= lo; --b) {
+      const uint32_t c = hist[b];
+      if ((int)(acc + c) >= need) { dec[0] = (uint32_t)b; dec[1] = c; dec[2] = acc; break; }
+      acc += c;
+    }
+  }
+  for (int b = lo; b < hi; ++b) hist[b] = 0u;
+  tm.sync();
+  bstar = (int)dec[0]; cstar = (int)dec[1]; above = (int)dec[2];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exact k-th largest of n keys under the order (key desc, index asc), by one team, as a threshold
+// pair.  Range narrowing on the order-preserving keys: the invariant is "the threshold key lies in
+// [lo, lo+span]; `need` of the keys in that range are selected, every key above it is".  Each pass
+// histograms the range into 2^hbits buckets (shared-memory reductions) and keeps the bucket the
+// threshold falls in; <= 64 survivors are ranked directly; a range of one key value is resolved by
+// index order.  Integer-only, hence order-independent and bit-exact (Q4).  Requires
+// 1 <= k < n, [lo, lo+span] = the exact key range of the row, and a zeroed histogram.
+// ---------------------------------------------------------------------------------------------
+__device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const TeamMem& m, uint32_t lo, uint32_t span) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + tm.nw * 16;  // [0] bstar [1] cstar [2] acc [5] key [6] idx [7] cand count
   int need = k, cnt_in = n;
   Thr r;
   for (;;) {
     if (span == 0) {  // all survivors share one key: the `need` lowest indices win
-      int base = 0;
-      r.key = lo; r.idx = n - 1;
-      for (int j0 = 0; j0 < n; j0 += 32) {
-        const int i = j0 + lane;
-        const uint32_t bal = __ballot_sync(FULL, i < n && key_at(v, i) == lo);
-        const int c = __popc(bal);
-        if (base + c >= need) { r.idx = j0 + (int)__fns(bal, 0, need - base); break; }
-        base += c;
+      if (tm.wid == 0) {
+        int base = 0, idx = n - 1;
+        for (int j0 = 0; j0 < n; j0 += 32) {
+          const int i = j0 + lane;
+          const uint32_t bal = __ballot_sync(FULL, i < n && ks.get(i) == lo);
+          const int c = __popc(bal);
+          if (base + c >= need) { idx = j0 + (int)__fns(bal, 0, need - base); break; }
+          base += c;
+        }
+        if (lane == 0) { dec[5] = lo; dec[6] = (uint32_t)idx; }
       }
+      tm.sync();
+      r.key = dec[5]; r.idx = (int)dec[6];
+      tm.sync();
       return r;
     }
-    if (cnt_in <= 64) {  // collect the survivors (ascending index) and rank them
-      int base = 0;
-      for (int j0 = 0; j0 < n; j0 += 32) {
-        const int i = j0 + lane;
-        const uint32_t key = i < n ? key_at(v, i) : 0u;
-        const bool in = i < n && (key - lo) <= span;
-        const uint32_t bal = __ballot_sync(FULL, in);
-        if (in) {
-          const int pos = base + __popc(bal & lt);
-          candk[pos] = key;
-          candi[pos] = i;
-        }
-        base += __popc(bal);
-      }
-      __syncwarp();
-      uint32_t wk = 0; int wi = 0; bool won = false;
-      for (int e = lane; e < cnt_in; e += 32) {
-        const uint32_t ke = candk[e];
-        const int ie = candi[e];
-        int rank = 0;
-        for (int f = 0; f < cnt_in; ++f) {
-          const uint32_t kf = candk[f];
-          rank += (kf > ke) || (kf == ke && candi[f] < ie);
-        }
-        if (rank == need - 1) { wk = ke; wi = ie; won = true; }
-      }
-      const uint32_t bal = __ballot_sync(FULL, won);
-      const int src = __ffs(bal) - 1;  // exactly one winner: ranks are a permutation
-      r.key = __shfl_sync(FULL, wk, src);
-      r.idx = __shfl_sync(FULL, wi, src);
-      __syncwarp();
-      return r;
-    }
-    const int sh = max(0, (32 - __clz(span)) - 4);  // (span >> sh) <= 15
-    uint32_t cnt[16];
-#pragma unroll
-    for (int b = 0; b < 16; ++b) cnt[b] = 0;
-    for (int i0 = 0; i0 < n; i0 += 32 * 255) {  // 8-bit packed counters: flush every 255 keys per lane
-      unsigned long long c0 = 0, c1 = 0;
-      const int i1 = min(n, i0 + 32 * 255);
+    if (cnt_in <= 64) {  // collect the survivors (any order) and rank them
+      if (tm.tid == 0) dec[7] = 0u;
+      tm.sync();
 #pragma unroll 4
-      for (int i = i0 + lane; i < i1; i += 32) {
-        const uint32_t d = key_at(v, i) - lo;
-        const uint32_t b = d >> sh;
-        const unsigned long long inc = d <= span ? (1ull << ((b & 7u) * 8u)) : 0ull;
-        c0 += b < 8u ? inc : 0ull;
-        c1 += b < 8u ? 0ull : inc;
+      for (int i = tm.tid; i < n; i += tm.nt) {
+        const uint32_t key = ks.get(i);
+        if ((key - lo) <= span) {
+          const uint32_t pos = atomicAdd(&dec[7], 1u);
+          m.candk[pos] = key;
+          m.candi[pos] = i;
+        }
       }
-#pragma unroll
-      for (int b = 0; b < 8; ++b) {
-        cnt[b] += (uint32_t)(c0 >> (8 * b)) & 255u;
-        cnt[8 + b] += (uint32_t)(c1 >> (8 * b)) & 255u;
+      tm.sync();
+      for (int e = tm.tid; e < cnt_in; e += tm.nt) {
+        const uint32_t ke = m.candk[e];
+        const int ie = m.candi[e];
+        int rank = 0;
+#pragma unroll 8
+        for (int f = 0; f < cnt_in; ++f) {
+          const uint32_t kf = m.candk[f];
+          rank += (kf > ke) || (kf == ke && m.candi[f] < ie);
+        }
+        if (rank == need - 1) { dec[5] = ke; dec[6] = (uint32_t)ie; }  // exactly one: ranks are a permutation
       }
+      tm.sync();
+      r.key = dec[5]; r.idx = (int)dec[6];
+      tm.sync();
+      return r;
     }
-#pragma unroll
-    for (int b = 0; b < 16; ++b) cnt[b] = __reduce_add_sync(FULL, cnt[b]);
-    int acc = 0, bstar = 0, cstar = 0;
-    bool found = false;
-#pragma unroll
-    for (int b = 15; b >= 0; --b) {
-      if (!found) {
-        if (acc + (int)cnt[b] >= need) { bstar = b; cstar = (int)cnt[b]; found = true; }
-        else acc += (int)cnt[b];
-      }
+    const int sh = max(0, (32 - __clz(span)) - m.hbits);  // (span >> sh) < 2^hbits
+#pragma unroll 4
+    for (int i = tm.tid; i < n; i += tm.nt) {
+      const uint32_t d = ks.get(i) - lo;
+      if (d <= span) red_shared_add(&m.hist[d >> sh], 1u);
     }
+    tm.sync();
+    int bstar, cstar, acc;
+    team_pick(m.hist, 1 << m.hbits, need, tm, m, bstar, cstar, acc);
     need -= acc;
     cnt_in = cstar;
     const uint32_t off = (uint32_t)bstar << sh;
@@ -176,12 +228,80 @@ __device__ Thr warp_kth(const float* v, int n, int k, uint32_t* candk, int32_t* 
   }
 }
 
-__device__ __forceinline__ bool selected(uint32_t key, int i, const Thr& t) {
-  return key > t.key || (key == t.key && i <= t.idx);
+// Team-wide min / max of the per-thread key range -> (lo, span).
+__device__ __forceinline__ void team_range(uint32_t kmin, uint32_t kmax, const Team& tm, const TeamMem& m,
+                                           uint32_t& lo, uint32_t& span) {
+  kmin = __reduce_min_sync(FULL, kmin);
+  kmax = __reduce_max_sync(FULL, kmax);
+  if (!tm.cta) { lo = kmin; span = kmax >= kmin ? kmax - kmin : 0u; return; }
+  if ((threadIdx.x & 31) == 0) { m.red[tm.wid * 2] = kmin; m.red[tm.wid * 2 + 1] = kmax; }
+  tm.sync();
+  for (int w = 0; w < tm.nw; ++w) { kmin = min(kmin, m.red[w * 2]); kmax = max(kmax, m.red[w * 2 + 1]); }
+  tm.sync();
+  lo = kmin; span = kmax >= kmin ? kmax - kmin : 0u;
+}
+
+// Ordered emission: the selected indices ascending into list[width] (padded with -1), the bitmask
+// into mask_g (global, may be null); with Mlist != null also the selected indices NOT in pmask
+// (ascending, padded to widthM).  Returns (nA << 16) | nM in every thread.
+__device__ uint32_t team_emit(const Keys& ks, int n, int k, const Thr& t, const Team& tm, const TeamMem& m,
+                              int32_t* list, int width, uint32_t* mask_g, int32_t* Mlist, int widthM) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt = (1u << lane) - 1u;
+  const int nwd = (n + 31) >> 5;
+  uint32_t* dec = m.red + tm.nw * 16;
+#pragma unroll 4
+  for (int w = tm.wid; w < nwd; w += tm.nw) {
+    const int i = w * 32 + lane;
+    const bool sel = i < n && k > 0 && selected(ks.get(i), i, t);
+    const uint32_t aw = __ballot_sync(FULL, sel);
+    if (lane == 0) m.amask[w] = aw;
+  }
+  tm.sync();
+  if (tm.wid == 0) {
+    uint32_t carry = 0;
+    for (int w0 = 0; w0 < nwd; w0 += 32) {
+      const int w = w0 + lane;
+      const uint32_t aw = w < nwd ? m.amask[w] : 0u;
+      const uint32_t mw = (Mlist && w < nwd) ? (aw & ~m.pmask[w]) : 0u;
+      const uint32_t v = ((uint32_t)__popc(aw) << 16) | (uint32_t)__popc(mw);
+      uint32_t incl = v;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t x = __shfl_up_sync(FULL, incl, off);
+        if (lane >= off) incl += x;
+      }
+      if (w < nwd) m.offs[w] = carry + incl - v;
+      carry += __shfl_sync(FULL, incl, 31);
+    }
+    if (lane == 0) dec[3] = carry;
+  }
+  tm.sync();
+  for (int w = tm.wid; w < nwd; w += tm.nw) {
+    const uint32_t aw = m.amask[w];
+    const uint32_t off = m.offs[w];
+    const int i = w * 32 + lane;
+    if ((aw >> lane) & 1u) {
+      list[(off >> 16) + __popc(aw & lt)] = i;
+      if (Mlist) {
+        const uint32_t mw = aw & ~m.pmask[w];
+        if ((mw >> lane) & 1u) Mlist[(off & 0xffffu) + __popc(mw & lt)] = i;
+      }
+    }
+    if (mask_g && lane == 0) mask_g[w] = aw;
+  }
+  const uint32_t tot = dec[3];
+  for (int j = (int)(tot >> 16) + tm.tid; j < width; j += tm.nt) list[j] = -1;
+  if (Mlist)
+    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
+  tm.sync();
+  return tot;
 }
 
 // ---------------------------------------------------------------------------------------------
 struct StepArgs {
+  alignas(64) CUtensorMap mapK;  // bf16 [rows = n_pages*Hkv*bs, d], box [bs, 64], 128-byte swizzle
+  alignas(64) CUtensorMap mapV;
   const uint16_t* kp; const uint16_t* vp; const int32_t* table; const int32_t* seq_lens;
   const uint16_t* q; const uint4* summ; float* out;
   // layer state (already offset to the layer)
@@ -191,48 +311,47 @@ struct StepArgs {
   // per-step scratch
   uint32_t* maskA; float* pred;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
-  uint32_t* ctl; unsigned long long* stats;
-  int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes;
+  uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
+  int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
   float scale; double score_c;
 };
 
 template <int D, int BS>
 struct Tile {
-  static constexpr int LD = D + 8;               // padded row stride (elements): ldmatrix conflict-free
-  static constexpr int CH = D / 8;               // 16-byte chunks per row
-  static constexpr int BYTES = 2 * BS * LD * 2;  // K tile + V tile
+  // Shared-memory image of one (block, KV head) tile as the copy engine writes it: the K half then
+  // the V half, each D/64 boxes of [BS rows x 128 bytes] in the 128-byte swizzle (the 16-byte
+  // chunk c of row r sits at chunk c ^ (r & 7)), so ldmatrix is conflict-free without padding.
+  static constexpr int NBOX = D / 64;
+  static constexpr int BOX_BYTES = BS * 128;
+  static constexpr int HALF = NBOX * BOX_BYTES;  // = BS * D * 2
+  static constexpr int BYTES = 2 * HALF;         // K tile + V tile
   static constexpr int SUB = BS < 64 ? BS : 64;  // tokens per softmax sub-tile
-  static constexpr int WFIT = (220 * 1024) / BYTES;
+  static constexpr int WFIT = (216 * 1024) / (BYTES + 1024);
   static constexpr int WMAX = WFIT < 12 ? WFIT : 12;  // warps per CTA (one tile buffer each)
+  __device__ static __forceinline__ const unsigned char* at(const unsigned char* half, int r, int c) {
+    return half + (c >> 3) * BOX_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+  }
 };
 
-// Issue the cp.async loads of one (block, KV head) tile; rows >= valid are zero-filled (unwritten
-// cache slots may hold anything, and 0 * NaN must not reach the PV product).  Two commit groups:
-// K first, so QK^T can start while V is still in flight.
+// Put the TMA loads of one (block, KV head) tile in flight: bars[0] completes when K has landed,
+// bars[1] when V has, so QK^T can start while V is still in flight.  The whole block is fetched;
+// rows >= valid (unwritten cache slots of the open block) are masked / zeroed by tile_compute.
 template <int D, int BS>
-__device__ __forceinline__ void tile_load(uint16_t* Ks, const StepArgs& a, int b, int h, int blk, int valid) {
+__device__ __forceinline__ void tile_load(unsigned char* Ks, unsigned long long* bars, const StepArgs& a, int b,
+                                          int h, int blk) {
   using T = Tile<D, BS>;
-  const int lane = threadIdx.x & 31;
-  uint16_t* Vs = Ks + BS * T::LD;
-  const size_t page = (size_t)__ldg(a.table + (size_t)b * a.MB + blk);
-  const uint16_t* gK = a.kp + ((page * a.Hkv + h) * BS) * (size_t)D;
-  const uint16_t* gV = a.vp + ((page * a.Hkv + h) * BS) * (size_t)D;
-#pragma unroll 8
-  for (int i = 0; i < (BS * T::CH) / 32; ++i) {
-    const int c = lane + i * 32, row = c / T::CH, col = c % T::CH;
-    uint16_t* dst = Ks + row * T::LD + col * 8;
-    if (row < valid) cp_async16(dst, gK + row * D + col * 8);
-    else *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
+  fence_proxy_async();  // this buffer was last touched through the generic proxy
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) {
+    const int page = __ldg(a.table + (size_t)b * a.MB + blk);
+    const int y = (page * a.Hkv + h) * BS;
+    mbar_expect_tx(&bars[0], T::HALF);
+#pragma unroll
+    for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + i * T::BOX_BYTES, &a.mapK, i * 64, y, &bars[0]);
+    mbar_expect_tx(&bars[1], T::HALF);
+#pragma unroll
+    for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + T::HALF + i * T::BOX_BYTES, &a.mapV, i * 64, y, &bars[1]);
   }
-  cp_async_commit();
-#pragma unroll 8
-  for (int i = 0; i < (BS * T::CH) / 32; ++i) {
-    const int c = lane + i * 32, row = c / T::CH, col = c % T::CH;
-    uint16_t* dst = Vs + row * T::LD + col * 8;
-    if (row < valid) cp_async16(dst, gV + row * D + col * 8);
-    else *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
-  }
-  cp_async_commit();
 }
 
 // Per-block partial state (the forward also writes l and m) by ONE warp from its
@@ -241,11 +360,12 @@ __device__ __forceinline__ void tile_load(uint16_t* Ks, const StepArgs& a, int b
 // The state is relative to the BLOCK-LOCAL maximum, so a block's partial is the same bits whether
 // it was computed speculatively, as a repair, or by the sequential path.
 template <int D, int BS>
-__device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs& a, int b, int h, int valid,
-                                             float* O, float* Mo, float* Lo, int width, int slot) {
+__device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long long* bars, uint32_t phase,
+                                             const StepArgs& a, int b, int h, int valid, float* O, float* Mo,
+                                             float* Lo, int width, int slot) {
   using T = Tile<D, BS>;
-  constexpr int LD = T::LD, SUB = T::SUB, NT8 = SUB / 8;
-  const uint16_t* Vs = Ks + BS * LD;
+  constexpr int SUB = T::SUB, NT8 = SUB / 8;
+  unsigned char* Vs = Ks + T::HALF;
   const int lane = threadIdx.x & 31;
   const int r0 = lane >> 2, tq = lane & 3, mat = lane >> 3, rr = lane & 7;
   const int G = a.G;
@@ -270,8 +390,7 @@ __device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs&
   float mrun0 = -CUDART_INF_F, mrun1 = -CUDART_INF_F, l0 = 0.f, l1 = 0.f;  // raw-logit max, denominators
   const float sl2 = a.scale * LOG2E_F;
 
-  cp_async_wait<1>();  // K landed
-  __syncwarp();
+  mbar_wait(&bars[0], phase);  // K landed
 #pragma unroll
   for (int st = 0; st < BS / SUB; ++st) {
     const int tok0 = st * SUB;
@@ -285,7 +404,7 @@ __device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs&
 #pragma unroll
       for (int k2 = 0; k2 < D / 32; ++k2) {
         uint32_t b0, b1, b2, b3;
-        ldmatrix_x4(b0, b1, b2, b3, Ks + (tok0 + nt * 8 + rr) * LD + k2 * 32 + mat * 8);
+        ldmatrix_x4(b0, b1, b2, b3, T::at(Ks, tok0 + nt * 8 + rr, k2 * 4 + mat));
         mma_bf16_16816(s[nt], qa[2 * k2], b0, b1);
         mma_bf16_16816(s[nt], qa[2 * k2 + 1], b2, b3);
       }
@@ -314,7 +433,16 @@ __device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs&
       for (int dt = 0; dt < D / 8; ++dt) { o[dt][0] *= f0; o[dt][1] *= f0; o[dt][2] *= f1; o[dt][3] *= f1; }
     }
     mrun0 = mn0; mrun1 = mn1;
-    if (st == 0) { cp_async_wait<0>(); __syncwarp(); }  // V landed
+    if (st == 0) {
+      mbar_wait(&bars[1], phase);  // V landed
+      if (valid < BS) {            // open block: 0 * (whatever an unwritten slot holds) must not reach P V
+        for (int i = lane; i < (BS - valid) * T::NBOX * 8; i += 32) {
+          const int r = valid + i / (T::NBOX * 8), c = i % (T::NBOX * 8);
+          *reinterpret_cast<uint4*>(Vs + (c >> 3) * T::BOX_BYTES + r * 128 + ((c & 7) << 4)) = make_uint4(0, 0, 0, 0);
+        }
+        __syncwarp();
+      }
+    }
     float ls0 = 0.f, ls1 = 0.f;
 #pragma unroll
     for (int kk = 0; kk < SUB / 16; ++kk) {
@@ -336,7 +464,7 @@ __device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs&
       for (int d2 = 0; d2 < D / 16; ++d2) {
         uint32_t b0, b1, b2, b3;
         ldmatrix_x4_trans(b0, b1, b2, b3,
-                          Vs + (tok0 + kk * 16 + (mat & 1) * 8 + rr) * LD + d2 * 16 + (mat >> 1) * 8);
+                          T::at(Vs, tok0 + kk * 16 + (mat & 1) * 8 + rr, d2 * 2 + (mat >> 1)));
         mma_bf16_16816(o[2 * d2], pa, b0, b1);
         mma_bf16_16816(o[2 * d2], pb, b0, b1);
         mma_bf16_16816(o[2 * d2 + 1], pa, b2, b3);
@@ -368,21 +496,28 @@ __device__ __forceinline__ void tile_compute(const uint16_t* Ks, const StepArgs&
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1: one chunk of summary rows of (b, h): sub-warps of D/8 lanes own a row (one 16-byte load per
-// lane), the group's queries are pre-summed per channel in fp64, products and sums are exact (Q1).
+// a1: one chunk of CR summary rows of (b, h): sub-warps of D/8 lanes own a row (one 16-byte load
+// per lane), the group's queries are pre-summed per channel in fp64, products and sums are exact
+// (Q1).  Split in two so the loads are in flight while the warp issues its tile prefetch.
+constexpr int SC_UNR = 16;
+
 template <int D>
-__device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int row0, int nb) {
-  constexpr int LPR = D / 8, RW = 32 / LPR, UNR = 8;
+__device__ __forceinline__ void score_load(const StepArgs& a, int b, int h, int row0, int nb, uint4 (&v)[SC_UNR]) {
+  constexpr int LPR = D / 8, RW = 32 / LPR;
   const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
   const uint4* rows = a.summ + ((size_t)b * a.Hkv + h) * a.MB * LPR;
-  const int rbase = row0 + sub;
-  uint4 v[UNR];
 #pragma unroll
-  for (int u = 0; u < UNR; ++u) {
-    const int r = rbase + u * RW;
+  for (int u = 0; u < SC_UNR; ++u) {
+    const int r = row0 + sub + u * RW;
     v[u] = r < nb ? __ldg(rows + (size_t)r * LPR + l) : make_uint4(0, 0, 0, 0);
   }
-  double qs[8];
+}
+
+// the group's queries summed per channel (exact in fp64): the 8 channels this lane owns
+template <int D>
+__device__ __forceinline__ void score_qsum(const StepArgs& a, int b, int h, double (&qs)[8]) {
+  constexpr int LPR = D / 8;
+  const int l = (threadIdx.x & 31) % LPR;
 #pragma unroll
   for (int j = 0; j < 8; ++j) qs[j] = 0.0;
   const uint16_t* qb = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D + l * 8;
@@ -395,9 +530,16 @@ __device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int
       qs[2 * j + 1] += (double)bf16_hi(w[j]);
     }
   }
+}
+
+template <int D>
+__device__ __forceinline__ void score_finish(const StepArgs& a, int b, int h, int row0, int nb,
+                                             const uint4 (&v)[SC_UNR], const double (&qs)[8]) {
+  constexpr int LPR = D / 8, RW = 32 / LPR;
+  const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
   float* out = a.scores + ((size_t)b * a.Hkv + h) * a.MB;
 #pragma unroll
-  for (int u = 0; u < UNR; ++u) {
+  for (int u = 0; u < SC_UNR; ++u) {
     const uint32_t w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
     double acc = 0.0;
 #pragma unroll
@@ -407,68 +549,66 @@ __device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int
     }
 #pragma unroll
     for (int off = LPR / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(FULL, acc, off);
-    const int r = rbase + u * RW;
+    const int r = row0 + sub + u * RW;
     if (l == 0 && r < nb) out[r] = f64_to_score(__dmul_rn(acc, a.score_c));
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // a5 preparation, independent of the scores (runs while they are being computed): bitmask of the
-// predicted set P in the warp's scratch.  Returns |P|.
-__device__ int select_prepare(const StepArgs& a, int row, uint32_t* scr, const int32_t* Pcur) {
-  const int lane = threadIdx.x & 31;
-  uint32_t* pmask = scr;  // [MBw]
-  for (int w = lane; w < a.MBw; w += 32) pmask[w] = 0u;
-  __syncwarp();
-  int np = 0;
+// predicted set P in the team's shared memory.  Returns |P| in every thread.
+__device__ int select_prepare(const StepArgs& a, int row, const Team& tm, const TeamMem& m, const int32_t* Pcur) {
+  uint32_t* dec = m.red + tm.nw * 16;
+  for (int w = tm.tid; w < a.MBw; w += tm.nt) m.pmask[w] = 0u;
+  if (tm.tid == 0) dec[4] = 0u;
+  tm.sync();
   if (a.spec) {
     const int32_t* P = Pcur + (size_t)row * a.Bud;
-    for (int j = lane; j < a.Bud; j += 32) {
+    int np = 0;
+    for (int j = tm.tid; j < a.Bud; j += tm.nt) {
       const int blk = __ldg(P + j);
-      if (blk >= 0 && blk < a.MB) { atomicOr(&pmask[blk >> 5], 1u << (blk & 31)); ++np; }
+      if (blk >= 0 && blk < a.MB) { atomicOr(&m.pmask[blk >> 5], 1u << (blk & 31)); ++np; }
     }
+    np = __reduce_add_sync(FULL, np);
+    if ((threadIdx.x & 31) == 0 && np) atomicAdd(&dec[4], (uint32_t)np);
   }
-  np = __reduce_add_sync(FULL, np);
-  __syncwarp();
-  return np;
+  tm.sync();
+  return (int)dec[4];
 }
 
-// a2 + a5 for one (sequence, KV head) row, by one warp, once the row's scores are complete.
-__device__ void job_select(const StepArgs& a, int row, uint32_t* scr, int np) {
-  const int lane = threadIdx.x & 31;
-  const uint32_t lt = (1u << lane) - 1u;
+// a2 + a5 for one (sequence, KV head) row, by one team, once the row's scores are complete.
+__device__ void job_select(const StepArgs& a, int row, const Team& tm, const TeamMem& m, int np, unsigned long long* tl) {
   const int b = row / a.Hkv;
   const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
-  const int nw = (nb + 31) >> 5;
-  const uint32_t* pmask = scr;           // [MBw]
-  uint32_t* candk = scr + a.MBw;         // [64]
-  int32_t* candi = reinterpret_cast<int32_t*>(candk + 64);
   uint32_t* ctl = a.ctl;
   const float* sc = a.scores + (size_t)row * a.MB;
   const int k = min(a.K, nb);
-  Thr t;
-  t.key = 0u; t.idx = 0x7fffffff;      // k >= n: everything is selected
-  if (k < nb) t = warp_kth(sc, nb, k, candk, candi);
-  int32_t* A_row = a.setA + (size_t)row * a.K;
-  int32_t* M_row = a.setM + (size_t)row * a.K;
-  uint32_t* mA = a.maskA + (size_t)row * a.MBw;
-  int nA = 0, nM = 0;
-  for (int j = 0; j < nw; ++j) {
-    const int i = j * 32 + lane;
-    const bool sel = i < nb && k > 0 && selected(key_at(sc, i), i, t);
-    const uint32_t aw = __ballot_sync(FULL, sel);
-    const uint32_t mw = aw & ~pmask[j];
-    if (sel) {
-      A_row[nA + __popc(aw & lt)] = i;
-      if ((mw >> lane) & 1u) M_row[nM + __popc(mw & lt)] = i;
-    }
-    if (lane == 0) mA[j] = aw;
-    nA += __popc(aw);
-    nM += __popc(mw);
+  const bool in_sm = nb <= m.key_cap;
+  uint32_t kmin = 0xffffffffu, kmax = 0u;
+#pragma unroll 8
+  for (int i = tm.tid; i < nb; i += tm.nt) {
+    const uint32_t key = score_key(__ldcg(sc + i));
+    if (in_sm) m.keys[i] = key;
+    kmin = min(kmin, key);
+    kmax = max(kmax, key);
   }
-  for (int j = nA + lane; j < a.K; j += 32) A_row[j] = -1;
-  for (int j = nM + lane; j < a.K; j += 32) M_row[j] = -1;
-  if (lane == 0) {
+  Keys ks{in_sm ? smem_u32(m.keys) : 0u, sc};
+  Thr t;
+  t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
+  if (k < nb) {                     // (uniform over the team)
+    uint32_t lo, span;
+    team_range(kmin, kmax, tm, m, lo, span);
+    if (tl && tm.tid == 0) tl[9] = gtime();
+    t = team_kth(ks, nb, k, tm, m, lo, span);
+  } else {
+    tm.sync();
+  }
+  if (tl && tm.tid == 0) tl[10] = gtime();
+  const uint32_t tot = team_emit(ks, nb, k, t, tm, m, a.setA + (size_t)row * a.K, a.K,
+                                 a.maskA + (size_t)row * a.MBw, a.setM + (size_t)row * a.K, a.K);
+  const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
+  if (tl && tm.tid == 0) tl[11] = gtime();
+  if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
     a.counts[row * 3 + 1] = np;
     a.counts[row * 3 + 2] = nM;
@@ -480,19 +620,21 @@ __device__ void job_select(const StepArgs& a, int row, uint32_t* scr, int np) {
     }
     ctl[CTL_HDR + 3 * a.Rmax + row] = (uint32_t)(np + nM);
     ctl[CTL_HDR + 4 * a.Rmax + row] = (uint32_t)nM;
+    atomicMax(&ctl[CTL_MAXM], (uint32_t)nM);
   }
-  signal_add(&ctl[CTL_HDR + 1 * a.Rmax + row], 1u);
+  __threadfence();
+  tm.sync();
+  if (tm.tid == 0) {
+    atomicAdd(&ctl[CTL_HDR + 1 * a.Rmax + row], 1u);
+    atomicAdd(&ctl[CTL_SELDONE], 1u);  // CTL_MAXM was raised before the fence above
+  }
 }
 
-// a8 + a3 for one row, by one warp: Eq. 3 in non-contracted fp64 (both lines use l^{t-1}; blocks
+// a8 + a3 for one row, by one team: Eq. 3 in non-contracted fp64 (both lines use l^{t-1}; blocks
 // scored for the first time get l = IS, v = 0), Eq. 2 rounded once to fp32, then the
 // same exact selection for P = top-min(Bud, #stateful) of the next step.
-__device__ void job_ema(const StepArgs& a, int row, uint32_t* scr, int32_t* Pnext) {
-  const int lane = threadIdx.x & 31;
-  const uint32_t lt = (1u << lane) - 1u;
+__device__ void job_ema(const StepArgs& a, int row, const Team& tm, const TeamMem& m, int32_t* Pnext, unsigned long long* tl) {
   const int b = row / a.Hkv;
-  uint32_t* candk = scr + a.MBw;
-  int32_t* candi = reinterpret_cast<int32_t*>(candk + 64);
   double* L = a.ema_l + (size_t)row * a.MB;
   double* V = a.ema_v + (size_t)row * a.MB;
   const double alpha = a.theta[b * 3 + 0], beta = a.theta[b * 3 + 1], gamma = a.theta[b * 3 + 2];
@@ -502,43 +644,59 @@ __device__ void job_ema(const StepArgs& a, int row, uint32_t* scr, int32_t* Pnex
   const int n_new = max(n, n_old);
   const float* sc = a.scores + (size_t)row * a.MB;
   float* pr = a.pred + (size_t)row * a.MB;
-  for (int i = lane; i < n_new; i += 32) {
-    double ln, vn;
-    if (i < n) {
-      const double x = (double)__ldcg(sc + i);
-      if (i < n_old) {
-        const double lo = L[i], vo = V[i];
-        vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(x, lo)), __dmul_rn(omb, vo));
-        ln = __dadd_rn(__dmul_rn(alpha, x), __dmul_rn(oma, lo));
-      } else {
-        ln = x;
-        vn = 0.0;
-      }
-      L[i] = ln;
-      V[i] = vn;
-    } else {
-      ln = L[i];
-      vn = V[i];
+  const bool in_sm = n_new <= m.key_cap;
+  uint32_t kmin = 0xffffffffu, kmax = 0u;
+  constexpr int EB = 6;  // elements per thread whose loads are in flight together
+  for (int i0 = tm.tid; i0 < n_new; i0 += EB * tm.nt) {
+    float x[EB];
+    double lo_[EB], vo_[EB];
+#pragma unroll
+    for (int e = 0; e < EB; ++e) {
+      const int i = i0 + e * tm.nt;
+      x[e] = i < n ? __ldcg(sc + i) : 0.f;
+      const bool has = i < n_new && (i < n_old || i >= n);
+      lo_[e] = has ? L[i] : 0.0;
+      vo_[e] = has ? V[i] : 0.0;
     }
-    pr[i] = f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn)));
+#pragma unroll
+    for (int e = 0; e < EB; ++e) {
+      const int i = i0 + e * tm.nt;
+      if (i >= n_new) break;
+      double ln = lo_[e], vn = vo_[e];
+      if (i < n) {
+        const double xd = (double)x[e];
+        if (i < n_old) {
+          vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, lo_[e])), __dmul_rn(omb, vo_[e]));
+          ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, lo_[e]));
+        } else {
+          ln = xd;
+          vn = 0.0;
+        }
+        L[i] = ln;
+        V[i] = vn;
+      }
+      const float p = f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn)));
+      const uint32_t key = score_key(p);
+      if (in_sm) m.keys[i] = key; else pr[i] = p;
+      kmin = min(kmin, key);
+      kmax = max(kmax, key);
+    }
   }
-  __syncwarp();
-  if (lane == 0) a.n_state[row] = n_new;
+  tm.sync();  // n_state is read by every thread above, written below
+  if (tm.tid == 0) a.n_state[row] = n_new;
   if (a.Bud <= 0) return;
-  int32_t* P_row = Pnext + (size_t)row * a.Bud;
   const int k = min(a.Bud, n_new);
+  Keys ks{in_sm ? smem_u32(m.keys) : 0u, pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;
-  if (k < n_new) t = warp_kth(pr, n_new, k, candk, candi);
-  int cnt = 0;
-  for (int j0 = 0; j0 < n_new; j0 += 32) {
-    const int i = j0 + lane;
-    const bool sel = i < n_new && k > 0 && selected(key_at(pr, i), i, t);
-    const uint32_t w = __ballot_sync(FULL, sel);
-    if (sel) P_row[cnt + __popc(w & lt)] = i;
-    cnt += __popc(w);
+  if (k < n_new) {
+    uint32_t lo, span;
+    team_range(kmin, kmax, tm, m, lo, span);
+    if (tl && tm.tid == 0) tl[9] = gtime();
+    t = team_kth(ks, n_new, k, tm, m, lo, span);
   }
-  for (int j = cnt + lane; j < a.Bud; j += 32) P_row[j] = -1;
+  if (tl && tm.tid == 0) tl[10] = gtime();
+  team_emit(ks, n_new, k, t, tm, m, Pnext + (size_t)row * a.Bud, a.Bud, nullptr, nullptr, 0);
 }
 
 // a7 for one (sequence, query head): Eq. 6-8 over the listed partial states, O unnormalised and
@@ -555,6 +713,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
   const int E = a.Bud + a.K;
   float* ws = reinterpret_cast<float*>(buf);             // [E] m, then weights
   uint32_t* cs = reinterpret_cast<uint32_t*>(buf) + E;   // [E] slot codes (REP bit: repair buffers)
+  float* ls = reinterpret_cast<float*>(buf) + 2 * E;     // [E] l
   const int np = a.spec ? __ldcg(a.counts + row * 3 + 1) : 0;
   const int nM = __ldcg(a.counts + row * 3 + 2);
   const uint32_t* mA = a.maskA + (size_t)row * a.MBw;
@@ -566,15 +725,18 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
   for (int j0 = 0; j0 < np; j0 += 32) {
     const int j = j0 + lane;
     bool use = false;
+    float me = 0.f, le = 0.f;
     if (j < np) {
       const int blk = __ldg(Pcur + (size_t)row * a.Bud + j);
+      me = __ldcg(a.m_spec + hb * a.Bud + j);
+      le = __ldcg(a.l_spec + hb * a.Bud + j);
       use = a.retain || ((__ldcg(mA + (blk >> 5)) >> (blk & 31)) & 1u);
     }
     const uint32_t bal = __ballot_sync(FULL, use);
     if (use) {
       const int e = n + __popc(bal & lt);
-      const float me = __ldcg(a.m_spec + hb * a.Bud + j);
       ws[e] = me;
+      ls[e] = le;
       cs[e] = (uint32_t)j;
       mx = fmaxf(mx, me);
     }
@@ -584,6 +746,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
   for (int j = lane; j < nM; j += 32) {
     const float me = __ldcg(a.m_rep + hb * a.K + j);
     ws[n + j] = me;
+    ls[n + j] = __ldcg(a.l_rep + hb * a.K + j);
     cs[n + j] = (uint32_t)j | REP;
     mx = fmaxf(mx, me);
   }
@@ -594,17 +757,15 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
   float lsum = 0.f;
   for (int e = lane; e < n; e += 32) {
     const float me = ws[e];
-    const uint32_t code = cs[e];
     const float w = me == -CUDART_INF_F ? 0.f : ex2((me - mx) * LOG2E_F);
-    const float le = (code & REP) ? __ldcg(a.l_rep + hb * a.K + (code & ~REP)) : __ldcg(a.l_spec + hb * a.Bud + code);
     ws[e] = w;
-    lsum = fmaf(w, le, lsum);
+    lsum = fmaf(w, ls[e], lsum);
   }
 #pragma unroll
   for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
   __syncwarp();
   float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll 8
+#pragma unroll 16
   for (int e = 0; e < n; ++e) {
     const float w = ws[e];
     const uint32_t code = cs[e];
@@ -627,14 +788,20 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
 // ---------------------------------------------------------------------------------------------
 template <int D, int BS>
 __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid_constant__ StepArgs a) {
-  using T = Tile<D, BS>;
-  constexpr int LPR = D / 8, CR = (32 / LPR) * 8;  // summary rows per score chunk
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int LPR = D / 8, BR = (32 / LPR) * SC_UNR;  // summary rows per batch of loads
+  const int CR = a.CR;                                   // rows per score chunk (a multiple of BR)
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  __shared__ __align__(8) unsigned long long bars_all[2 * 12];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
-  const int gw = warp * gridDim.x + blockIdx.x, NW = W * gridDim.x;  // consecutive ids sit on different SMs
-  unsigned char* buf = smem_raw + (size_t)warp * (a.buf_bytes + a.scr_bytes);
-  uint16_t* Ks = reinterpret_cast<uint16_t*>(buf);
-  uint32_t* scr = reinterpret_cast<uint32_t*>(buf + a.buf_bytes);
+  const int NC = gridDim.x, NW = W * NC;
+  const int gw = warp * NC + blockIdx.x;  // consecutive ids sit on different SMs
+  const int per_warp = a.buf_bytes + a.scr_bytes;
+  unsigned char* buf = smem_raw + (size_t)warp * per_warp;
+  unsigned char* Ks = buf;
+  unsigned long long* bars = bars_all + 2 * warp;
+  uint32_t ph = 0;  // parity of the next tile to land in this warp's buffer
+  if (lane == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init(); }
+  __syncwarp();
   uint32_t* ctl = a.ctl;
   uint32_t* score_done = ctl + CTL_HDR;
   uint32_t* sel_flag = ctl + CTL_HDR + a.Rmax;
@@ -645,10 +812,19 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   const int par = *a.parity & 1;
   const int32_t* Pcur = par ? a.P1 : a.P0;
   int32_t* Pnext = par ? a.P0 : a.P1;
+  unsigned long long* tl = a.tl ? a.tl + ((size_t)blockIdx.x * W + warp) * 16 : nullptr;
+  if (tl && lane == 0) tl[0] = gtime();
 
-  // ---- phase 0: first speculative tile in flight -------------------------------------------
+  // Roles.  Team mode (J = 2R job CTAs at the end of the grid): the job CTAs' warps are ranked
+  // after every worker warp, so speculative units land on worker CTAs first.
+  const int NWK = NC - a.J;
+  const bool job_cta = (int)blockIdx.x >= NWK;
+  const bool job_warp = a.J == 0 && (NW - 1 - gw) < 2 * R;  // warp mode: highest-numbered warps
+  const int rank = !job_cta ? warp * NWK + (int)blockIdx.x : NWK * W + warp * a.J + ((int)blockIdx.x - NWK);
+
+  // first speculative unit of this warp
   const int U = a.spec ? R * a.Bud : 0;
-  int u = gw;
+  int u = rank;
   int ub = 0, uh = 0, ublk = -1, uvalid = 0;
   auto unit_decode = [&](int unit) {
     const int slot = unit / R, row = unit - slot * R;
@@ -657,72 +833,163 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     if (ublk >= a.MB) ublk = -1;
     uvalid = ublk >= 0 ? min(BS, __ldg(a.seq_lens + ub) - ublk * BS) : 0;
   };
-  if (u < U) {
-    unit_decode(u);
-    if (ublk >= 0) tile_load<D, BS>(Ks, a, ub, uh, ublk, uvalid);
-  }
+  const bool prefetch = !job_cta && !job_warp && u < U;
+  if (prefetch) unit_decode(u);
+  if (tl && lane == 0) tl[6] = gtime() + (unsigned long long)(ublk & 0);
 
-  // ---- phase 1: scores ----------------------------------------------------------------------
+  // ---- phase 1: scores; the first tile goes in flight right behind the first chunk's loads ------
   {
     const int cpr = (a.MB + CR - 1) / CR;  // chunks per row (static upper bound)
+    bool issued = !prefetch;
     for (int it = gw; it < R * cpr; it += NW) {
       const int ch = it / R, row = it - ch * R;
       const int b = row / a.Hkv, h = row - b * a.Hkv;
       const int nb = min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs);
       if (ch * CR >= nb) continue;
-      score_chunk<D>(a, b, h, ch * CR, nb);
+      double qs[8];
+      for (int r0 = ch * CR; r0 < min(nb, (ch + 1) * CR); r0 += BR) {
+        uint4 v[SC_UNR];
+        score_load<D>(a, b, h, r0, nb, v);
+        if (r0 == ch * CR) score_qsum<D>(a, b, h, qs);
+        if (!issued) {
+          if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
+          issued = true;
+          if (tl && lane == 0) tl[7] = gtime();
+        }
+        score_finish<D>(a, b, h, r0, nb, v, qs);
+      }
       signal_add(&score_done[row], 1u);
     }
+    if (!issued && ublk >= 0) { tile_load<D, BS>(Ks, bars, a, ub, uh, ublk); if (tl && lane == 0) tl[7] = gtime(); }
   }
+  if (tl && lane == 0) tl[1] = gtime();
 
-  // ---- phase 2: row jobs on the highest-numbered warps --------------------------------------
-  for (int jj = NW - 1 - gw; jj < 2 * R; jj += NW) {
+  // ---- phase 2: row jobs -------------------------------------------------------------------------
+  if (job_cta) {
+    const int jj = (int)blockIdx.x - NWK;
     const int row = jj < R ? jj : jj - R;
     const int b = row / a.Hkv;
     const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
+    Team tm{(int)threadIdx.x, (int)blockDim.x, warp, W, true};
+    TeamMem m;
+    uint32_t* p = reinterpret_cast<uint32_t*>(smem_raw);
+    m.pmask = p; p += a.MBw;
+    m.amask = p; p += a.MBw;
+    m.offs = p; p += a.MBw;
+    m.red = p; p += W * 16 + 8;
+    m.hist = p; p += 2048; m.hbits = 11;
+    for (int i = threadIdx.x; i < 2048; i += blockDim.x) m.hist[i] = 0u;
+    m.candk = p; p += 64;
+    m.candi = reinterpret_cast<int32_t*>(p); p += 64;
+    m.keys = p;
+    m.key_cap = (int)(((size_t)W * per_warp - (size_t)((unsigned char*)p - smem_raw)) / 4);
     int np = 0;
-    if (jj < R) np = select_prepare(a, row, scr, Pcur);
-    wait_ge(&score_done[row], (uint32_t)((nb + CR - 1) / CR), &ctl[CTL_ERR]);
-    if (jj < R) job_select(a, row, scr, np);
-    else job_ema(a, row, scr, Pnext);
+    if (jj < R) np = select_prepare(a, row, tm, m, Pcur);
+    if (threadIdx.x == 0) {
+      uint32_t it = 0;
+      const uint32_t target = (uint32_t)((nb + CR - 1) / CR);
+      while (ld_acquire(&score_done[row]) < target) {
+        __nanosleep(20);
+        if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); break; }
+      }
+    }
+    __syncthreads();
+    if (tl && threadIdx.x == 0) tl[8] = gtime();
+    if (jj < R) job_select(a, row, tm, m, np, tl);
+    else job_ema(a, row, tm, m, Pnext, tl);
+    __syncthreads();  // the team's memory becomes per-warp tile buffers again
+  } else if (job_warp) {
+    Team tm{lane, 32, 0, 1, false};
+    TeamMem m;
+    uint32_t* p = reinterpret_cast<uint32_t*>(buf + a.buf_bytes);
+    m.pmask = p; p += a.MBw;
+    m.amask = p; p += a.MBw;
+    m.offs = p; p += a.MBw;
+    m.red = p; p += 16 + 8;
+    m.hist = p; p += 256; m.hbits = 8;
+    for (int i = lane; i < 256; i += 32) m.hist[i] = 0u;
+    m.candk = p; p += 64;
+    m.candi = reinterpret_cast<int32_t*>(p);
+    m.keys = reinterpret_cast<uint32_t*>(buf);
+    m.key_cap = a.buf_bytes / 4;
+    for (int jj = NW - 1 - gw; jj < 2 * R; jj += NW) {
+      const int row = jj < R ? jj : jj - R;
+      const int b = row / a.Hkv;
+      const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
+      int np = 0;
+      if (jj < R) np = select_prepare(a, row, tm, m, Pcur);
+      wait_ge(&score_done[row], (uint32_t)((nb + CR - 1) / CR), &ctl[CTL_ERR]);
+      if (jj < R) job_select(a, row, tm, m, np, tl);
+      else job_ema(a, row, tm, m, Pnext, tl);
+      __syncwarp();
+    }
   }
+  if (tl && lane == 0) tl[2] = gtime();
 
   // ---- phase 3: speculative units -------------------------------------------------------------
+  if (!prefetch && u < U) {  // job warps start their units only now
+    unit_decode(u);
+    if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
+  }
   while (u < U) {
     const int slot = u / R, row = u - slot * R;
     const int cb = ub, chh = uh, cvalid = uvalid;
     const bool real = ublk >= 0;
-    if (real) tile_compute<D, BS>(Ks, a, cb, chh, cvalid, a.O_spec, a.m_spec, a.l_spec, a.Bud, slot);
+    if (real) { tile_compute<D, BS>(Ks, bars, ph, a, cb, chh, cvalid, a.O_spec, a.m_spec, a.l_spec, a.Bud, slot); ph ^= 1u; }
     u += NW;
     if (u < U) {  // refill the buffer before publishing: the next tile's latency starts now
       unit_decode(u);
-      if (ublk >= 0) tile_load<D, BS>(Ks, a, ub, uh, ublk, uvalid);
+      if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
     }
     if (real) signal_add(&units_done[row], 1u);
   }
+  if (tl && lane == 0) tl[3] = gtime();
 
-  // ---- phase 4: repair units --------------------------------------------------------------------
-  for (int it = gw; it < R * a.K; it += NW) {
-    const int slot = it / R, row = it - slot * R;
-    wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
-    const int nM = (int)__ldcg(nM_g + row);
-    if (slot >= nM) continue;
-    const int b = row / a.Hkv, h = row - b * a.Hkv;
-    const int blk = __ldcg(a.setM + (size_t)row * a.K + slot);
-    const int valid = min(BS, __ldg(a.seq_lens + b) - blk * BS);
-    tile_load<D, BS>(Ks, a, b, h, blk, valid);
-    tile_compute<D, BS>(Ks, a, b, h, valid, a.O_rep, a.m_rep, a.l_rep, a.K, slot);
-    signal_add(&units_done[row], 1u);
+  // ---- phase 4: repair units, claimed by whoever is free ---------------------------------------
+  {
+    const int NT = R * a.K;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = (int)atomicAdd(&ctl[CTL_RTICKET], 1u);
+      t = __shfl_sync(FULL, t, 0);
+      if (t >= NT) break;
+      const int slot = t / R, row = t - slot * R;
+      wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
+      const int nM = (int)__ldcg(nM_g + row);
+      if (slot >= nM) {
+        // a void ticket; once every row is selected and no row has this many misses, all later ones are too
+        uint32_t stop = 0;
+        if (lane == 0) stop = ld_acquire(&ctl[CTL_SELDONE]) >= (uint32_t)R && (uint32_t)slot >= ld_acquire(&ctl[CTL_MAXM]);
+        if (__shfl_sync(FULL, stop, 0)) break;
+        continue;
+      }
+      const int b = row / a.Hkv, h = row - b * a.Hkv;
+      const int blk = __ldcg(a.setM + (size_t)row * a.K + slot);
+      const int valid = min(BS, __ldg(a.seq_lens + b) - blk * BS);
+      tile_load<D, BS>(Ks, bars, a, b, h, blk);
+      tile_compute<D, BS>(Ks, bars, ph, a, b, h, valid, a.O_rep, a.m_rep, a.l_rep, a.K, slot);
+      ph ^= 1u;
+      signal_add(&units_done[row], 1u);
+    }
   }
+  if (tl && lane == 0) tl[4] = gtime();
 
-  // ---- phase 5: merge ---------------------------------------------------------------------------
-  for (int it = gw; it < a.B * a.Hq; it += NW) {
-    const int b = it / a.Hq, hq = it - b * a.Hq;
-    const int row = b * a.Hkv + hq / a.G;
-    wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
-    wait_ge(&units_done[row], __ldcg(units_total + row), &ctl[CTL_ERR]);
-    job_merge<D>(a, b, hq, buf, Pcur);
+  // ---- phase 5: merge, claimed by whoever is free ------------------------------------------------
+  {
+    const int NT = a.B * a.Hq;
+    for (;;) {
+      int t = 0;
+      if (lane == 0) t = (int)atomicAdd(&ctl[CTL_MTICKET], 1u);
+      t = __shfl_sync(FULL, t, 0);
+      if (t >= NT) break;
+      const int b = t / a.Hq, hq = t - b * a.Hq;
+      const int row = b * a.Hkv + hq / a.G;
+      wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
+      wait_ge(&units_done[row], __ldcg(units_total + row), &ctl[CTL_ERR]);
+      job_merge<D>(a, b, hq, buf, Pcur);
+    }
   }
+  if (tl && lane == 0) tl[5] = gtime();
 
   // ---- exit: the last warp of the grid resets the step's counters and flips the parity ---------
   __syncwarp();
@@ -734,7 +1001,10 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   last = __shfl_sync(FULL, last, 0);
   if (last) {
     for (int i = lane; i < 5 * a.Rmax; i += 32) ctl[CTL_HDR + i] = 0u;
-    if (lane == 0) { ctl[CTL_EXIT] = 0u; *a.parity = par ^ 1; }
+    if (lane == 0) {
+      ctl[CTL_EXIT] = 0u; ctl[CTL_RTICKET] = 0u; ctl[CTL_MTICKET] = 0u; ctl[CTL_SELDONE] = 0u; ctl[CTL_MAXM] = 0u;
+      *a.parity = par ^ 1;
+    }
   }
 }
 
@@ -743,17 +1013,34 @@ template <int D, int BS>
 static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s) {
   using T = Tile<D, BS>;
   StepArgs a = a0;
-  const int merge_bytes = (c->Bud + c->K) * 8;
+  const int merge_bytes = (c->Bud + c->K) * 12;
+  const int R = a.B * a.Hkv;
   a.buf_bytes = (std::max(T::BYTES, merge_bytes) + 15) & ~15;
-  a.scr_bytes = ((a.MBw + 128) * 4 + 15) & ~15;
-  const int per_warp = a.buf_bytes + a.scr_bytes;
-  int W = std::min(T::WMAX, c->smem_optin / per_warp);
-  if (W < 1) return cudaErrorInvalidConfiguration;
+  // Row jobs: a whole CTA per job when rows are few (its bookkeeping lives in the CTA's pooled
+  // buffers), else one warp per job with a 256-bucket histogram in its own scratch.
+  a.J = 2 * R <= c->n_sm / 4 ? 2 * R : 0;
+  int W = 0, per_warp = 0;
+  for (;;) {
+    a.scr_bytes = (3 * a.MBw + 24 + 128 + (a.J ? 0 : 256)) * 4;
+    a.scr_bytes += (1024 - (a.buf_bytes + a.scr_bytes) % 1024) % 1024;  // tile buffers stay 1024-byte aligned (swizzle atom)
+    per_warp = a.buf_bytes + a.scr_bytes;
+    W = std::min(T::WMAX, (c->smem_optin - 1024) / per_warp);
+    if (W < 1) return cudaErrorInvalidConfiguration;
+    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 128 + 64;
+    if (a.J && team_words * 4 > (size_t)W * per_warp) { a.J = 0; continue; }
+    break;
+  }
   const size_t smem = (size_t)W * per_warp;
+  {  // score chunk: about one per warp, a whole number of load batches
+    const int BR = (32 / (D / 8)) * SC_UNR;
+    const long long rows = (long long)R * a.MB, NWh = (long long)W * c->n_sm;
+    a.CR = (int)(((rows + NWh - 1) / NWh + BR - 1) / BR) * BR;
+    if (a.CR < BR) a.CR = BR;
+  }
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute((const void*)k_step<D, BS>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - 1024);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
@@ -770,10 +1057,51 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   return cudaLaunchKernelEx(&cfg, k_step<D, BS>, a);
 }
 
+// Tensor map of a K or V page pool for the copy engine: bf16 [rows, d] with rows = page * Hkv * bs
+// (the library is not told n_pages; tile coordinates are int32, so the row extent is 2^31), box =
+// [bs rows, 64 channels = 128 bytes], 128-byte swizzle.  Encoded on the host, cached per pointer.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+static int page_map(prr_ctx* c, const void* base, CUtensorMap* out) {
+  static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap is 128 bytes");
+  auto it = c->tmaps.find(base);
+  if (it == c->tmaps.end()) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return (int)cudaErrorNotSupported;
+    alignas(64) CUtensorMap m;
+    const cuuint64_t dims[2] = {(cuuint64_t)c->D, (cuuint64_t)1 << 31};
+    const cuuint64_t strides[1] = {(cuuint64_t)c->D * 2};
+    const cuuint32_t box[2] = {64u, (cuuint32_t)c->bs};
+    const cuuint32_t es[2] = {1u, 1u};
+    if (fn(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return (int)cudaErrorInvalidValue;
+    std::array<uint64_t, 16> blob;
+    memcpy(blob.data(), &m, 128);
+    if (c->tmaps.size() > 4096) c->tmaps.clear();
+    it = c->tmaps.emplace(base, blob).first;
+  }
+  memcpy(out, it->second.data(), 128);
+  return 0;
+}
+
 int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
                 int spec, cudaStream_t s) {
   const size_t r = (size_t)kv->layer * c->maxB * c->Hkv;
   StepArgs a{};
+  if (int e = page_map(c, kv->k_pages, &a.mapK)) return e;
+  if (int e = page_map(c, kv->v_pages, &a.mapV)) return e;
   a.kp = (const uint16_t*)kv->k_pages; a.vp = (const uint16_t*)kv->v_pages;
   a.table = kv->block_table; a.seq_lens = kv->seq_lens;
   a.q = (const uint16_t*)q; a.summ = (const uint4*)summaries; a.out = out;
@@ -786,7 +1114,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.maskA = c->maskA; a.pred = c->pred;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
-  a.ctl = c->ctl; a.stats = c->stats;
+  a.ctl = c->ctl; a.stats = c->stats; a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.Rmax = c->maxB * c->Hkv;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;

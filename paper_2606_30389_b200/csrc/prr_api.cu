@@ -128,6 +128,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->maskA, srows * (size_t)((c->MB + 31) / 32)));
   A(dalloc(c, &c->pred, srows * (size_t)c->MB));
   A(dalloc(c, &c->ctl, (size_t)8 + 5 * srows));
+  c->tl_warps = c->n_sm * 32;
+  A(dalloc(c, &c->tl, (size_t)c->tl_warps * 16));
   A(dalloc(c, &c->merge_src, srows * (c->Bud + c->K)));
   A(dalloc(c, &c->merge_n, srows));
   A(dalloc(c, &c->nblk, (size_t)c->maxB));
@@ -611,6 +613,24 @@ extern "C" int32_t prr_check(prr_ctx* ctx, void* stream) {
   PRR_CUDA(ctx, cudaStreamSynchronize(s));
   if (err) PRR_FAIL(ctx, PRR_E_STATE, "prr_check: a fused step gave up waiting on a dependency counter");
   return check_launch(ctx, "prr_check");
+}
+
+extern "C" int32_t prr_timeline_enable(prr_ctx* ctx, int32_t on) {
+  if (!ctx) return PRR_E_INVALID;
+  ctx->tl_on = on ? 1 : 0;
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_timeline_read(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps, int32_t* n_warps_out,
+                                     void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (!stamps_host || max_warps < 1) PRR_FAIL(ctx, PRR_E_INVALID, "prr_timeline_read: bad argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int n = max_warps < ctx->tl_warps ? max_warps : ctx->tl_warps;
+  PRR_CUDA(ctx, cudaMemcpyAsync(stamps_host, ctx->tl, (size_t)n * 16 * sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
+  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  if (n_warps_out) *n_warps_out = n;
+  return PRR_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -3,7 +3,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <array>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/prr.h"
@@ -39,8 +41,10 @@ struct prr_ctx {
   unsigned long long* stats = nullptr; // [4]
   uint32_t* maskA = nullptr;  // [maxB, Hkv, ceil(MB/32)] bitmask of A (fused step)
   float* pred = nullptr;      // [maxB, Hkv, MB] Eq. 2 predictions of the row being ranked (fused step)
-  uint32_t* ctl = nullptr;    // fused step: exit counter, error flag, per-row dependency counters
+  uint32_t* ctl = nullptr;    // fused step: exit counter, error flag, tickets, per-row dependency counters
+  unsigned long long* tl = nullptr; int tl_on = 0, tl_warps = 0; // fused step: per-warp phase stamps (debug)
   int n_sm = 0, smem_optin = 0, fused = 1;
+  std::unordered_map<const void*, std::array<uint64_t, 16>> tmaps; // encoded CUtensorMap per K/V page pool
   // ---- calibration scratch (allocated on first prr_calibrate) ----
   double* cal_state = nullptr; size_t cal_state_elems = 0; // [80, Hkv, N, 2]
   uint32_t* cal_mask = nullptr; size_t cal_mask_words = 0; // [Hkv, T, ceil(N/32)]

@@ -22,6 +22,7 @@ SYMBOLS = [
     "prr_set_ema_params", "prr_reset_ema", "prr_calibrate", "prr_predict", "prr_ema_update", "prr_score",
     "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_decode_step_host",
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
+    "prr_timeline_enable", "prr_timeline_read",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
 ]
 
@@ -235,6 +236,18 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().prr_launch_count(self._h))
+
+    def timeline_enable(self, on=True):
+        self._chk(lib().prr_timeline_enable(self._h, int(on)))
+
+    def timeline_read(self, max_warps=8192, stream=None):
+        """uint64 numpy [n_warps, 16]: %globaltimer stamps (ns) of the last fused step's warps."""
+        import numpy as np
+        buf = np.zeros((max_warps, 16), dtype=np.uint64)
+        n = C.c_int32(0)
+        self._chk(lib().prr_timeline_read(self._h, buf.ctypes.data_as(C.c_void_p), max_warps, C.byref(n),
+                                          C.c_void_p(_stream(stream))))
+        return buf[:n.value]
 
     # -- graphs ------------------------------------------------------------------------------
     def graph_begin(self, stream=None):
