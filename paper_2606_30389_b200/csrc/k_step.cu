@@ -95,6 +95,8 @@ struct TeamMem {
   uint32_t* hist; int hbits;       // [1 << hbits], zero on entry to and exit from team_kth
   uint32_t* red;                   // [nw*16] per-warp slots, then 8 decision words
   uint32_t* candk; int32_t* candi; // [64] each
+  int32_t* plist;                  // [Bud] the predicted blocks by slot (select jobs)
+  double *Ls, *Vs; int st_cap;     // staged EMA state of the row [st_cap] each (8-byte aligned)
 };
 __device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
   uint32_t v;
@@ -122,6 +124,7 @@ __device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, cons
   const int per = (NB + tm.nt - 1) / tm.nt;
   const int hi = NB - tm.tid * per, lo = max(0, hi - per);
   uint32_t sum = 0;
+#pragma unroll 4
   for (int b = lo; b < hi; ++b) sum += hist[b];
   uint32_t incl = sum;
 #pragma unroll
@@ -132,17 +135,20 @@ __device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, cons
   if (tm.cta) {
     if (lane == 31) m.red[tm.wid] = incl;
     __syncthreads();
+#pragma unroll 1
     for (int w = 0; w < tm.wid; ++w) incl += m.red[w];
   }
   const uint32_t excl = incl - sum;
   if ((int)excl < need && need <= (int)incl) {  // the crossing is in this thread's buckets (exactly one thread)
     uint32_t acc = excl;
+#pragma unroll 1
     for (int b = hi - 1; b >= lo; --b) {
       const uint32_t c = hist[b];
       if ((int)(acc + c) >= need) { dec[0] = (uint32_t)b; dec[1] = c; dec[2] = acc; break; }
       acc += c;
     }
   }
+#pragma unroll 1
   for (int b = lo; b < hi; ++b) hist[b] = 0u;
   tm.sync();
   bstar = (int)dec[0]; cstar = (int)dec[1]; above = (int)dec[2];
@@ -157,7 +163,7 @@ __device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, cons
 // index order.  Integer-only, hence order-independent and bit-exact (Q4).  Requires
 // 1 <= k < n, [lo, lo+span] = the exact key range of the row, and a zeroed histogram.
 // ---------------------------------------------------------------------------------------------
-__device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const TeamMem& m, uint32_t lo, uint32_t span) {
+__device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const TeamMem& m, uint32_t lo, uint32_t span, unsigned long long* tl) {
   const int lane = threadIdx.x & 31;
   uint32_t* dec = m.red + tm.nw * 16;  // [0] bstar [1] cstar [2] acc [5] key [6] idx [7] cand count
   int need = k, cnt_in = n;
@@ -166,6 +172,7 @@ __device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const Team
     if (span == 0) {  // all survivors share one key: the `need` lowest indices win
       if (tm.wid == 0) {
         int base = 0, idx = n - 1;
+#pragma unroll 1
         for (int j0 = 0; j0 < n; j0 += 32) {
           const int i = j0 + lane;
           const uint32_t bal = __ballot_sync(FULL, i < n && ks.get(i) == lo);
@@ -193,11 +200,12 @@ __device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const Team
         }
       }
       tm.sync();
+#pragma unroll 1
       for (int e = tm.tid; e < cnt_in; e += tm.nt) {
         const uint32_t ke = m.candk[e];
         const int ie = m.candi[e];
         int rank = 0;
-#pragma unroll 8
+#pragma unroll 4
         for (int f = 0; f < cnt_in; ++f) {
           const uint32_t kf = m.candk[f];
           rank += (kf > ke) || (kf == ke && m.candi[f] < ie);
@@ -236,6 +244,7 @@ __device__ __forceinline__ void team_range(uint32_t kmin, uint32_t kmax, const T
   if (!tm.cta) { lo = kmin; span = kmax >= kmin ? kmax - kmin : 0u; return; }
   if ((threadIdx.x & 31) == 0) { m.red[tm.wid * 2] = kmin; m.red[tm.wid * 2 + 1] = kmax; }
   tm.sync();
+#pragma unroll 1
   for (int w = 0; w < tm.nw; ++w) { kmin = min(kmin, m.red[w * 2]); kmax = max(kmax, m.red[w * 2 + 1]); }
   tm.sync();
   lo = kmin; span = kmax >= kmin ? kmax - kmin : 0u;
@@ -260,6 +269,7 @@ __device__ uint32_t team_emit(const Keys& ks, int n, int k, const Thr& t, const 
   tm.sync();
   if (tm.wid == 0) {
     uint32_t carry = 0;
+#pragma unroll 1
     for (int w0 = 0; w0 < nwd; w0 += 32) {
       const int w = w0 + lane;
       const uint32_t aw = w < nwd ? m.amask[w] : 0u;
@@ -277,6 +287,7 @@ __device__ uint32_t team_emit(const Keys& ks, int n, int k, const Thr& t, const 
     if (lane == 0) dec[3] = carry;
   }
   tm.sync();
+#pragma unroll 2
   for (int w = tm.wid; w < nwd; w += tm.nw) {
     const uint32_t aw = m.amask[w];
     const uint32_t off = m.offs[w];
@@ -291,8 +302,10 @@ __device__ uint32_t team_emit(const Keys& ks, int n, int k, const Thr& t, const 
     if (mask_g && lane == 0) mask_g[w] = aw;
   }
   const uint32_t tot = dec[3];
+#pragma unroll 1
   for (int j = (int)(tot >> 16) + tm.tid; j < width; j += tm.nt) list[j] = -1;
   if (Mlist)
+#pragma unroll 1
     for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
   tm.sync();
   return tot;
@@ -309,7 +322,7 @@ struct StepArgs {
   int32_t* P0; int32_t* P1; int32_t* parity;
   int32_t* setA; int32_t* setM; int32_t* counts;
   // per-step scratch
-  uint32_t* maskA; float* pred;
+  uint32_t* maskA; float* pred; uint32_t* msrc; int32_t* mn;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
   uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
@@ -337,13 +350,12 @@ struct Tile {
 // bars[1] when V has, so QK^T can start while V is still in flight.  The whole block is fetched;
 // rows >= valid (unwritten cache slots of the open block) are masked / zeroed by tile_compute.
 template <int D, int BS>
-__device__ __forceinline__ void tile_load(unsigned char* Ks, unsigned long long* bars, const StepArgs& a, int b,
-                                          int h, int blk) {
+__device__ __forceinline__ void tile_load(unsigned char* Ks, unsigned long long* bars, const StepArgs& a, int page,
+                                          int h) {
   using T = Tile<D, BS>;
   fence_proxy_async();  // this buffer was last touched through the generic proxy
   __syncwarp();
   if ((threadIdx.x & 31) == 0) {
-    const int page = __ldg(a.table + (size_t)b * a.MB + blk);
     const int y = (page * a.Hkv + h) * BS;
     mbar_expect_tx(&bars[0], T::HALF);
 #pragma unroll
@@ -496,118 +508,263 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1: one chunk of CR summary rows of (b, h): sub-warps of D/8 lanes own a row (one 16-byte load
-// per lane), the group's queries are pre-summed per channel in fp64, products and sums are exact
-// (Q1).  Split in two so the loads are in flight while the warp issues its tile prefetch.
-constexpr int SC_UNR = 16;
-
+// a1: summary rows [r0, end) of (b, h) by one warp.  The rows are copied to the warp's own (still
+// idle) tile buffer with cp.async -- every 16-byte request of the chunk is in flight at once and
+// the code stays a short rolled loop (instruction cache) -- then sub-warps of D/8 lanes take a row
+// each: the group's queries are pre-summed per channel in fp64, products and sums are exact (Q1).
 template <int D>
-__device__ __forceinline__ void score_load(const StepArgs& a, int b, int h, int row0, int nb, uint4 (&v)[SC_UNR]) {
+__device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int r0, int end, unsigned char* stage,
+                                            unsigned long long* tl) {
   constexpr int LPR = D / 8, RW = 32 / LPR;
   const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
-  const uint4* rows = a.summ + ((size_t)b * a.Hkv + h) * a.MB * LPR;
-#pragma unroll
-  for (int u = 0; u < SC_UNR; ++u) {
-    const int r = row0 + sub + u * RW;
-    v[u] = r < nb ? __ldg(rows + (size_t)r * LPR + l) : make_uint4(0, 0, 0, 0);
-  }
-}
-
-// the group's queries summed per channel (exact in fp64): the 8 channels this lane owns
-template <int D>
-__device__ __forceinline__ void score_qsum(const StepArgs& a, int b, int h, double (&qs)[8]) {
-  constexpr int LPR = D / 8;
-  const int l = (threadIdx.x & 31) % LPR;
+  const uint4* rows = a.summ + (((size_t)b * a.Hkv + h) * a.MB + r0) * LPR + l;
+  float* out = a.scores + ((size_t)b * a.Hkv + h) * a.MB + r0;
+  const int nr = end - r0;
+  uint4* st = reinterpret_cast<uint4*>(stage) + l;
+#pragma unroll 4
+  for (int r = sub; r < nr; r += RW) cp_async16(st + r * LPR, rows + (size_t)r * LPR);
+  cp_async_commit();
+  // the group's queries summed per channel (exact in fp64): the 8 channels this lane owns
+  double qs[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j) qs[j] = 0.0;
   const uint16_t* qb = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D + l * 8;
-  for (int g = 0; g < a.G; ++g) {
-    const uint4 t = __ldg(reinterpret_cast<const uint4*>(qb + (size_t)g * D));
-    const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll 1
+  for (int g0 = 0; g0 < a.G; g0 += 4) {  // four query rows per batch of loads (zeros add nothing)
+    uint4 t[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      qs[2 * j] += (double)bf16_lo(w[j]);
-      qs[2 * j + 1] += (double)bf16_hi(w[j]);
+    for (int e = 0; e < 4; ++e)
+      t[e] = g0 + e < a.G ? __ldg(reinterpret_cast<const uint4*>(qb + (size_t)(g0 + e) * D)) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const uint32_t w[4] = {t[e].x, t[e].y, t[e].z, t[e].w};
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        qs[2 * j] += (double)bf16_lo(w[j]);
+        qs[2 * j + 1] += (double)bf16_hi(w[j]);
+      }
     }
   }
-}
-
-template <int D>
-__device__ __forceinline__ void score_finish(const StepArgs& a, int b, int h, int row0, int nb,
-                                             const uint4 (&v)[SC_UNR], const double (&qs)[8]) {
-  constexpr int LPR = D / 8, RW = 32 / LPR;
-  const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
-  float* out = a.scores + ((size_t)b * a.Hkv + h) * a.MB;
+  if (tl && lane == 0) tl[6] = gtime();
+  cp_async_wait<0>();
+  __syncwarp();
+  if (tl && lane == 0) tl[13] = gtime();
+#pragma unroll 1
+  for (int rr0 = 0; rr0 < nr; rr0 += 4 * RW) {  // warp-uniform trip count (full-mask shuffles below)
+    double acc[4];
 #pragma unroll
-  for (int u = 0; u < SC_UNR; ++u) {
-    const uint32_t w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
-    double acc = 0.0;
+    for (int e = 0; e < 4; ++e) {
+      const int r = rr0 + e * RW + sub;
+      const uint4 v = r < nr ? st[r * LPR] : make_uint4(0, 0, 0, 0);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+      double a0 = 0.0, a1 = 0.0;  // every partial sum is exact (Q1), so the order of accumulation is free
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      acc = fma((double)bf16_lo(w[j]), qs[2 * j], acc);
-      acc = fma((double)bf16_hi(w[j]), qs[2 * j + 1], acc);
+      for (int j = 0; j < 4; ++j) {
+        a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
+        a1 = fma((double)bf16_hi(w[j]), qs[2 * j + 1], a1);
+      }
+      acc[e] = a0 + a1;
     }
 #pragma unroll
-    for (int off = LPR / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(FULL, acc, off);
-    const int r = row0 + sub + u * RW;
-    if (l == 0 && r < nb) out[r] = f64_to_score(__dmul_rn(acc, a.score_c));
+    for (int off = LPR / 2; off >= 1; off >>= 1)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) acc[e] += __shfl_xor_sync(FULL, acc[e], off);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int r = rr0 + e * RW + sub;
+      if (l == 0 && r < nr) out[r] = f64_to_score(__dmul_rn(acc[e], a.score_c));
+    }
   }
+  __syncwarp();
 }
 
 // ---------------------------------------------------------------------------------------------
-// a5 preparation, independent of the scores (runs while they are being computed): bitmask of the
-// predicted set P in the team's shared memory.  Returns |P| in every thread.
-__device__ int select_prepare(const StepArgs& a, int row, const Team& tm, const TeamMem& m, const int32_t* Pcur) {
-  uint32_t* dec = m.red + tm.nw * 16;
-  for (int w = tm.tid; w < a.MBw; w += tm.nt) m.pmask[w] = 0u;
-  if (tm.tid == 0) dec[4] = 0u;
-  tm.sync();
-  if (a.spec) {
-    const int32_t* P = Pcur + (size_t)row * a.Bud;
-    int np = 0;
-    for (int j = tm.tid; j < a.Bud; j += tm.nt) {
-      const int blk = __ldg(P + j);
-      if (blk >= 0 && blk < a.MB) { atomicOr(&m.pmask[blk >> 5], 1u << (blk & 31)); ++np; }
-    }
-    np = __reduce_add_sync(FULL, np);
-    if ((threadIdx.x & 31) == 0 && np) atomicAdd(&dec[4], (uint32_t)np);
-  }
-  tm.sync();
-  return (int)dec[4];
-}
-
-// a2 + a5 for one (sequence, KV head) row, by one team, once the row's scores are complete.
-__device__ void job_select(const StepArgs& a, int row, const Team& tm, const TeamMem& m, int np, unsigned long long* tl) {
+// One row job by one team (a single code path for both kinds, so the kernel holds ONE copy of the
+// selection code: the instruction cache is 32 KB and this code runs once per step, on the
+// critical path).
+//   select(row): a2 + a5.  Before the scores exist: bitmask of the predicted set P in shared
+//                memory.  After: keys -> exact K-th -> A ascending + bitmask, M = A\P, publish.
+//   ema(row):    a8 + a3.  Before the scores exist: the row's (l, v) state is staged in shared
+//                memory (HBM latency hidden behind the score phase).  After: Eq. 3 in
+//                non-contracted fp64 (both lines use l^{t-1}; blocks scored for the first time
+//                get l = IS, v = 0), Eq. 2 rounded once to fp32, the same exact
+//                selection -> P = top-min(Bud, #stateful) of the NEXT step.
+__device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const TeamMem& m, const int32_t* Pcur,
+                        int32_t* Pnext, const uint32_t* score_done, unsigned long long* tl) {
+  const bool is_sel = jj < R;
+  const int row = is_sel ? jj : jj - R;
   const int b = row / a.Hkv;
   const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
+  uint32_t* dec = m.red + tm.nw * 16;
   uint32_t* ctl = a.ctl;
   const float* sc = a.scores + (size_t)row * a.MB;
-  const int k = min(a.K, nb);
-  const bool in_sm = nb <= m.key_cap;
-  uint32_t kmin = 0xffffffffu, kmax = 0u;
-#pragma unroll 8
-  for (int i = tm.tid; i < nb; i += tm.nt) {
-    const uint32_t key = score_key(__ldcg(sc + i));
-    if (in_sm) m.keys[i] = key;
-    kmin = min(kmin, key);
-    kmax = max(kmax, key);
+  double* L = a.ema_l + (size_t)row * a.MB;
+  double* V = a.ema_v + (size_t)row * a.MB;
+  int np = 0, n_old = 0, n = nb;
+  bool st_sm = false;
+  // ---- before the scores ----
+  if (is_sel) {
+#pragma unroll 1
+    for (int w = tm.tid; w < a.MBw; w += tm.nt) m.pmask[w] = 0u;
+    if (tm.tid == 0) dec[4] = 0u;
+    tm.sync();
+    if (a.spec) {
+      const int32_t* P = Pcur + (size_t)row * a.Bud;
+      for (int j = tm.tid; j < a.Bud; j += tm.nt) {
+        const int blk = __ldg(P + j);
+        const bool ok = blk >= 0 && blk < a.MB;
+        m.plist[j] = ok ? blk : -1;
+        if (ok) { atomicOr(&m.pmask[blk >> 5], 1u << (blk & 31)); ++np; }
+      }
+      np = __reduce_add_sync(FULL, np);
+      if ((threadIdx.x & 31) == 0 && np) atomicAdd(&dec[4], (uint32_t)np);
+    }
+    tm.sync();
+    np = (int)dec[4];
+  } else {
+    n_old = a.n_state[row];
+    n = max(nb, n_old);
+    st_sm = n <= m.st_cap;
+    if (st_sm) {
+#pragma unroll 1
+      for (int i0 = tm.tid; i0 < n_old; i0 += 6 * tm.nt) {
+        double x[6], y[6];
+#pragma unroll
+        for (int e = 0; e < 6; ++e) {
+          const int i = i0 + e * tm.nt;
+          x[e] = i < n_old ? L[i] : 0.0;
+          y[e] = i < n_old ? V[i] : 0.0;
+        }
+#pragma unroll
+        for (int e = 0; e < 6; ++e) {
+          const int i = i0 + e * tm.nt;
+          if (i < n_old) { m.Ls[i] = x[e]; m.Vs[i] = y[e]; }
+        }
+      }
+    }
   }
-  Keys ks{in_sm ? smem_u32(m.keys) : 0u, sc};
+  const bool in_sm = n <= m.key_cap;
+  // ---- wait for the row's scores ----
+  if (tm.tid == 0) {
+    uint32_t it = 0;
+    const uint32_t target = (uint32_t)((nb + a.CR - 1) / a.CR);
+    while (ld_acquire(&score_done[row]) < target) {
+      __nanosleep(20);
+      if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); break; }
+    }
+  }
+  tm.sync();
+  if (tl && tm.tid == 0) tl[8] = gtime();
+  // ---- keys ----
+  uint32_t kmin = 0xffffffffu, kmax = 0u;
+  float* pr = a.pred + (size_t)row * a.MB;
+  constexpr int KB = 12;  // scores per thread whose loads are in flight together
+  if (is_sel) {
+#pragma unroll 1
+    for (int i0 = tm.tid; i0 < nb; i0 += KB * tm.nt) {
+      float x[KB];
+#pragma unroll
+      for (int e = 0; e < KB; ++e) {
+        const int i = i0 + e * tm.nt;
+        x[e] = i < nb ? __ldcg(sc + i) : 0.f;
+      }
+#pragma unroll
+      for (int e = 0; e < KB; ++e) {
+        const int i = i0 + e * tm.nt;
+        if (i < nb) {
+          const uint32_t key = score_key(x[e]);
+          if (in_sm) m.keys[i] = key;
+          kmin = min(kmin, key);
+          kmax = max(kmax, key);
+        }
+      }
+    }
+  } else {
+    const double alpha = a.theta[b * 3 + 0], beta = a.theta[b * 3 + 1], gamma = a.theta[b * 3 + 2];
+    const double oma = __dsub_rn(1.0, alpha), omb = __dsub_rn(1.0, beta);
+    if (in_sm) {  // the row's scores, every load in flight at once; each thread re-reads only what it stored
+#pragma unroll 1
+      for (int i0 = tm.tid; i0 < nb; i0 += KB * tm.nt) {
+        float x[KB];
+#pragma unroll
+        for (int e = 0; e < KB; ++e) {
+          const int i = i0 + e * tm.nt;
+          x[e] = i < nb ? __ldcg(sc + i) : 0.f;
+        }
+#pragma unroll
+        for (int e = 0; e < KB; ++e) {
+          const int i = i0 + e * tm.nt;
+          if (i < nb) m.keys[i] = __float_as_uint(x[e]);
+        }
+      }
+    }
+#pragma unroll 2
+    for (int i = tm.tid; i < n; i += tm.nt) {
+      const bool has = i < n_old;
+      double ln = 0.0, vn = 0.0;
+      if (has) { ln = st_sm ? m.Ls[i] : L[i]; vn = st_sm ? m.Vs[i] : V[i]; }
+      if (i < nb) {
+        const double xd = (double)(in_sm ? __uint_as_float(m.keys[i]) : __ldcg(sc + i));
+        if (has) {
+          const double lo_ = ln;
+          vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, lo_)), __dmul_rn(omb, vn));
+          ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, lo_));
+        } else {
+          ln = xd;
+          vn = 0.0;
+        }
+        L[i] = ln;
+        V[i] = vn;
+      }
+      const float p = f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn)));
+      const uint32_t key = score_key(p);
+      if (in_sm) m.keys[i] = key; else pr[i] = p;
+      kmin = min(kmin, key);
+      kmax = max(kmax, key);
+    }
+    tm.sync();  // n_state is read by every thread above, written below
+    if (tm.tid == 0) a.n_state[row] = n;
+    if (a.Bud <= 0) return;
+  }
+  // ---- exact selection (one call site) ----
+  const int k = min(is_sel ? a.K : a.Bud, n);
+  Keys ks{in_sm ? smem_u32(m.keys) : 0u, is_sel ? sc : pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
-  if (k < nb) {                     // (uniform over the team)
+  if (k < n) {                      // (uniform over the team)
     uint32_t lo, span;
     team_range(kmin, kmax, tm, m, lo, span);
     if (tl && tm.tid == 0) tl[9] = gtime();
-    t = team_kth(ks, nb, k, tm, m, lo, span);
+    t = team_kth(ks, n, k, tm, m, lo, span, tl);
   } else {
     tm.sync();
   }
   if (tl && tm.tid == 0) tl[10] = gtime();
-  const uint32_t tot = team_emit(ks, nb, k, t, tm, m, a.setA + (size_t)row * a.K, a.K,
-                                 a.maskA + (size_t)row * a.MBw, a.setM + (size_t)row * a.K, a.K);
-  const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
+  const uint32_t tot =
+      team_emit(ks, n, k, t, tm, m, is_sel ? a.setA + (size_t)row * a.K : Pnext + (size_t)row * a.Bud,
+                is_sel ? a.K : a.Bud, is_sel ? a.maskA + (size_t)row * a.MBw : nullptr,
+                is_sel ? a.setM + (size_t)row * a.K : nullptr, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
+  if (!is_sel) return;
+  // ---- publish (select only) ----
+  const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
+  if (tm.wid == 0) {  // the row's merge list: hit slots (all of P when retained) ascending, then the repair slots
+    const int lane = threadIdx.x & 31;
+    uint32_t* ms = a.msrc + (size_t)row * (a.Bud + a.K);
+    int base = 0;
+    if (a.spec) {
+      for (int j0 = 0; j0 < a.Bud; j0 += 32) {
+        const int j = j0 + lane;
+        const int blk = j < a.Bud ? m.plist[j] : -1;
+        const bool use = blk >= 0 && (a.retain || ((blk >> 5) < ((nb + 31) >> 5) && ((m.amask[blk >> 5] >> (blk & 31)) & 1u)));
+        const uint32_t bal = __ballot_sync(FULL, use);
+        if (use) ms[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)j;
+        base += __popc(bal);
+      }
+    }
+    for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
+    if (lane == 0) a.mn[row] = base + nM;
+  }
   if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
     a.counts[row * 3 + 1] = np;
@@ -630,131 +787,53 @@ __device__ void job_select(const StepArgs& a, int row, const Team& tm, const Tea
   }
 }
 
-// a8 + a3 for one row, by one team: Eq. 3 in non-contracted fp64 (both lines use l^{t-1}; blocks
-// scored for the first time get l = IS, v = 0), Eq. 2 rounded once to fp32, then the
-// same exact selection for P = top-min(Bud, #stateful) of the next step.
-__device__ void job_ema(const StepArgs& a, int row, const Team& tm, const TeamMem& m, int32_t* Pnext, unsigned long long* tl) {
-  const int b = row / a.Hkv;
-  double* L = a.ema_l + (size_t)row * a.MB;
-  double* V = a.ema_v + (size_t)row * a.MB;
-  const double alpha = a.theta[b * 3 + 0], beta = a.theta[b * 3 + 1], gamma = a.theta[b * 3 + 2];
-  const double oma = __dsub_rn(1.0, alpha), omb = __dsub_rn(1.0, beta);
-  const int n_old = a.n_state[row];
-  const int n = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
-  const int n_new = max(n, n_old);
-  const float* sc = a.scores + (size_t)row * a.MB;
-  float* pr = a.pred + (size_t)row * a.MB;
-  const bool in_sm = n_new <= m.key_cap;
-  uint32_t kmin = 0xffffffffu, kmax = 0u;
-  constexpr int EB = 6;  // elements per thread whose loads are in flight together
-  for (int i0 = tm.tid; i0 < n_new; i0 += EB * tm.nt) {
-    float x[EB];
-    double lo_[EB], vo_[EB];
-#pragma unroll
-    for (int e = 0; e < EB; ++e) {
-      const int i = i0 + e * tm.nt;
-      x[e] = i < n ? __ldcg(sc + i) : 0.f;
-      const bool has = i < n_new && (i < n_old || i >= n);
-      lo_[e] = has ? L[i] : 0.0;
-      vo_[e] = has ? V[i] : 0.0;
-    }
-#pragma unroll
-    for (int e = 0; e < EB; ++e) {
-      const int i = i0 + e * tm.nt;
-      if (i >= n_new) break;
-      double ln = lo_[e], vn = vo_[e];
-      if (i < n) {
-        const double xd = (double)x[e];
-        if (i < n_old) {
-          vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, lo_[e])), __dmul_rn(omb, vo_[e]));
-          ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, lo_[e]));
-        } else {
-          ln = xd;
-          vn = 0.0;
-        }
-        L[i] = ln;
-        V[i] = vn;
-      }
-      const float p = f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn)));
-      const uint32_t key = score_key(p);
-      if (in_sm) m.keys[i] = key; else pr[i] = p;
-      kmin = min(kmin, key);
-      kmax = max(kmax, key);
-    }
-  }
-  tm.sync();  // n_state is read by every thread above, written below
-  if (tm.tid == 0) a.n_state[row] = n_new;
-  if (a.Bud <= 0) return;
-  const int k = min(a.Bud, n_new);
-  Keys ks{in_sm ? smem_u32(m.keys) : 0u, pr};
-  Thr t;
-  t.key = 0u; t.idx = 0x7fffffff;
-  if (k < n_new) {
-    uint32_t lo, span;
-    team_range(kmin, kmax, tm, m, lo, span);
-    if (tl && tm.tid == 0) tl[9] = gtime();
-    t = team_kth(ks, n_new, k, tm, m, lo, span);
-  }
-  if (tl && tm.tid == 0) tl[10] = gtime();
-  team_emit(ks, n_new, k, t, tm, m, Pnext + (size_t)row * a.Bud, a.Bud, nullptr, nullptr, 0);
-}
-
-// a7 for one (sequence, query head): Eq. 6-8 over the listed partial states, O unnormalised and
-// one division at the end.  Entry order is fixed (speculative slots ascending, then repair slots
-// ascending), so the result is deterministic; any order is the same real number (Q11).
+// a7 for one (sequence, query head, 32-channel slice of d): Eq. 6-8 over the listed partial states,
+// O unnormalised and one division at the end.  The warp is 4 groups of 8 lanes; a group owns every
+// 4th entry and its lanes one float4 of the 128-byte slice, so a pass has 4 x unroll entries in
+// flight; the groups are folded with two shuffles.  Entry order is fixed (speculative slots
+// ascending, then repair slots ascending) and so is the reduction tree: the result is
+// deterministic; any order is the same real number (Q11).
 template <int D>
-__device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, const int32_t* Pcur) {
-  constexpr int VEC = D / 32;
+__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, const int32_t* Pcur) {
   constexpr uint32_t REP = 0x80000000u;
   const int lane = threadIdx.x & 31;
-  const uint32_t lt = (1u << lane) - 1u;
   const int h = hq / a.G, row = b * a.Hkv + h;
   const size_t hb = (size_t)b * a.Hq + hq;
   const int E = a.Bud + a.K;
   float* ws = reinterpret_cast<float*>(buf);             // [E] m, then weights
   uint32_t* cs = reinterpret_cast<uint32_t*>(buf) + E;   // [E] slot codes (REP bit: repair buffers)
   float* ls = reinterpret_cast<float*>(buf) + 2 * E;     // [E] l
-  const int np = a.spec ? __ldcg(a.counts + row * 3 + 1) : 0;
-  const int nM = __ldcg(a.counts + row * 3 + 2);
-  const uint32_t* mA = a.maskA + (size_t)row * a.MBw;
-  const float* Os = a.O_spec + hb * a.Bud * D;
-  const float* Or = a.O_rep + hb * a.K * D;
-  int n = 0;
+  // the row's merge list was written by select(row): slot codes, speculative slots first
+  const int n = __ldcg(a.mn + row);
+  const uint32_t* ms = a.msrc + (size_t)row * E;
   float mx = -CUDART_INF_F;
-  // entries: hits (or all of P when retained) ...
-  for (int j0 = 0; j0 < np; j0 += 32) {
-    const int j = j0 + lane;
-    bool use = false;
-    float me = 0.f, le = 0.f;
-    if (j < np) {
-      const int blk = __ldg(Pcur + (size_t)row * a.Bud + j);
-      me = __ldcg(a.m_spec + hb * a.Bud + j);
-      le = __ldcg(a.l_spec + hb * a.Bud + j);
-      use = a.retain || ((__ldcg(mA + (blk >> 5)) >> (blk & 31)) & 1u);
+  // (rolled loops with a run-time trip count serialise their loads: batches with predication instead)
+#pragma unroll 1
+  for (int e0 = lane; e0 < n; e0 += 4 * 32) {
+    uint32_t code[4];
+    float me[4], le[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < n ? __ldcg(ms + e0 + 32 * u) : 0u;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t j = code[u] & ~REP;
+      const bool on = e0 + 32 * u < n;
+      const float* mp = (code[u] & REP) ? a.m_rep + hb * a.K + j : a.m_spec + hb * a.Bud + j;
+      const float* lp = (code[u] & REP) ? a.l_rep + hb * a.K + j : a.l_spec + hb * a.Bud + j;
+      me[u] = on ? __ldcg(mp) : -CUDART_INF_F;
+      le[u] = on ? __ldcg(lp) : 0.f;
     }
-    const uint32_t bal = __ballot_sync(FULL, use);
-    if (use) {
-      const int e = n + __popc(bal & lt);
-      ws[e] = me;
-      ls[e] = le;
-      cs[e] = (uint32_t)j;
-      mx = fmaxf(mx, me);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = e0 + 32 * u;
+      if (e < n) { ws[e] = me[u]; ls[e] = le[u]; cs[e] = code[u]; mx = fmaxf(mx, me[u]); }
     }
-    n += __popc(bal);
   }
-  // ... then the repaired blocks
-  for (int j = lane; j < nM; j += 32) {
-    const float me = __ldcg(a.m_rep + hb * a.K + j);
-    ws[n + j] = me;
-    ls[n + j] = __ldcg(a.l_rep + hb * a.K + j);
-    cs[n + j] = (uint32_t)j | REP;
-    mx = fmaxf(mx, me);
-  }
-  n += nM;
 #pragma unroll
   for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
   __syncwarp();
   float lsum = 0.f;
+#pragma unroll 2
   for (int e = lane; e < n; e += 32) {
     const float me = ws[e];
     const float w = me == -CUDART_INF_F ? 0.f : ex2((me - mx) * LOG2E_F);
@@ -764,37 +843,53 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, unsigned char* buf, 
 #pragma unroll
   for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
   __syncwarp();
-  float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll 16
-  for (int e = 0; e < n; ++e) {
-    const float w = ws[e];
-    const uint32_t code = cs[e];
-    const float* Op = ((code & REP) ? Or + (size_t)(code & ~REP) * D : Os + (size_t)code * D) + lane * VEC;
-    if (VEC == 4) {
-      const float4 x = __ldcg(reinterpret_cast<const float4*>(Op));
-      acc[0] = fmaf(w, x.x, acc[0]); acc[1] = fmaf(w, x.y, acc[1]);
-      acc[2] = fmaf(w, x.z, acc[2]); acc[3] = fmaf(w, x.w, acc[3]);
-    } else {
-      const float2 x = __ldcg(reinterpret_cast<const float2*>(Op));
-      acc[0] = fmaf(w, x.x, acc[0]); acc[1] = fmaf(w, x.y, acc[1]);
+  const int grp = lane >> 3, l8 = lane & 7;
+  const float* Os = a.O_spec + hb * a.Bud * D + dq * 32 + l8 * 4;
+  const float* Or = a.O_rep + hb * a.K * D + dq * 32 + l8 * 4;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+  for (int e0 = grp; e0 < n; e0 += 4 * 10) {  // 10 rows per lane (40 entries per warp) in flight
+    float4 x[10];
+    float w[10];
+#pragma unroll
+    for (int u = 0; u < 10; ++u) {
+      const int e = e0 + 4 * u;
+      const bool on = e < n;
+      const uint32_t code = on ? cs[e] : 0u;
+      w[u] = on ? ws[e] : 0.f;
+      const float* Op = (code & REP) ? Or + (size_t)(code & ~REP) * D : Os + (size_t)code * D;
+      x[u] = on ? __ldcg(reinterpret_cast<const float4*>(Op)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < 10; ++u) {
+      acc.x = fmaf(w[u], x[u].x, acc.x); acc.y = fmaf(w[u], x[u].y, acc.y);
+      acc.z = fmaf(w[u], x[u].z, acc.z); acc.w = fmaf(w[u], x[u].w, acc.w);
     }
   }
-  float* o = a.out + hb * D + lane * VEC;
 #pragma unroll
-  for (int c = 0; c < VEC; ++c) o[c] = lsum > 0.f ? acc[c] / lsum : 0.f;
+  for (int off = 8; off <= 16; off <<= 1) {
+    acc.x += __shfl_xor_sync(FULL, acc.x, off); acc.y += __shfl_xor_sync(FULL, acc.y, off);
+    acc.z += __shfl_xor_sync(FULL, acc.z, off); acc.w += __shfl_xor_sync(FULL, acc.w, off);
+  }
+  if (grp == 0) {
+    float4 o;
+    o.x = lsum > 0.f ? acc.x / lsum : 0.f; o.y = lsum > 0.f ? acc.y / lsum : 0.f;
+    o.z = lsum > 0.f ? acc.z / lsum : 0.f; o.w = lsum > 0.f ? acc.w / lsum : 0.f;
+    *reinterpret_cast<float4*>(a.out + hb * D + dq * 32 + l8 * 4) = o;
+  }
   __syncwarp();
 }
 
 // ---------------------------------------------------------------------------------------------
 template <int D, int BS>
 __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid_constant__ StepArgs a) {
-  constexpr int LPR = D / 8, BR = (32 / LPR) * SC_UNR;  // summary rows per batch of loads
-  const int CR = a.CR;                                   // rows per score chunk (a multiple of BR)
+  constexpr int LPR = D / 8;
+  constexpr int NQ = D / 32;                             // merge slices per query head
+  const int CR = a.CR;                                   // rows per score chunk
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long bars_all[2 * 12];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
   const int NC = gridDim.x, NW = W * NC;
-  const int gw = warp * NC + blockIdx.x;  // consecutive ids sit on different SMs
   const int per_warp = a.buf_bytes + a.scr_bytes;
   unsigned char* buf = smem_raw + (size_t)warp * per_warp;
   unsigned char* Ks = buf;
@@ -813,180 +908,196 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   const int32_t* Pcur = par ? a.P1 : a.P0;
   int32_t* Pnext = par ? a.P0 : a.P1;
   unsigned long long* tl = a.tl ? a.tl + ((size_t)blockIdx.x * W + warp) * 16 : nullptr;
-  if (tl && lane == 0) tl[0] = gtime();
+  if (tl && lane == 0) { tl[0] = gtime(); tl[12] = 0; tl[13] = 0; tl[14] = 0; tl[15] = 0; }
 
-  // Roles.  Team mode (J = 2R job CTAs at the end of the grid): the job CTAs' warps are ranked
-  // after every worker warp, so speculative units land on worker CTAs first.
+  // Roles.  Team mode (J job CTAs at the end of the grid, one row job each): the job CTAs take no
+  // score chunk (they stage P / the EMA state and then wait) and are ranked after every worker
+  // warp, so speculative units land on worker CTAs first.  Warp mode (J = 0): the highest-numbered
+  // warps take the row jobs after their score chunk.
   const int NWK = NC - a.J;
   const bool job_cta = (int)blockIdx.x >= NWK;
-  const bool job_warp = a.J == 0 && (NW - 1 - gw) < 2 * R;  // warp mode: highest-numbered warps
-  const int rank = !job_cta ? warp * NWK + (int)blockIdx.x : NWK * W + warp * a.J + ((int)blockIdx.x - NWK);
+  const int gw = warp * NWK + (int)blockIdx.x;  // worker-warp id: consecutive ids sit on different SMs
+  const int NWS = NWK * W;                      // warps that score
+  const bool job_warp = a.J == 0 && (NW - 1 - gw) < 2 * R;
 
-  // first speculative unit of this warp
+  // the unit this warp computes next: (ub, uh, ublk) with its tile in flight when `pend`
   const int U = a.spec ? R * a.Bud : 0;
-  int u = rank;
-  int ub = 0, uh = 0, ublk = -1, uvalid = 0;
-  auto unit_decode = [&](int unit) {
-    const int slot = unit / R, row = unit - slot * R;
-    ub = row / a.Hkv; uh = row - ub * a.Hkv;
-    ublk = __ldg(Pcur + (size_t)row * a.Bud + slot);
-    if (ublk >= a.MB) ublk = -1;
-    uvalid = ublk >= 0 ? min(BS, __ldg(a.seq_lens + ub) - ublk * BS) : 0;
+  int u = gw;
+  int ub = 0, uh = 0, ublk = -1, uvalid = 0, upage = 0, urow = 0, uslot = 0;
+  bool urep = false, pend = false;
+  int ulen = 0;
+  auto unit_decode_a = [&](int unit) {  // issue the independent loads (no use of their values yet)
+    uslot = unit / R; urow = unit - uslot * R;
+    ub = urow / a.Hkv; uh = urow - ub * a.Hkv;
+    ublk = __ldg(Pcur + (size_t)urow * a.Bud + uslot);
+    ulen = __ldg(a.seq_lens + ub);
   };
+  auto unit_decode_b = [&]() {
+    if (ublk >= a.MB) ublk = -1;
+    uvalid = 0;
+    if (ublk >= 0) {
+      uvalid = min(BS, ulen - ublk * BS);
+      upage = __ldg(a.table + (size_t)ub * a.MB + ublk);
+    }
+  };
+  auto unit_decode = [&](int unit) { unit_decode_a(unit); unit_decode_b(); };
   const bool prefetch = !job_cta && !job_warp && u < U;
-  if (prefetch) unit_decode(u);
-  if (tl && lane == 0) tl[6] = gtime() + (unsigned long long)(ublk & 0);
+  if (prefetch) unit_decode_a(u);
 
-  // ---- phase 1: scores; the first tile goes in flight right behind the first chunk's loads ------
-  {
+  // ---- phase 1: scores.  The warp's first speculative tile goes in flight only once its summary
+  // rows have LANDED: the 25 MB of tile traffic would otherwise queue in front of the 4 MB that
+  // heads the critical path.
+  if (!job_cta) {
     const int cpr = (a.MB + CR - 1) / CR;  // chunks per row (static upper bound)
-    bool issued = !prefetch;
-    for (int it = gw; it < R * cpr; it += NW) {
+    const int maxr = a.buf_bytes / (LPR * 16);  // rows the staging buffer holds
+#pragma unroll 1
+    for (int it = gw; it < R * cpr; it += NWS) {
       const int ch = it / R, row = it - ch * R;
       const int b = row / a.Hkv, h = row - b * a.Hkv;
       const int nb = min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs);
       if (ch * CR >= nb) continue;
-      double qs[8];
-      for (int r0 = ch * CR; r0 < min(nb, (ch + 1) * CR); r0 += BR) {
-        uint4 v[SC_UNR];
-        score_load<D>(a, b, h, r0, nb, v);
-        if (r0 == ch * CR) score_qsum<D>(a, b, h, qs);
-        if (!issued) {
-          if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
-          issued = true;
-          if (tl && lane == 0) tl[7] = gtime();
-        }
-        score_finish<D>(a, b, h, r0, nb, v, qs);
-      }
+      const int end = min(nb, (ch + 1) * CR);
+#pragma unroll 1
+      for (int r0 = ch * CR; r0 < end; r0 += maxr) score_chunk<D>(a, b, h, r0, min(end, r0 + maxr), Ks, tl);
+      if (tl && lane == 0) tl[14] = gtime();
       signal_add(&score_done[row], 1u);
+      if (tl && lane == 0) tl[15] = gtime();
     }
-    if (!issued && ublk >= 0) { tile_load<D, BS>(Ks, bars, a, ub, uh, ublk); if (tl && lane == 0) tl[7] = gtime(); }
+    if (prefetch) unit_decode_b();
+    if (prefetch && ublk >= 0) {
+      tile_load<D, BS>(Ks, bars, a, upage, uh);
+      pend = true;
+      if (tl && lane == 0) tl[7] = gtime();
+    }
   }
   if (tl && lane == 0) tl[1] = gtime();
 
   // ---- phase 2: row jobs -------------------------------------------------------------------------
-  if (job_cta) {
-    const int jj = (int)blockIdx.x - NWK;
-    const int row = jj < R ? jj : jj - R;
-    const int b = row / a.Hkv;
-    const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
-    Team tm{(int)threadIdx.x, (int)blockDim.x, warp, W, true};
+  if (job_cta || job_warp) {
+    Team tm;
     TeamMem m;
-    uint32_t* p = reinterpret_cast<uint32_t*>(smem_raw);
+    uint32_t* p;
+    size_t cap_bytes;
+    if (job_cta) {
+      tm = Team{(int)threadIdx.x, (int)blockDim.x, warp, W, true};
+      p = reinterpret_cast<uint32_t*>(smem_raw);
+      m.hbits = 11;
+    } else {
+      tm = Team{lane, 32, 0, 1, false};
+      p = reinterpret_cast<uint32_t*>(buf + a.buf_bytes);
+      m.hbits = 8;
+    }
     m.pmask = p; p += a.MBw;
     m.amask = p; p += a.MBw;
     m.offs = p; p += a.MBw;
-    m.red = p; p += W * 16 + 8;
-    m.hist = p; p += 2048; m.hbits = 11;
-    for (int i = threadIdx.x; i < 2048; i += blockDim.x) m.hist[i] = 0u;
+    m.red = p; p += tm.nw * 16 + 8;
+    m.hist = p; p += 1 << m.hbits;
+#pragma unroll 1
+    for (int i = tm.tid; i < (1 << m.hbits); i += tm.nt) m.hist[i] = 0u;
     m.candk = p; p += 64;
     m.candi = reinterpret_cast<int32_t*>(p); p += 64;
-    m.keys = p;
-    m.key_cap = (int)(((size_t)W * per_warp - (size_t)((unsigned char*)p - smem_raw)) / 4);
-    int np = 0;
-    if (jj < R) np = select_prepare(a, row, tm, m, Pcur);
-    if (threadIdx.x == 0) {
-      uint32_t it = 0;
-      const uint32_t target = (uint32_t)((nb + CR - 1) / CR);
-      while (ld_acquire(&score_done[row]) < target) {
-        __nanosleep(20);
-        if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); break; }
-      }
+    m.plist = reinterpret_cast<int32_t*>(p); p += a.Bud;
+    unsigned char* pool;
+    if (job_cta) {
+      pool = reinterpret_cast<unsigned char*>(p);
+      cap_bytes = (size_t)W * per_warp - (size_t)(pool - smem_raw);
+    } else {
+      pool = buf;
+      cap_bytes = (size_t)a.buf_bytes;
     }
-    __syncthreads();
-    if (tl && threadIdx.x == 0) tl[8] = gtime();
-    if (jj < R) job_select(a, row, tm, m, np, tl);
-    else job_ema(a, row, tm, m, Pnext, tl);
-    __syncthreads();  // the team's memory becomes per-warp tile buffers again
-  } else if (job_warp) {
-    Team tm{lane, 32, 0, 1, false};
-    TeamMem m;
-    uint32_t* p = reinterpret_cast<uint32_t*>(buf + a.buf_bytes);
-    m.pmask = p; p += a.MBw;
-    m.amask = p; p += a.MBw;
-    m.offs = p; p += a.MBw;
-    m.red = p; p += 16 + 8;
-    m.hist = p; p += 256; m.hbits = 8;
-    for (int i = lane; i < 256; i += 32) m.hist[i] = 0u;
-    m.candk = p; p += 64;
-    m.candi = reinterpret_cast<int32_t*>(p);
-    m.keys = reinterpret_cast<uint32_t*>(buf);
-    m.key_cap = a.buf_bytes / 4;
-    for (int jj = NW - 1 - gw; jj < 2 * R; jj += NW) {
-      const int row = jj < R ? jj : jj - R;
-      const int b = row / a.Hkv;
-      const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
-      int np = 0;
-      if (jj < R) np = select_prepare(a, row, tm, m, Pcur);
-      wait_ge(&score_done[row], (uint32_t)((nb + CR - 1) / CR), &ctl[CTL_ERR]);
-      if (jj < R) job_select(a, row, tm, m, np, tl);
-      else job_ema(a, row, tm, m, Pnext, tl);
-      __syncwarp();
+    pool += (16 - ((uintptr_t)pool & 15)) & 15;
+    // pool: keys [cap] u32, then l [cap], v [cap] fp64 (20 bytes per block)
+    const int cap = (int)((cap_bytes - 16) / 20) & ~3;
+    m.keys = reinterpret_cast<uint32_t*>(pool);
+    m.key_cap = cap;
+    m.Ls = reinterpret_cast<double*>(pool + (size_t)cap * 4);
+    m.Vs = m.Ls + cap;
+    m.st_cap = cap;
+    const int j0 = job_cta ? (int)blockIdx.x - NWK : NW - 1 - gw;
+    const int jstep = job_cta ? a.J : NW;
+#pragma unroll 1
+    for (int jj = j0; jj < 2 * R; jj += jstep) {
+      run_job(a, jj, R, tm, m, Pcur, Pnext, score_done, tl);
+      tm.sync();
     }
+    tm.sync();  // the team's memory becomes per-warp tile buffers again
   }
   if (tl && lane == 0) tl[2] = gtime();
 
-  // ---- phase 3: speculative units -------------------------------------------------------------
-  if (!prefetch && u < U) {  // job warps start their units only now
-    unit_decode(u);
-    if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
-  }
-  while (u < U) {
-    const int slot = u / R, row = u - slot * R;
-    const int cb = ub, chh = uh, cvalid = uvalid;
-    const bool real = ublk >= 0;
-    if (real) { tile_compute<D, BS>(Ks, bars, ph, a, cb, chh, cvalid, a.O_spec, a.m_spec, a.l_spec, a.Bud, slot); ph ^= 1u; }
-    u += NW;
-    if (u < U) {  // refill the buffer before publishing: the next tile's latency starts now
-      unit_decode(u);
-      if (ublk >= 0) tile_load<D, BS>(Ks, bars, a, ub, uh, ublk);
-    }
-    if (real) signal_add(&units_done[row], 1u);
-  }
-  if (tl && lane == 0) tl[3] = gtime();
-
-  // ---- phase 4: repair units, claimed by whoever is free ---------------------------------------
-  {
+  // ---- phases 3 + 4: per-block partial states.  First this warp's share of the speculative units
+  // (a4, static, the next tile is put in flight before the finished one is published), then
+  // repair units (a6) claimed by ticket -> (row, slot) by whichever warp is free, each waiting
+  // for select(row).  One loop, one copy of the tile code.
+  if (!job_cta) {
     const int NT = R * a.K;
+    bool finished = false;
+#pragma unroll 1
     for (;;) {
-      int t = 0;
-      if (lane == 0) t = (int)atomicAdd(&ctl[CTL_RTICKET], 1u);
-      t = __shfl_sync(FULL, t, 0);
-      if (t >= NT) break;
-      const int slot = t / R, row = t - slot * R;
-      wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
-      const int nM = (int)__ldcg(nM_g + row);
-      if (slot >= nM) {
-        // a void ticket; once every row is selected and no row has this many misses, all later ones are too
-        uint32_t stop = 0;
-        if (lane == 0) stop = ld_acquire(&ctl[CTL_SELDONE]) >= (uint32_t)R && (uint32_t)slot >= ld_acquire(&ctl[CTL_MAXM]);
-        if (__shfl_sync(FULL, stop, 0)) break;
-        continue;
+      if (!pend) {
+        if (u < U) {
+          unit_decode(u);
+          if (ublk < 0) { u += NWS; continue; }
+          urep = false;
+        } else {
+          if (tl && lane == 0 && !urep) tl[3] = gtime();
+          // claim a repair unit
+#pragma unroll 1
+          for (;;) {
+            int t = 0;
+            if (lane == 0) t = (int)atomicAdd(&ctl[CTL_RTICKET], 1u);
+            t = __shfl_sync(FULL, t, 0);
+            if (t >= NT) { finished = true; break; }
+            uslot = t / R; urow = t - uslot * R;
+            wait_ge(&sel_flag[urow], 1u, &ctl[CTL_ERR]);
+            const int nM = (int)__ldcg(nM_g + urow);
+            if (uslot < nM) break;
+            // a void ticket; once every row is selected and no row has this many misses, all later ones are too
+            uint32_t stop = 0;
+            if (lane == 0) stop = ld_acquire(&ctl[CTL_SELDONE]) >= (uint32_t)R && (uint32_t)uslot >= ld_acquire(&ctl[CTL_MAXM]);
+            if (__shfl_sync(FULL, stop, 0)) { finished = true; break; }
+          }
+          if (finished) break;
+          urep = true;
+          ub = urow / a.Hkv; uh = urow - ub * a.Hkv;
+          ublk = __ldcg(a.setM + (size_t)urow * a.K + uslot);
+          uvalid = min(BS, __ldg(a.seq_lens + ub) - ublk * BS);
+          upage = __ldg(a.table + (size_t)ub * a.MB + ublk);
+        }
+        tile_load<D, BS>(Ks, bars, a, upage, uh);
       }
-      const int b = row / a.Hkv, h = row - b * a.Hkv;
-      const int blk = __ldcg(a.setM + (size_t)row * a.K + slot);
-      const int valid = min(BS, __ldg(a.seq_lens + b) - blk * BS);
-      tile_load<D, BS>(Ks, bars, a, b, h, blk);
-      tile_compute<D, BS>(Ks, bars, ph, a, b, h, valid, a.O_rep, a.m_rep, a.l_rep, a.K, slot);
+      const int crow = urow;
+      const bool crep = urep;
+      tile_compute<D, BS>(Ks, bars, ph, a, ub, uh, uvalid, crep ? a.O_rep : a.O_spec, crep ? a.m_rep : a.m_spec,
+                          crep ? a.l_rep : a.l_spec, crep ? a.K : a.Bud, uslot);
       ph ^= 1u;
-      signal_add(&units_done[row], 1u);
+      pend = false;
+      if (!crep) {
+        u += NWS;
+        if (u < U) {  // refill the buffer before publishing: the next tile's latency starts now
+          unit_decode(u);
+          if (ublk >= 0) { tile_load<D, BS>(Ks, bars, a, upage, uh); pend = true; }
+        }
+      }
+      signal_add(&units_done[crow], 1u);
     }
   }
   if (tl && lane == 0) tl[4] = gtime();
 
   // ---- phase 5: merge, claimed by whoever is free ------------------------------------------------
-  {
-    const int NT = a.B * a.Hq;
+  if (job_cta || a.J == 0) {
+    const int NT = a.B * a.Hq * NQ;
+#pragma unroll 1
     for (;;) {
       int t = 0;
       if (lane == 0) t = (int)atomicAdd(&ctl[CTL_MTICKET], 1u);
       t = __shfl_sync(FULL, t, 0);
       if (t >= NT) break;
-      const int b = t / a.Hq, hq = t - b * a.Hq;
+      const int bh = t / NQ, dq = t - bh * NQ;
+      const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
       wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
       wait_ge(&units_done[row], __ldcg(units_total + row), &ctl[CTL_ERR]);
-      job_merge<D>(a, b, hq, buf, Pcur);
+      job_merge<D>(a, b, hq, dq, buf, Pcur);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
@@ -1000,6 +1111,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   }
   last = __shfl_sync(FULL, last, 0);
   if (last) {
+#pragma unroll 1
     for (int i = lane; i < 5 * a.Rmax; i += 32) ctl[CTL_HDR + i] = 0u;
     if (lane == 0) {
       ctl[CTL_EXIT] = 0u; ctl[CTL_RTICKET] = 0u; ctl[CTL_MTICKET] = 0u; ctl[CTL_SELDONE] = 0u; ctl[CTL_MAXM] = 0u;
@@ -1021,21 +1133,25 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   a.J = 2 * R <= c->n_sm / 4 ? 2 * R : 0;
   int W = 0, per_warp = 0;
   for (;;) {
-    a.scr_bytes = (3 * a.MBw + 24 + 128 + (a.J ? 0 : 256)) * 4;
+    a.scr_bytes = (3 * a.MBw + 24 + 128 + (a.J ? 0 : 256 + c->Bud)) * 4;
     a.scr_bytes += (1024 - (a.buf_bytes + a.scr_bytes) % 1024) % 1024;  // tile buffers stay 1024-byte aligned (swizzle atom)
     per_warp = a.buf_bytes + a.scr_bytes;
     W = std::min(T::WMAX, (c->smem_optin - 1024) / per_warp);
     if (W < 1) return cudaErrorInvalidConfiguration;
-    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 128 + 64;
+    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 128 + 64 + c->Bud;
     if (a.J && team_words * 4 > (size_t)W * per_warp) { a.J = 0; continue; }
     break;
   }
+  if (a.J) {  // worker CTAs: enough warps for one wave of speculative units; the rest also merge
+    const int U = a.spec ? R * a.Bud : 0;
+    a.J = std::max(a.J, std::min(c->n_sm - (U + W - 1) / W, c->n_sm / 4));
+  }
   const size_t smem = (size_t)W * per_warp;
-  {  // score chunk: about one per warp, a whole number of load batches
-    const int BR = (32 / (D / 8)) * SC_UNR;
-    const long long rows = (long long)R * a.MB, NWh = (long long)W * c->n_sm;
-    a.CR = (int)(((rows + NWh - 1) / NWh + BR - 1) / BR) * BR;
-    if (a.CR < BR) a.CR = BR;
+  {  // score chunk: one per scoring warp (job CTAs do not score), so every warp's summary loads are one batch
+    const int RW = 32 / (D / 8);
+    const long long rows = (long long)R * a.MB, NWS = (long long)W * (c->n_sm - a.J);
+    a.CR = (int)((rows + NWS - 1) / NWS);
+    if (a.CR < 2 * RW) a.CR = 2 * RW;
   }
   static bool attr_set = false;
   if (!attr_set) {
@@ -1111,7 +1227,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.theta = c->theta + (size_t)kv->layer * c->maxB * 3;
   a.P0 = c->Pbuf[0] + r * c->Bud; a.P1 = c->Pbuf[1] + r * c->Bud; a.parity = c->parity + kv->layer;
   a.setA = c->setA + r * c->K; a.setM = c->setM + r * c->K; a.counts = c->counts + r * 3;
-  a.maskA = c->maskA; a.pred = c->pred;
+  a.maskA = c->maskA; a.pred = c->pred; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
   a.ctl = c->ctl; a.stats = c->stats; a.tl = c->tl_on ? c->tl : nullptr;
