@@ -31,6 +31,7 @@
 #include <cuda.h>
 #include <math_constants.h>
 
+#include <cstdlib>
 #include <cstring>
 
 #include "prr_dev.cuh"
@@ -41,9 +42,11 @@ namespace prr {
 constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr uint32_t SPIN_LIMIT = 1u << 22;  // ~0.1-0.5 s of polling, then give up loudly
 
-// ctl header words, then 5 arrays of Rmax words:
-//   [0] score_done, [1] sel_flag, [2] units_done, [3] units_total, [4] nM
-enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_RTICKET = 2, CTL_MTICKET = 3, CTL_SELDONE = 4, CTL_MAXM = 5, CTL_HDR = 8 };
+// Dependencies between warps are epoch-valued FLAGS, not counters: a producer publishes with one
+// st.release of the launch's epoch (no atomics, nothing to reset), a consumer polls exactly the
+// flags of the items it needs.  ctl = header, then sel[Rmax], spec-unit flags [Rmax*Bud], repair-
+// unit flags [Rmax*K], score-chunk flags [Rmax*MB].
+enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_EPOCH = 2, CTL_HDR = 8 };
 
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
   uint32_t v;
@@ -56,23 +59,49 @@ __device__ __forceinline__ unsigned long long gtime() {
   return t;
 }
 
-// Warp-collective wait until *p >= target.  Lane 0 polls; __syncwarp orders the other lanes.
-__device__ __forceinline__ void wait_ge(const uint32_t* p, uint32_t target, uint32_t* err) {
-  if ((threadIdx.x & 31) == 0) {
-    uint32_t it = 0;
-    while (ld_acquire(p) < target) {
-      __nanosleep(20);
-      if (++it > SPIN_LIMIT) { atomicExch(err, 1u); break; }
-    }
+__device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+// One thread spins until *p == v (acquire).  Bounded: gives up loudly.
+__device__ __forceinline__ void spin_eq(const uint32_t* p, uint32_t v, uint32_t* err) {
+  uint32_t it = 0;
+  while (ld_acquire(p) != v) {
+    __nanosleep(20);
+    if (++it > SPIN_LIMIT) { atomicExch(err, 1u); break; }
   }
+}
+// Warp-collective wait until *p == v.  Lane 0 polls; __syncwarp orders the other lanes after it.
+__device__ __forceinline__ void wait_eq(const uint32_t* p, uint32_t v, uint32_t* err) {
+  if ((threadIdx.x & 31) == 0) spin_eq(p, v, err);
   __syncwarp();
 }
-
-// Release: every lane has fenced its own stores, then one lane bumps / sets the counter.
-__device__ __forceinline__ void signal_add(uint32_t* p, uint32_t v) {
-  __threadfence();
+// Warp-collective wait until f[0 .. n) all equal v.  The warp stays converged: every lane polls up
+// to four flags per round trip and the loop exits on a vote (lanes spinning in private loops would
+// be serialised).
+__device__ __forceinline__ void wait_flags(const uint32_t* f, int n, uint32_t v, uint32_t* err) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll 1
+  for (int base = 0; base < n; base += 128) {
+    uint32_t it = 0;
+#pragma unroll 1
+    for (;;) {
+      bool ok = true;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int c = base + lane + 32 * k;
+        if (c < n) ok = ok && (ld_acquire(f + c) == v);
+      }
+      if (__all_sync(FULL, ok)) break;
+      __nanosleep(20);
+      if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(err, 1u); break; }
+    }
+  }
+}
+// Warp-collective publish: the lanes' earlier stores are ordered before lane 0's release by the
+// warp barrier (the release is cumulative over it).
+__device__ __forceinline__ void signal_set(uint32_t* p, uint32_t v) {
   __syncwarp();
-  if ((threadIdx.x & 31) == 0) atomicAdd(p, v);
+  if ((threadIdx.x & 31) == 0) st_release(p, v);
 }
 
 struct Thr { uint32_t key; int idx; };  // selected(i) <=> key_i > key || (key_i == key && i <= idx)
@@ -324,9 +353,10 @@ struct StepArgs {
   // per-step scratch
   uint32_t* maskA; float* pred; uint32_t* msrc; int32_t* mn;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
-  uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
+  uint32_t* ctl; uint32_t* sel; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
+  unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
-  float scale; double score_c;
+  float scale; float pace_ns; double score_c;
 };
 
 template <int D, int BS>
@@ -513,17 +543,21 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
 // the code stays a short rolled loop (instruction cache) -- then sub-warps of D/8 lanes take a row
 // each: the group's queries are pre-summed per channel in fp64, products and sums are exact (Q1).
 template <int D>
-__device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int r0, int end, unsigned char* stage,
-                                            unsigned long long* tl) {
+__device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int r0, int end_ld, unsigned char* stage,
+                                           unsigned long long* tl) {
   constexpr int LPR = D / 8, RW = 32 / LPR;
   const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
   const uint4* rows = a.summ + (((size_t)b * a.Hkv + h) * a.MB + r0) * LPR + l;
   float* out = a.scores + ((size_t)b * a.Hkv + h) * a.MB + r0;
-  const int nr = end - r0;
+  // The copies do not wait for the sequence length: rows up to the chunk's end inside the summary
+  // buffer are fetched (rows past the last block hold stale data and are never scored).
+  const int nld = end_ld - r0;
   uint4* st = reinterpret_cast<uint4*>(stage) + l;
 #pragma unroll 4
-  for (int r = sub; r < nr; r += RW) cp_async16(st + r * LPR, rows + (size_t)r * LPR);
+  for (int r = sub; r < nld; r += RW) cp_async16(st + r * LPR, rows + (size_t)r * LPR);
   cp_async_commit();
+  if (tl && lane == 0) tl[12] = gtime();
+  const int len = __ldg(a.seq_lens + b);
   // the group's queries summed per channel (exact in fp64): the 8 channels this lane owns
   double qs[8];
 #pragma unroll
@@ -545,6 +579,8 @@ __device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int
       }
     }
   }
+  const int nb = max(0, min(a.MB, (len + a.bs - 1) / a.bs));
+  const int nr = min(end_ld, nb) - r0;
   if (tl && lane == 0) tl[6] = gtime();
   cp_async_wait<0>();
   __syncwarp();
@@ -576,6 +612,7 @@ __device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int
     }
   }
   __syncwarp();
+  return nb;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -590,7 +627,7 @@ __device__ __forceinline__ void score_chunk(const StepArgs& a, int b, int h, int
 //                get l = IS, v = 0), Eq. 2 rounded once to fp32, the same exact
 //                selection -> P = top-min(Bud, #stateful) of the NEXT step.
 __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const TeamMem& m, const int32_t* Pcur,
-                        int32_t* Pnext, const uint32_t* score_done, unsigned long long* tl) {
+                        int32_t* Pnext, uint32_t ep, unsigned long long* tl) {
   const bool is_sel = jj < R;
   const int row = is_sel ? jj : jj - R;
   const int b = row / a.Hkv;
@@ -645,13 +682,10 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   }
   const bool in_sm = n <= m.key_cap;
   // ---- wait for the row's scores ----
-  if (tm.tid == 0) {
-    uint32_t it = 0;
-    const uint32_t target = (uint32_t)((nb + a.CR - 1) / a.CR);
-    while (ld_acquire(&score_done[row]) < target) {
-      __nanosleep(20);
-      if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); break; }
-    }
+  if (tm.wid == 0) {  // one flag per score chunk of the row, a few per lane
+    const int cprs = (a.MB + a.CR - 1) / a.CR, target = (nb + a.CR - 1) / a.CR;
+    const uint32_t* f = a.sfl + (size_t)row * cprs;
+    wait_flags(f, target, ep, &ctl[CTL_ERR]);
   }
   tm.sync();
   if (tl && tm.tid == 0) tl[8] = gtime();
@@ -775,16 +809,9 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
       atomicAdd(&a.stats[2], (unsigned long long)nM);
       atomicAdd(&a.stats[3], (unsigned long long)np);
     }
-    ctl[CTL_HDR + 3 * a.Rmax + row] = (uint32_t)(np + nM);
-    ctl[CTL_HDR + 4 * a.Rmax + row] = (uint32_t)nM;
-    atomicMax(&ctl[CTL_MAXM], (uint32_t)nM);
   }
-  __threadfence();
-  tm.sync();
-  if (tm.tid == 0) {
-    atomicAdd(&ctl[CTL_HDR + 1 * a.Rmax + row], 1u);
-    atomicAdd(&ctl[CTL_SELDONE], 1u);  // CTL_MAXM was raised before the fence above
-  }
+  tm.sync();  // every thread's stores (A, M, merge list, counts) are ordered before the release
+  if (tm.tid == 0) st_release(&a.sel[row], ep);
 }
 
 // a7 for one (sequence, query head, 32-channel slice of d): Eq. 6-8 over the listed partial states,
@@ -794,7 +821,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
 template <int D>
-__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, const int32_t* Pcur) {
+__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep) {
   constexpr uint32_t REP = 0x80000000u;
   const int lane = threadIdx.x & 31;
   const int h = hq / a.G, row = b * a.Hkv + h;
@@ -809,11 +836,29 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   float mx = -CUDART_INF_F;
   // (rolled loops with a run-time trip count serialise their loads: batches with predication instead)
 #pragma unroll 1
-  for (int e0 = lane; e0 < n; e0 += 4 * 32) {
+  for (int eb = 0; eb < n; eb += 4 * 32) {  // warp-uniform trips (votes inside)
+    const int e0 = eb + lane;
     uint32_t code[4];
     float me[4], le[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < n ? __ldcg(ms + e0 + 32 * u) : 0u;
+    {  // wait for exactly these entries' units (over-predicted blocks that are not merged are not waited
+       // for); the warp stays converged and exits on a vote
+      uint32_t it = 0;
+#pragma unroll 1
+      for (;;) {
+        bool ok = true;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const uint32_t j = code[u] & ~REP;
+          const uint32_t* fp = (code[u] & REP) ? a.ufr + (size_t)row * a.K + j : a.ufs + (size_t)row * a.Bud + j;
+          if (e0 + 32 * u < n) ok = ok && (ld_acquire(fp) == ep);
+        }
+        if (__all_sync(FULL, ok)) break;
+        __nanosleep(20);
+        if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
+      }
+    }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const uint32_t j = code[u] & ~REP;
@@ -898,11 +943,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   if (lane == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init(); }
   __syncwarp();
   uint32_t* ctl = a.ctl;
-  uint32_t* score_done = ctl + CTL_HDR;
-  uint32_t* sel_flag = ctl + CTL_HDR + a.Rmax;
-  uint32_t* units_done = ctl + CTL_HDR + 2 * a.Rmax;
-  const uint32_t* units_total = ctl + CTL_HDR + 3 * a.Rmax;
-  const uint32_t* nM_g = ctl + CTL_HDR + 4 * a.Rmax;
+  const uint32_t ep = __ldcg(ctl + CTL_EPOCH) + 1u;  // this launch's epoch: the value every flag of the step takes
   const int R = a.B * a.Hkv;
   const int par = *a.parity & 1;
   const int32_t* Pcur = par ? a.P1 : a.P0;
@@ -954,17 +995,31 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     for (int it = gw; it < R * cpr; it += NWS) {
       const int ch = it / R, row = it - ch * R;
       const int b = row / a.Hkv, h = row - b * a.Hkv;
-      const int nb = min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs);
-      if (ch * CR >= nb) continue;
-      const int end = min(nb, (ch + 1) * CR);
+      const int end = min(a.MB, (ch + 1) * CR);
+      int nb = 0;
 #pragma unroll 1
-      for (int r0 = ch * CR; r0 < end; r0 += maxr) score_chunk<D>(a, b, h, r0, min(end, r0 + maxr), Ks, tl);
+      for (int r0 = ch * CR; r0 < end; r0 += maxr) {
+        nb = score_chunk<D>(a, b, h, r0, min(end, r0 + maxr), Ks, tl);
+        if (r0 + maxr >= nb) break;
+      }
       if (tl && lane == 0) tl[14] = gtime();
-      signal_add(&score_done[row], 1u);
+      if (ch * CR >= nb) continue;  // a chunk past the sequence's last block: nobody waits for it
+      signal_set(&a.sfl[(size_t)row * cpr + ch], ep);
       if (tl && lane == 0) tl[15] = gtime();
     }
     if (prefetch) unit_decode_b();
+    // No bulk tile traffic from this SM before all of its warps have published their scores: a
+    // release waits for the SM's outstanding memory traffic.
+    __syncthreads();
     if (prefetch && ublk >= 0) {
+      // Traffic shaping: the first wave of speculative tiles is issued at the rate HBM can serve it
+      // (warp gw waits gw x tile_time) instead of all at once, so the queues in front of L2 stay
+      // short and the small critical-path accesses (flags, scores, lists) are not stuck behind
+      // megabytes of bulk requests.  Total speculative time is unchanged: it is bandwidth-bound.
+      if (a.pace_ns > 0.f) {
+        const unsigned long long t_go = gtime() + (unsigned long long)((float)gw * a.pace_ns);
+        while (gtime() < t_go) __nanosleep(32);
+      }
       tile_load<D, BS>(Ks, bars, a, upage, uh);
       pend = true;
       if (tl && lane == 0) tl[7] = gtime();
@@ -1017,7 +1072,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     const int jstep = job_cta ? a.J : NW;
 #pragma unroll 1
     for (int jj = j0; jj < 2 * R; jj += jstep) {
-      run_job(a, jj, R, tm, m, Pcur, Pnext, score_done, tl);
+      run_job(a, jj, R, tm, m, Pcur, Pnext, ep, tl);
       tm.sync();
     }
     tm.sync();  // the team's memory becomes per-warp tile buffers again
@@ -1031,6 +1086,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   if (!job_cta) {
     const int NT = R * a.K;
     bool finished = false;
+    int tr = gw;  // next repair ticket of this warp
 #pragma unroll 1
     for (;;) {
       if (!pend) {
@@ -1040,32 +1096,26 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
           urep = false;
         } else {
           if (tl && lane == 0 && !urep) tl[3] = gtime();
-          // claim a repair unit
+          // the next repair unit of this warp: tickets (slot-major) are dealt out statically; a
+          // ticket is void when its row has fewer misses than its slot
 #pragma unroll 1
           for (;;) {
-            int t = 0;
-            if (lane == 0) t = (int)atomicAdd(&ctl[CTL_RTICKET], 1u);
-            t = __shfl_sync(FULL, t, 0);
-            if (t >= NT) { finished = true; break; }
-            uslot = t / R; urow = t - uslot * R;
-            wait_ge(&sel_flag[urow], 1u, &ctl[CTL_ERR]);
-            const int nM = (int)__ldcg(nM_g + urow);
-            if (uslot < nM) break;
-            // a void ticket; once every row is selected and no row has this many misses, all later ones are too
-            uint32_t stop = 0;
-            if (lane == 0) stop = ld_acquire(&ctl[CTL_SELDONE]) >= (uint32_t)R && (uint32_t)uslot >= ld_acquire(&ctl[CTL_MAXM]);
-            if (__shfl_sync(FULL, stop, 0)) { finished = true; break; }
+            if (tr >= NT) { finished = true; break; }
+            uslot = tr / R; urow = tr - uslot * R;
+            tr += NWS;
+            wait_eq(&a.sel[urow], ep, &ctl[CTL_ERR]);
+            ublk = __ldcg(a.setM + (size_t)urow * a.K + uslot);
+            if (ublk >= 0) break;
           }
           if (finished) break;
           urep = true;
           ub = urow / a.Hkv; uh = urow - ub * a.Hkv;
-          ublk = __ldcg(a.setM + (size_t)urow * a.K + uslot);
           uvalid = min(BS, __ldg(a.seq_lens + ub) - ublk * BS);
           upage = __ldg(a.table + (size_t)ub * a.MB + ublk);
         }
         tile_load<D, BS>(Ks, bars, a, upage, uh);
       }
-      const int crow = urow;
+      const int crow = urow, cslot = uslot;
       const bool crep = urep;
       tile_compute<D, BS>(Ks, bars, ph, a, ub, uh, uvalid, crep ? a.O_rep : a.O_spec, crep ? a.m_rep : a.m_spec,
                           crep ? a.l_rep : a.l_spec, crep ? a.K : a.Bud, uslot);
@@ -1078,7 +1128,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
           if (ublk >= 0) { tile_load<D, BS>(Ks, bars, a, upage, uh); pend = true; }
         }
       }
-      signal_add(&units_done[crow], 1u);
+      signal_set(crep ? &a.ufr[(size_t)crow * a.K + cslot] : &a.ufs[(size_t)crow * a.Bud + cslot], ep);
     }
   }
   if (tl && lane == 0) tl[4] = gtime();
@@ -1086,18 +1136,15 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   // ---- phase 5: merge, claimed by whoever is free ------------------------------------------------
   if (job_cta || a.J == 0) {
     const int NT = a.B * a.Hq * NQ;
+    const int mw = a.J ? ((int)blockIdx.x - NWK) * W + warp : gw;  // merge items are dealt out statically
+    const int nmw = a.J ? a.J * W : NW;
 #pragma unroll 1
-    for (;;) {
-      int t = 0;
-      if (lane == 0) t = (int)atomicAdd(&ctl[CTL_MTICKET], 1u);
-      t = __shfl_sync(FULL, t, 0);
-      if (t >= NT) break;
+    for (int t = mw; t < NT; t += nmw) {
       const int bh = t / NQ, dq = t - bh * NQ;
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
-      wait_ge(&sel_flag[row], 1u, &ctl[CTL_ERR]);
-      wait_ge(&units_done[row], __ldcg(units_total + row), &ctl[CTL_ERR]);
-      job_merge<D>(a, b, hq, dq, buf, Pcur);
+      wait_eq(&a.sel[row], ep, &ctl[CTL_ERR]);
+      job_merge<D>(a, b, hq, dq, buf, ep);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
@@ -1111,10 +1158,9 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   }
   last = __shfl_sync(FULL, last, 0);
   if (last) {
-#pragma unroll 1
-    for (int i = lane; i < 5 * a.Rmax; i += 32) ctl[CTL_HDR + i] = 0u;
     if (lane == 0) {
-      ctl[CTL_EXIT] = 0u; ctl[CTL_RTICKET] = 0u; ctl[CTL_MTICKET] = 0u; ctl[CTL_SELDONE] = 0u; ctl[CTL_MAXM] = 0u;
+      ctl[CTL_EXIT] = 0u;
+      ctl[CTL_EPOCH] = ep;
       *a.parity = par ^ 1;
     }
   }
@@ -1230,12 +1276,20 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.maskA = c->maskA; a.pred = c->pred; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
-  a.ctl = c->ctl; a.stats = c->stats; a.tl = c->tl_on ? c->tl : nullptr;
+  a.ctl = c->ctl; a.stats = c->stats;
+  {
+    const size_t rm = (size_t)c->maxB * c->Hkv;
+    a.sel = c->ctl + CTL_HDR; a.ufs = a.sel + rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
+  } a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.Rmax = c->maxB * c->Hkv;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.scale = c->sm_scale; a.score_c = c->score_c;
+  {  // ns per speculative tile at ~6.4 TB/s (PRR_PACE scales it, 0 disables)
+    static const float pace = [] { const char* e = getenv("PRR_PACE"); return e ? (float)atof(e) : 1.0f; }();
+    a.pace_ns = pace * (float)(2.0 * c->bs * c->D * 2.0) / 6400.0f;
+  }
   cudaError_t e = cudaErrorInvalidValue;
 #define PRR_CASE(DD, BB) if (c->D == DD && c->bs == BB) e = launch_step_t<DD, BB>(c, a, s);
   PRR_CASE(128, 64) PRR_CASE(128, 32) PRR_CASE(128, 16) PRR_CASE(128, 128)
