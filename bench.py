@@ -185,9 +185,8 @@ class Stack:
         for _ in range(n):
             l, t = self.pos % self.R, self.pos // self.R
             inp = self.inps[l]
-            self.ctx.append(self.kvs[l], inp.k_new[t], inp.v_new[t], self.summ[l], stream=stream)
-            fn = self.ctx.attend if sequential else self.ctx.decode_step
-            fn(self.kvs[l], inp.q_dec[t], self.summ[l], self.out[l], stream=stream)
+            self.ctx.step_append(self.kvs[l], inp.q_dec[t], inp.k_new[t], inp.v_new[t], self.summ[l], self.out[l],
+                                 sequential=sequential, stream=stream)
             self.pos += 1
 
     def capture(self, n, stream, sequential=False, chunk=None):

@@ -172,6 +172,15 @@ int32_t prr_attend(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const vo
  * and the next step's prediction run off the critical path.  Call prr_append first. */
 int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* summaries,
                         float* out, void* stream);
+/* prr_append followed by prr_decode_step (sequential = 0) or prr_attend (sequential != 0) as ONE
+ * call: a0-a8 of SURVEY.md section 8(a).  With PRR_FUSED orchestration the append rides in the
+ * same launch as the rest of the step (the new token's k/v and the open block's summary are patched
+ * into the tiles that need them on chip; the cache, the summary row and seq_lens are written for
+ * the following steps); results are identical to the two separate calls.  Arguments as in
+ * prr_append / prr_decode_step; kv->seq_lens holds the lengths BEFORE the append on entry and is
+ * incremented by the call. */
+int32_t prr_step_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* k_new,
+                        const void* v_new, void* summaries, float* out, int32_t sequential, void* stream);
 /* prr_append + prr_decode_step with HOST q/k_new/v_new/out (pinned or pageable): copies the
  * inputs to library staging buffers, runs the step, copies out back and synchronises. */
 int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_host,

@@ -123,7 +123,8 @@ struct TeamMem {
   uint32_t *pmask, *amask, *offs;  // [MBw] each
   uint32_t* hist; int hbits;       // [1 << hbits], zero on entry to and exit from team_kth
   uint32_t* red;                   // [nw*16] per-warp slots, then 8 decision words
-  uint32_t* candk; int32_t* candi; // [64] each
+  unsigned long long* cand;        // [CAND] candidates (key << 32 | ~index), 8-byte aligned
+  uint32_t* rk;                    // [CAND] partial ranks, zero between uses
   int32_t* plist;                  // [Bud] the predicted blocks by slot (select jobs)
   double *Ls, *Vs; int st_cap;     // staged EMA state of the row [st_cap] each (8-byte aligned)
 };
@@ -192,10 +193,54 @@ __device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, cons
 // index order.  Integer-only, hence order-independent and bit-exact (Q4).  Requires
 // 1 <= k < n, [lo, lo+span] = the exact key range of the row, and a zeroed histogram.
 // ---------------------------------------------------------------------------------------------
-__device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const TeamMem& m, uint32_t lo, uint32_t span, unsigned long long* tl) {
+constexpr int CAND = 128;  // survivors that are ranked directly
+
+// The need-th (1-based) of the cnt candidates under (key desc, index asc).  A candidate is one
+// 64-bit word (key << 32 | ~index): larger word = better.  All threads work: the comparisons of a
+// candidate are split over nt / cnt threads whose partial ranks meet in shared memory (rk[], zero on
+// entry and on exit).
+__device__ __forceinline__ Thr team_rank(int cnt, int need, const Team& tm, const TeamMem& m) {
+  uint32_t* dec = m.red + tm.nw * 16;
+  if (tm.nt >= cnt) {  // (uniform) a candidate's comparisons are split over nt / cnt threads
+    const int parts = tm.nt / cnt;
+    const int e = tm.tid % cnt, p = tm.tid / cnt;
+    unsigned long long ce = 0ull;
+    if (p < parts) {
+      ce = m.cand[e];
+      const int per = (cnt + parts - 1) / parts;
+      const int f0 = p * per, f1 = min(cnt, f0 + per);
+      uint32_t rank = 0;
+#pragma unroll 4
+      for (int f = f0; f < f1; ++f) rank += m.cand[f] > ce;
+      if (parts > 1) atomicAdd(&m.rk[e], rank); else m.rk[e] = rank;
+    }
+    tm.sync();
+    if (p == 0) {
+      if ((int)m.rk[e] == need - 1) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }  // exactly one
+      m.rk[e] = 0u;
+    }
+  } else {             // fewer threads than candidates: a thread ranks several
+#pragma unroll 1
+    for (int e = tm.tid; e < cnt; e += tm.nt) {
+      const unsigned long long ce = m.cand[e];
+      uint32_t rank = 0;
+#pragma unroll 4
+      for (int f = 0; f < cnt; ++f) rank += m.cand[f] > ce;
+      if ((int)rank == need - 1) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }
+    }
+  }
+  tm.sync();
+  Thr r;
+  r.key = dec[5]; r.idx = (int)dec[6];
+  tm.sync();
+  return r;
+}
+
+__device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const TeamMem& m, uint32_t lo, uint32_t span,
+                        int cnt_in) {
   const int lane = threadIdx.x & 31;
   uint32_t* dec = m.red + tm.nw * 16;  // [0] bstar [1] cstar [2] acc [5] key [6] idx [7] cand count
-  int need = k, cnt_in = n;
+  int need = k;
   Thr r;
   for (;;) {
     if (span == 0) {  // all survivors share one key: the `need` lowest indices win
@@ -216,7 +261,7 @@ __device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const Team
       tm.sync();
       return r;
     }
-    if (cnt_in <= 64) {  // collect the survivors (any order) and rank them
+    if (cnt_in <= CAND) {  // collect the survivors (any order) and rank them
       if (tm.tid == 0) dec[7] = 0u;
       tm.sync();
 #pragma unroll 4
@@ -224,27 +269,11 @@ __device__ Thr team_kth(const Keys& ks, int n, int k, const Team& tm, const Team
         const uint32_t key = ks.get(i);
         if ((key - lo) <= span) {
           const uint32_t pos = atomicAdd(&dec[7], 1u);
-          m.candk[pos] = key;
-          m.candi[pos] = i;
+          m.cand[pos] = ((unsigned long long)key << 32) | (uint32_t)~i;
         }
       }
       tm.sync();
-#pragma unroll 1
-      for (int e = tm.tid; e < cnt_in; e += tm.nt) {
-        const uint32_t ke = m.candk[e];
-        const int ie = m.candi[e];
-        int rank = 0;
-#pragma unroll 4
-        for (int f = 0; f < cnt_in; ++f) {
-          const uint32_t kf = m.candk[f];
-          rank += (kf > ke) || (kf == ke && m.candi[f] < ie);
-        }
-        if (rank == need - 1) { dec[5] = ke; dec[6] = (uint32_t)ie; }  // exactly one: ranks are a permutation
-      }
-      tm.sync();
-      r.key = dec[5]; r.idx = (int)dec[6];
-      tm.sync();
-      return r;
+      return team_rank(cnt_in, need, tm, m);
     }
     const int sh = max(0, (32 - __clz(span)) - m.hbits);  // (span >> sh) < 2^hbits
 #pragma unroll 4
@@ -341,10 +370,15 @@ __device__ uint32_t team_emit(const Keys& ks, int n, int k, const Thr& t, const 
 }
 
 // ---------------------------------------------------------------------------------------------
+struct StepArgs;
+__device__ __forceinline__ int seq_len(const StepArgs& a, int b);
 struct StepArgs {
   alignas(64) CUtensorMap mapK;  // bf16 [rows = n_pages*Hkv*bs, d], box [bs, 64], 128-byte swizzle
   alignas(64) CUtensorMap mapV;
   const uint16_t* kp; const uint16_t* vp; const int32_t* table; const int32_t* seq_lens;
+  // fused append (a0): app = 1 -> seq_lens holds the lengths BEFORE the append, every length below is +1
+  const uint16_t* k_new; const uint16_t* v_new; uint16_t* kp_w; uint16_t* vp_w; uint4* summ_w; double* open_sum;
+  int32_t* seq_lens_w; int app;
   const uint16_t* q; const uint4* summ; float* out;
   // layer state (already offset to the layer)
   float* scores; double* ema_l; double* ema_v; int32_t* n_state; const double* theta;
@@ -358,6 +392,8 @@ struct StepArgs {
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
   float scale; float pace_ns; double score_c;
 };
+
+__device__ __forceinline__ int seq_len(const StepArgs& a, int b) { return __ldg(a.seq_lens + b) + a.app; }
 
 template <int D, int BS>
 struct Tile {
@@ -404,7 +440,8 @@ __device__ __forceinline__ void tile_load(unsigned char* Ks, unsigned long long*
 template <int D, int BS>
 __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long long* bars, uint32_t phase,
                                              const StepArgs& a, int b, int h, int valid, float* O, float* Mo,
-                                             float* Lo, int width, int slot) {
+                                             float* Lo, int width, int slot, const uint16_t* patch_k,
+                                             const uint16_t* patch_v) {
   using T = Tile<D, BS>;
   constexpr int SUB = T::SUB, NT8 = SUB / 8;
   unsigned char* Vs = Ks + T::HALF;
@@ -433,6 +470,12 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
   const float sl2 = a.scale * LOG2E_F;
 
   mbar_wait(&bars[0], phase);  // K landed
+  if (patch_k) {  // fused append: the token appended by this launch is not in the cache yet
+    if (lane < D / 8)
+      *reinterpret_cast<uint4*>(const_cast<unsigned char*>(T::at(Ks, valid - 1, lane))) =
+          __ldg(reinterpret_cast<const uint4*>(patch_k) + lane);
+    __syncwarp();
+  }
 #pragma unroll
   for (int st = 0; st < BS / SUB; ++st) {
     const int tok0 = st * SUB;
@@ -477,6 +520,12 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
     mrun0 = mn0; mrun1 = mn1;
     if (st == 0) {
       mbar_wait(&bars[1], phase);  // V landed
+      if (patch_v) {
+        if (lane < D / 8)
+          *reinterpret_cast<uint4*>(const_cast<unsigned char*>(T::at(Vs, valid - 1, lane))) =
+              __ldg(reinterpret_cast<const uint4*>(patch_v) + lane);
+        __syncwarp();
+      }
       if (valid < BS) {            // open block: 0 * (whatever an unwritten slot holds) must not reach P V
         for (int i = lane; i < (BS - valid) * T::NBOX * 8; i += 32) {
           const int r = valid + i / (T::NBOX * 8), c = i % (T::NBOX * 8);
@@ -557,7 +606,7 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
   for (int r = sub; r < nld; r += RW) cp_async16(st + r * LPR, rows + (size_t)r * LPR);
   cp_async_commit();
   if (tl && lane == 0) tl[12] = gtime();
-  const int len = __ldg(a.seq_lens + b);
+  const int len = seq_len(a, b);
   // the group's queries summed per channel (exact in fp64): the 8 channels this lane owns
   double qs[8];
 #pragma unroll
@@ -585,6 +634,37 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
   cp_async_wait<0>();
   __syncwarp();
   if (tl && lane == 0) tl[13] = gtime();
+  if (a.app) {
+    // a0: the warp that scores the block the new token falls in appends it: cache slot, running sum
+    // and mean-key summary (exact fp64 sum, one division, one RNE to bf16, Q2) -- and patches the
+    // summary row it has just staged, so the score below is the score after the append.
+    const int pos = len - 1, ob = pos / a.bs, slot = pos - ob * a.bs;
+    if (ob >= r0 && ob < r0 + nr && sub == 0) {
+      const size_t ch = ((size_t)b * a.Hkv + h) * D + l * 8;
+      const uint4 kn = __ldg(reinterpret_cast<const uint4*>(a.k_new + ch));
+      const uint4 vn = __ldg(reinterpret_cast<const uint4*>(a.v_new + ch));
+      const size_t page = (size_t)__ldg(a.table + (size_t)b * a.MB + ob);
+      const size_t dst = ((page * a.Hkv + h) * a.bs + slot) * (size_t)D + l * 8;
+      *reinterpret_cast<uint4*>(a.kp_w + dst) = kn;
+      *reinterpret_cast<uint4*>(a.vp_w + dst) = vn;
+      const uint32_t w[4] = {kn.x, kn.y, kn.z, kn.w};
+      uint32_t o[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const double x0 = (double)bf16_lo(w[j]), x1 = (double)bf16_hi(w[j]);
+        const double s0 = slot == 0 ? x0 : __dadd_rn(a.open_sum[ch + 2 * j], x0);
+        const double s1 = slot == 0 ? x1 : __dadd_rn(a.open_sum[ch + 2 * j + 1], x1);
+        a.open_sum[ch + 2 * j] = s0;
+        a.open_sum[ch + 2 * j + 1] = s1;
+        o[j] = (uint32_t)f64_to_bf16_rne(__ddiv_rn(s0, (double)(slot + 1))) |
+               ((uint32_t)f64_to_bf16_rne(__ddiv_rn(s1, (double)(slot + 1))) << 16);
+      }
+      const uint4 row = make_uint4(o[0], o[1], o[2], o[3]);
+      st[(ob - r0) * LPR] = row;
+      a.summ_w[(((size_t)b * a.Hkv + h) * a.MB + ob) * LPR + l] = row;
+    }
+    __syncwarp();
+  }
 #pragma unroll 1
   for (int rr0 = 0; rr0 < nr; rr0 += 4 * RW) {  // warp-uniform trip count (full-mask shuffles below)
     double acc[4];
@@ -616,6 +696,113 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Fast path of the selection for rows with n <= KB * team threads (every config of BASELINE.json):
+// thread t holds the keys of the blocks t, t + nt, ... in REGISTERS, so the passes below are
+// straight-line predicated code without shared-memory round trips or per-element branches.  The
+// results are the same exact (key desc, index asc) selection; rows that do not fit, or whose first
+// pass leaves more than CAND candidates, continue in the generic code (team_kth / team_emit).
+constexpr int KB = 12;
+
+// First pass with a fixed bucket map (the top hbits of the key: monotone in the key), then the
+// survivors are ranked directly.  k < n.
+__device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& ks, int n, int k, const Team& tm,
+                                        const TeamMem& m, unsigned long long* tl) {
+  uint32_t* dec = m.red + tm.nw * 16;
+  const int sh = 32 - m.hbits;
+#pragma unroll
+  for (int e = 0; e < KB; ++e) {
+    const int i = tm.tid + e * tm.nt;
+    if (i < n) red_shared_add(&m.hist[key[e] >> sh], 1u);
+  }
+  if (tm.tid == 0) dec[7] = 0u;
+  tm.sync();
+  if (tl && tm.tid == 0) tl[12] = gtime();
+  int bstar, cstar, acc;
+  team_pick(m.hist, 1 << m.hbits, k, tm, m, bstar, cstar, acc);
+  if (tl && tm.tid == 0) tl[13] = gtime();
+  const int need = k - acc;
+  const uint32_t lo = (uint32_t)bstar << sh, span = (1u << sh) - 1u;
+  Thr r;
+  if (need == cstar) { r.key = lo; r.idx = 0x7fffffff; return r; }  // the whole bucket is selected
+  if (cstar > CAND) return team_kth(ks, n, need, tm, m, lo, span, cstar);
+#pragma unroll
+  for (int e = 0; e < KB; ++e) {
+    const int i = tm.tid + e * tm.nt;
+    if (i < n && (key[e] - lo) <= span) {
+      const uint32_t pos = atomicAdd(&dec[7], 1u);
+      m.cand[pos] = ((unsigned long long)key[e] << 32) | (uint32_t)~i;
+    }
+  }
+  tm.sync();
+  if (tl && tm.tid == 0) tl[14] = gtime();
+  return team_rank(cstar, need, tm, m);
+}
+
+// Ordered emission from the registers (see team_emit for the outputs).
+__device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, int k, const Thr& t, const Team& tm,
+                                              const TeamMem& m, int32_t* list, int width, uint32_t* mask_g,
+                                              int32_t* Mlist, int widthM) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt = (1u << lane) - 1u;
+  const int nwd = (n + 31) >> 5, nw32 = tm.nt >> 5;
+  uint32_t* dec = m.red + tm.nw * 16;
+  uint32_t bal[KB], mwd[KB];
+#pragma unroll
+  for (int e = 0; e < KB; ++e) {  // lanes of a warp hold 32 consecutive blocks: one mask word per (warp, e)
+    const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
+    const bool sel = i < n && k > 0 && selected(key[e], i, t);
+    bal[e] = __ballot_sync(FULL, sel);
+    mwd[e] = 0u;
+    if (w < nwd) {
+      if (Mlist) mwd[e] = bal[e] & ~m.pmask[w];
+      if (lane == 0) {
+        m.amask[w] = bal[e];
+        m.offs[w] = ((uint32_t)__popc(bal[e]) << 16) | (uint32_t)__popc(mwd[e]);
+      }
+    }
+  }
+  tm.sync();
+  if (tm.wid == 0) {  // exclusive scan of the per-word counts, in block order
+    uint32_t carry = 0;
+#pragma unroll 1
+    for (int w0 = 0; w0 < nwd; w0 += 32) {
+      const int w = w0 + lane;
+      const uint32_t v = w < nwd ? m.offs[w] : 0u;
+      uint32_t incl = v;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t x = __shfl_up_sync(FULL, incl, off);
+        if (lane >= off) incl += x;
+      }
+      if (w < nwd) m.offs[w] = carry + incl - v;
+      carry += __shfl_sync(FULL, incl, 31);
+    }
+    if (lane == 0) dec[3] = carry;
+  }
+  tm.sync();
+#pragma unroll
+  for (int e = 0; e < KB; ++e) {
+    const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
+    if (w < nwd) {
+      const uint32_t off = m.offs[w];
+      if ((bal[e] >> lane) & 1u) {
+        list[(off >> 16) + __popc(bal[e] & lt)] = i;
+        if ((mwd[e] >> lane) & 1u) Mlist[(off & 0xffffu) + __popc(mwd[e] & lt)] = i;
+      }
+      if (mask_g && lane == 0) mask_g[w] = bal[e];
+    }
+  }
+  const uint32_t tot = dec[3];
+#pragma unroll 1
+  for (int j = (int)(tot >> 16) + tm.tid; j < width; j += tm.nt) list[j] = -1;
+  if (Mlist)
+#pragma unroll 1
+    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
+  tm.sync();
+  return tot;
+}
+
+// ---------------------------------------------------------------------------------------------
 // One row job by one team (a single code path for both kinds, so the kernel holds ONE copy of the
 // selection code: the instruction cache is 32 KB and this code runs once per step, on the
 // critical path).
@@ -631,7 +818,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   const bool is_sel = jj < R;
   const int row = is_sel ? jj : jj - R;
   const int b = row / a.Hkv;
-  const int nb = max(0, min(a.MB, (__ldg(a.seq_lens + b) + a.bs - 1) / a.bs));
+  const int nb = max(0, min(a.MB, (seq_len(a, b) + a.bs - 1) / a.bs));
   uint32_t* dec = m.red + tm.nw * 16;
   uint32_t* ctl = a.ctl;
   const float* sc = a.scores + (size_t)row * a.MB;
@@ -765,19 +952,34 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   Keys ks{in_sm ? smem_u32(m.keys) : 0u, is_sel ? sc : pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
-  if (k < n) {                      // (uniform over the team)
-    uint32_t lo, span;
-    team_range(kmin, kmax, tm, m, lo, span);
-    if (tl && tm.tid == 0) tl[9] = gtime();
-    t = team_kth(ks, n, k, tm, m, lo, span, tl);
+  const bool fast = in_sm && n <= KB * tm.nt;  // (uniform over the team)
+  uint32_t kreg[KB];
+  if (fast) {
+#pragma unroll
+    for (int e = 0; e < KB; ++e) {  // each thread re-reads only what it stored
+      const int i = tm.tid + e * tm.nt;
+      kreg[e] = i < n ? m.keys[i] : 0u;
+    }
+  }
+  if (k < n) {
+    if (fast) {
+      if (tl && tm.tid == 0) tl[9] = gtime();
+      t = fast_kth(kreg, ks, n, k, tm, m, tl);
+    } else {
+      uint32_t lo, span;
+      team_range(kmin, kmax, tm, m, lo, span);
+      if (tl && tm.tid == 0) tl[9] = gtime();
+      t = team_kth(ks, n, k, tm, m, lo, span, n);
+    }
   } else {
     tm.sync();
   }
   if (tl && tm.tid == 0) tl[10] = gtime();
-  const uint32_t tot =
-      team_emit(ks, n, k, t, tm, m, is_sel ? a.setA + (size_t)row * a.K : Pnext + (size_t)row * a.Bud,
-                is_sel ? a.K : a.Bud, is_sel ? a.maskA + (size_t)row * a.MBw : nullptr,
-                is_sel ? a.setM + (size_t)row * a.K : nullptr, a.K);
+  int32_t* list = is_sel ? a.setA + (size_t)row * a.K : Pnext + (size_t)row * a.Bud;
+  uint32_t* mask_g = is_sel ? a.maskA + (size_t)row * a.MBw : nullptr;
+  int32_t* Mlist = is_sel ? a.setM + (size_t)row * a.K : nullptr;
+  const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K)
+                            : team_emit(ks, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
   if (!is_sel) return;
   // ---- publish (select only) ----
@@ -971,7 +1173,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     uslot = unit / R; urow = unit - uslot * R;
     ub = urow / a.Hkv; uh = urow - ub * a.Hkv;
     ublk = __ldg(Pcur + (size_t)urow * a.Bud + uslot);
-    ulen = __ldg(a.seq_lens + ub);
+    ulen = seq_len(a, ub);
   };
   auto unit_decode_b = [&]() {
     if (ublk >= a.MB) ublk = -1;
@@ -1049,8 +1251,10 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     m.hist = p; p += 1 << m.hbits;
 #pragma unroll 1
     for (int i = tm.tid; i < (1 << m.hbits); i += tm.nt) m.hist[i] = 0u;
-    m.candk = p; p += 64;
-    m.candi = reinterpret_cast<int32_t*>(p); p += 64;
+    p += ((uintptr_t)p >> 2) & 1;  // 8-byte alignment
+    m.cand = reinterpret_cast<unsigned long long*>(p); p += 2 * CAND;
+    m.rk = p; p += CAND;
+    for (int i = tm.tid; i < CAND; i += tm.nt) m.rk[i] = 0u;
     m.plist = reinterpret_cast<int32_t*>(p); p += a.Bud;
     unsigned char* pool;
     if (job_cta) {
@@ -1110,15 +1314,19 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
           if (finished) break;
           urep = true;
           ub = urow / a.Hkv; uh = urow - ub * a.Hkv;
-          uvalid = min(BS, __ldg(a.seq_lens + ub) - ublk * BS);
+          ulen = seq_len(a, ub);
+          uvalid = min(BS, ulen - ublk * BS);
           upage = __ldg(a.table + (size_t)ub * a.MB + ublk);
         }
         tile_load<D, BS>(Ks, bars, a, upage, uh);
       }
       const int crow = urow, cslot = uslot;
+      const bool patch = a.app && uvalid > 0 && ublk == (ulen - 1) / BS;
       const bool crep = urep;
       tile_compute<D, BS>(Ks, bars, ph, a, ub, uh, uvalid, crep ? a.O_rep : a.O_spec, crep ? a.m_rep : a.m_spec,
-                          crep ? a.l_rep : a.l_spec, crep ? a.K : a.Bud, uslot);
+                          crep ? a.l_rep : a.l_spec, crep ? a.K : a.Bud, uslot,
+                          patch ? a.k_new + ((size_t)ub * a.Hkv + uh) * D : nullptr,
+                          patch ? a.v_new + ((size_t)ub * a.Hkv + uh) * D : nullptr);
       ph ^= 1u;
       pend = false;
       if (!crep) {
@@ -1158,6 +1366,8 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   }
   last = __shfl_sync(FULL, last, 0);
   if (last) {
+    if (a.app)
+      for (int b = lane; b < a.B; b += 32) a.seq_lens_w[b] += 1;
     if (lane == 0) {
       ctl[CTL_EXIT] = 0u;
       ctl[CTL_EPOCH] = ep;
@@ -1179,12 +1389,12 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   a.J = 2 * R <= c->n_sm / 4 ? 2 * R : 0;
   int W = 0, per_warp = 0;
   for (;;) {
-    a.scr_bytes = (3 * a.MBw + 24 + 128 + (a.J ? 0 : 256 + c->Bud)) * 4;
+    a.scr_bytes = (3 * a.MBw + 24 + 3 * CAND + 2 + (a.J ? 0 : 256 + c->Bud)) * 4;
     a.scr_bytes += (1024 - (a.buf_bytes + a.scr_bytes) % 1024) % 1024;  // tile buffers stay 1024-byte aligned (swizzle atom)
     per_warp = a.buf_bytes + a.scr_bytes;
     W = std::min(T::WMAX, (c->smem_optin - 1024) / per_warp);
     if (W < 1) return cudaErrorInvalidConfiguration;
-    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 128 + 64 + c->Bud;
+    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 3 * CAND + 2 + 64 + c->Bud;
     if (a.J && team_words * 4 > (size_t)W * per_warp) { a.J = 0; continue; }
     break;
   }
@@ -1259,13 +1469,17 @@ static int page_map(prr_ctx* c, const void* base, CUtensorMap* out) {
 }
 
 int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
-                int spec, cudaStream_t s) {
+                int spec, cudaStream_t s, const void* k_new, const void* v_new) {
   const size_t r = (size_t)kv->layer * c->maxB * c->Hkv;
   StepArgs a{};
   if (int e = page_map(c, kv->k_pages, &a.mapK)) return e;
   if (int e = page_map(c, kv->v_pages, &a.mapV)) return e;
   a.kp = (const uint16_t*)kv->k_pages; a.vp = (const uint16_t*)kv->v_pages;
   a.table = kv->block_table; a.seq_lens = kv->seq_lens;
+  a.app = (k_new && v_new) ? 1 : 0;
+  a.k_new = (const uint16_t*)k_new; a.v_new = (const uint16_t*)v_new;
+  a.kp_w = (uint16_t*)kv->k_pages; a.vp_w = (uint16_t*)kv->v_pages; a.summ_w = (uint4*)summaries;
+  a.open_sum = c->open_sum + (size_t)kv->layer * c->maxB * c->Hkv * c->D; a.seq_lens_w = (int32_t*)kv->seq_lens;
   a.q = (const uint16_t*)q; a.summ = (const uint4*)summaries; a.out = out;
   a.scores = c->scores + r * c->MB;
   a.ema_l = c->ema_l + r * c->MB; a.ema_v = c->ema_v + r * c->MB;

@@ -448,8 +448,9 @@ static void enqueue_ema(prr_ctx* c, const prr_paged_kv* kv, cudaStream_t main, b
 }
 
 static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries,
-                      float* out, int spec, cudaStream_t s, const char* fn) {
-  const int e = launch_step(c, kv, q, summaries, out, spec, s);
+                      float* out, int spec, cudaStream_t s, const char* fn, const void* k_new = nullptr,
+                      const void* v_new = nullptr) {
+  const int e = launch_step(c, kv, q, summaries, out, spec, s, k_new, v_new);
   if (e) {
     cudaGetLastError();
     PRR_FAIL(c, PRR_E_CUDA, "%s: fused step launch: %s", fn, cudaGetErrorString((cudaError_t)e));
@@ -525,6 +526,22 @@ extern "C" int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const v
   return check_launch(ctx, "prr_decode_step");
 }
 
+extern "C" int32_t prr_step_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* k_new,
+                                   const void* v_new, void* summaries, float* out, int32_t sequential,
+                                   void* stream) {
+  CHECK_KV("prr_step_append");
+  CHECK_PTR(q, "prr_step_append"); CHECK_PTR(k_new, "prr_step_append"); CHECK_PTR(v_new, "prr_step_append");
+  CHECK_PTR(summaries, "prr_step_append");
+  if (!out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_step_append: null out");
+  if (ctx->fused)  // a0 rides in the same launch as a1-a8
+    return fused_step(ctx, kv, q, summaries, out, sequential ? 0 : 1, (cudaStream_t)stream, "prr_step_append",
+                      k_new, v_new);
+  const int r = prr_append(ctx, kv, k_new, v_new, summaries, stream);
+  if (r) return r;
+  return sequential ? prr_attend(ctx, kv, q, summaries, out, stream)
+                    : prr_decode_step(ctx, kv, q, summaries, out, stream);
+}
+
 extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_host,
                                         const void* k_new_host, const void* v_new_host, void* summaries,
                                         float* out_host, void* stream) {
@@ -536,9 +553,7 @@ extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, co
   PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_q, q_host, qb * 2, cudaMemcpyHostToDevice, s));
   PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_k, k_new_host, kb * 2, cudaMemcpyHostToDevice, s));
   PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_v, v_new_host, kb * 2, cudaMemcpyHostToDevice, s));
-  int r = prr_append(ctx, kv, ctx->st_k, ctx->st_v, summaries, stream);
-  if (r) return r;
-  r = prr_decode_step(ctx, kv, ctx->st_q, summaries, ctx->st_out, stream);
+  const int r = prr_step_append(ctx, kv, ctx->st_q, ctx->st_k, ctx->st_v, summaries, ctx->st_out, 0, stream);
   if (r) return r;
   PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));
   PRR_CUDA(ctx, cudaStreamSynchronize(s));

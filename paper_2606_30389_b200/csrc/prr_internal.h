@@ -112,7 +112,7 @@ void launch_merge(prr_ctx* c, int batch, const int32_t* merge_src, const int32_t
 // k_step.cu: one fused launch for a whole layer-step; spec = 0 is the sequential path.  Returns 0
 // or a cudaError_t.
 int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
-                int spec, cudaStream_t s);
+                int spec, cudaStream_t s, const void* k_new = nullptr, const void* v_new = nullptr);
 // k_calib.cu
 int launch_calibrate(prr_ctx* c, int layer, int seq, const float* IS, int T, int N,
                      const int32_t* n_valid, cudaStream_t s);

@@ -20,7 +20,8 @@ FUSED, STREAMS = 0, 1
 SYMBOLS = [
     "prr_create", "prr_destroy", "prr_last_error", "prr_version", "prr_build_summaries", "prr_append",
     "prr_set_ema_params", "prr_reset_ema", "prr_calibrate", "prr_predict", "prr_ema_update", "prr_score",
-    "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_decode_step_host",
+    "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_step_append",
+    "prr_decode_step_host",
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
     "prr_timeline_enable", "prr_timeline_read",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
@@ -201,6 +202,12 @@ class Context:
     def decode_step(self, kv, q, summaries, out, stream=None):
         self._chk(lib().prr_decode_step(self._h, C.byref(kv), C.c_void_p(_p(q)), C.c_void_p(_p(summaries)),
                                         C.c_void_p(_p(out)), C.c_void_p(_stream(stream))))
+
+    def step_append(self, kv, q, k_new, v_new, summaries, out, sequential=False, stream=None):
+        """prr_append + prr_decode_step (or prr_attend) as one call: one launch when fused."""
+        self._chk(lib().prr_step_append(self._h, C.byref(kv), C.c_void_p(_p(q)), C.c_void_p(_p(k_new)),
+                                        C.c_void_p(_p(v_new)), C.c_void_p(_p(summaries)), C.c_void_p(_p(out)),
+                                        C.c_int32(int(bool(sequential))), C.c_void_p(_stream(stream))))
 
     def decode_step_host(self, kv, q_host, k_new_host, v_new_host, summaries, out_host, stream=None):
         self._chk(lib().prr_decode_step_host(self._h, C.byref(kv), C.c_void_p(_p(q_host)),

@@ -71,6 +71,12 @@ class GpuLayer:
         (self.ctx.attend if sequential else self.ctx.decode_step)(self.kv, q, self.summ, self.out)
         return self.out
 
+    def step_append(self, t, sequential=False):
+        """prr_step_append: a0-a8 in one call (one launch with the fused orchestration)."""
+        self.ctx.step_append(self.kv, self.inp.q_dec[t].contiguous(), self.inp.k_new[t].contiguous(),
+                             self.inp.v_new[t].contiguous(), self.summ, self.out, sequential=sequential)
+        return self.out
+
     def sets(self):
         cfg = self.cfg
         dev = self.out.device

@@ -238,7 +238,8 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
             assert np.array_equal(H.unpad(M[b, h]), np.setdiff1d(A[b, h], P[b, h]))
 
 
-def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True):
+def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True,
+               fused_append=False):
     steps = cfg.steps if steps is None else steps
     cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps)
     twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget) if seq_check else None
@@ -252,9 +253,10 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
     worst = (0.0, 0.0)
     hits = tot = 0
     for t in range(steps):
-        gl.append(t)
+        if not fused_append:
+            gl.append(t)
         ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
-        out = gl.step(t)
+        out = gl.step_append(t) if fused_append else gl.step(t)
         torch.cuda.synchronize()
         r = ol.step(synth.bits(inp.q_dec[t]))
         sc = gl.scores()
@@ -275,6 +277,11 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
                 hits += len(r["A"][b][h]) - len(r["M"][b][h]); tot += len(r["A"][b][h])
     st = gl.ctx.get_stats()
     assert st[0] == tot and st[1] == hits and st[2] == tot - hits
+    if fused_append and twin:   # the cache, the summaries and the lengths the fused append leaves behind
+        assert torch.equal(gl.seq_lens, twin.seq_lens), "seq_lens after fused append"
+        assert torch.equal(gl.k_pages.view(torch.int16), twin.k_pages.view(torch.int16)), "k_pages after fused append"
+        assert torch.equal(gl.v_pages.view(torch.int16), twin.v_pages.view(torch.int16)), "v_pages after fused append"
+        assert torch.equal(gl.summ.view(torch.int16), twin.summ.view(torch.int16)), "summaries after fused append"
     return worst, hits / max(tot, 1)
 
 
@@ -282,6 +289,21 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
 @pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
 def test_decode_steps_small_shapes(cfg, policy):
     run_decode(cfg, policy=policy)
+
+
+@pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
+@pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
+def test_step_append_small_shapes(cfg, policy):
+    """prr_step_append (a0 fused into the step's launch) against the oracle and against the
+    separate prr_append + prr_attend calls of a twin layer, including the cache it leaves behind."""
+    run_decode(cfg, policy=policy, fused_append=True)
+
+
+def test_step_append_block_boundary_and_full_size():
+    """Appends that open a new block (slot 0) and the headline config at full size."""
+    run_decode(T16.scaled(ctx_lo=16 * 5, ctx_hi=16 * 5), steps=20, fused_append=True)   # starts on a boundary
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=4, fused_append=True)
+    run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=2, seq_check=False, fused_append=True)
 
 
 def test_decode_c0_full():
