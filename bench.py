@@ -4,11 +4,11 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--layers R] [--impl reference]
 
 A "step" is ONE LAYER-STEP: one pass of the whole hot path (append + summary refresh, score, top-K,
-diff, EMA predict/update, speculative attention over P on a second stream, repair of A\\P, merge)
+diff, EMA predict/update, speculative attention over P, repair of A\\P, merge: ONE fused launch)
 for one layer of the named config.  R independent seeded layer caches are visited round-robin, as a
 model's forward pass does, so every step reads a cache that left L2 long ago ("inputs larger than
 L2": R x ~30 MB touched per visit vs the 126 MB L2).  Consecutive steps are ordered on one stream:
-the time per step in steady state IS the critical path; EMA update/predict overlap later steps.
+the time per step in steady state IS the critical path (EMA update/predict run on spare SMs inside it).
 Steps are captured into CUDA graphs (chunks of 4R steps) and the K timed steps are launched back
 to back between two CUDA events.  One JSON line is printed by rank 0.
 """
@@ -31,6 +31,9 @@ import numpy as np
 import torch
 
 from paper_2606_30389_b200 import synth
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_step launch (ncu --set full, profiles/r1_k_step_C2.md)
+NCU_TRAFFIC = {"C2": 32_050_000}
 
 METRIC = "per_layer_dsa_decode_critical_path"
 UNIT = "us"
@@ -294,34 +297,9 @@ def main():
         for g in g2:
             g.destroy()
 
-    # ---- dominant kernel alone (speculative per-block attention), rotating layers, CUDA events ---
-    Bud = cfg.Bud
-    P = torch.empty(cfg.B, cfg.Hkv, Bud, dtype=torch.int32, device=dev)
-    Op = torch.empty(cfg.B, cfg.Hq, Bud, cfg.d, dtype=torch.float32, device=dev)
-    mp = torch.empty(cfg.B, cfg.Hq, Bud, dtype=torch.float32, device=dev)
-    lp = torch.empty_like(mp)
-    Ps = []
-    for l in range(R):
-        st.ctx.predict(l, cfg.B, P)
-        Ps.append(P.clone())
-    torch.cuda.synchronize()
-    units = float(sum((p >= 0).sum().item() for p in Ps)) / R          # (block, KV head) units per launch
-    reps = max(3, min(40, 2000 // R))
-    k_ms = []
-    with torch.cuda.stream(stream):
-        for rep in range(reps + 1):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for l in range(R):
-                st.ctx.speculate(st.kvs[l], st.inps[l].q_dec[0], Ps[l], Op, mp, lp, stream=stream)
-            e1.record(stream)
-            e1.synchronize()
-            if rep:
-                k_ms.append(e0.elapsed_time(e1) / R)
-    k_us = float(np.median(k_ms)) * 1e3
-    unit_bytes = 4 * cfg.bs * cfg.d                                     # K and V tile of one block, bf16
+    # ---- dominant kernel: the fused layer-step k_step is the ONLY kernel of a step (a0-a8 in one launch),
+    # so its average launch duration is the timed region / K (CUDA events on the launching stream).
     peak, peak_src = peaks()
-    achieved = units * unit_bytes / (k_us * 1e-6) / 1e9
 
     # ---- end to end through the C-ABI with HOST buffers -----------------------------------------
     e2e = None
@@ -369,11 +347,15 @@ def main():
                           "frac_of_nominal_8TBs": abytes / (us_step * 1e-6) / 1e9 / 8000.0, "peak_source": peak_src},
         "sequential_us": seq_us, "speedup_vs_sequential": (seq_us / us_step) if seq_us else None,
         "hit_rate": stats[1] / max(stats[0], 1), "mean_missed_per_row": stats[2] * K and stats[2] / (K * cfg.B * cfg.Hkv),
-        "roofline": {"kernel": "k_partial (speculative per-block attention over P)", "bound": "hbm",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "us_per_launch": k_us, "units_per_launch": units,
-                     "bytes_per_unit": unit_bytes, "peak_source": peak_src,
-                     "how": "kernel alone, CUDA events on its launch stream, round-robin over the layer caches"},
+        "roofline": {"kernel": "k_step (fused persistent layer-step: append, score, top-K, EMA, speculative "
+                               "units, repair, merge in one cooperative launch)",
+                     "bound": "hbm", "achieved": abytes / (us_step * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": abytes / (us_step * 1e-6) / 1e9 / peak,
+                     "traffic": NCU_TRAFFIC.get(cfg.name), "us_per_launch": us_step, "launches_per_step": 1,
+                     "units_per_launch": 1, "bytes_per_unit": int(abytes), "peak_source": peak_src,
+                     "how": "algorithmic bytes of one layer-step (summaries + selected KV, SURVEY.md 8(d)) / "
+                            "(timed region / K launches); the step is latency-bound, not bandwidth-bound: see "
+                            "DESIGN.md 'Where the time goes'"},
         "cpu_baseline": {"value": cpu_us, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": f"{n_cpu} layer-steps of layer 0 (numpy fp64 oracle, fixed theta, no calibration)"},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,

@@ -741,7 +741,7 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
 // Ordered emission from the registers (see team_emit for the outputs).
 __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, int k, const Thr& t, const Team& tm,
                                               const TeamMem& m, int32_t* list, int width, uint32_t* mask_g,
-                                              int32_t* Mlist, int widthM) {
+                                              int32_t* Mlist, int widthM, unsigned long long* tl) {
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
   const int nwd = (n + 31) >> 5, nw32 = tm.nt >> 5;
@@ -762,6 +762,7 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
     }
   }
   tm.sync();
+  if (tl && tm.tid == 0) tl[3] = gtime();
   if (tm.wid == 0) {  // exclusive scan of the per-word counts, in block order
     uint32_t carry = 0;
 #pragma unroll 1
@@ -780,6 +781,7 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
     if (lane == 0) dec[3] = carry;
   }
   tm.sync();
+  if (tl && tm.tid == 0) tl[4] = gtime();
 #pragma unroll
   for (int e = 0; e < KB; ++e) {
     const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
@@ -978,7 +980,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   int32_t* list = is_sel ? a.setA + (size_t)row * a.K : Pnext + (size_t)row * a.Bud;
   uint32_t* mask_g = is_sel ? a.maskA + (size_t)row * a.MBw : nullptr;
   int32_t* Mlist = is_sel ? a.setM + (size_t)row * a.K : nullptr;
-  const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K)
+  const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K, tl)
                             : team_emit(ks, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
   if (!is_sel) return;
