@@ -1001,7 +1001,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
       }
     }
     for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
-    if (lane == 0) a.mn[row] = base + nM;
+    if (lane == 0) a.mn[row] = (base << 16) | (base + nM);  // speculative entries | all entries
   }
   if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
@@ -1035,95 +1035,114 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   uint32_t* cs = reinterpret_cast<uint32_t*>(buf) + E;   // [E] slot codes (REP bit: repair buffers)
   float* ls = reinterpret_cast<float*>(buf) + 2 * E;     // [E] l
   // the row's merge list was written by select(row): slot codes, speculative slots first
-  const int n = __ldcg(a.mn + row);
+  const uint32_t pk = (uint32_t)__ldcg(a.mn + row);
+  const int n = (int)(pk & 0xffffu), nh = (int)(pk >> 16);
   const uint32_t* ms = a.msrc + (size_t)row * E;
-  float mx = -CUDART_INF_F;
-  // (rolled loops with a run-time trip count serialise their loads: batches with predication instead)
-#pragma unroll 1
-  for (int eb = 0; eb < n; eb += 4 * 32) {  // warp-uniform trips (votes inside)
-    const int e0 = eb + lane;
-    uint32_t code[4];
-    float me[4], le[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < n ? __ldcg(ms + e0 + 32 * u) : 0u;
-    {  // wait for exactly these entries' units (over-predicted blocks that are not merged are not waited
-       // for); the warp stays converged and exits on a vote
-      uint32_t it = 0;
-#pragma unroll 1
-      for (;;) {
-        bool ok = true;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const uint32_t j = code[u] & ~REP;
-          const uint32_t* fp = (code[u] & REP) ? a.ufr + (size_t)row * a.K + j : a.ufs + (size_t)row * a.Bud + j;
-          if (e0 + 32 * u < n) ok = ok && (ld_acquire(fp) == ep);
-        }
-        if (__all_sync(FULL, ok)) break;
-        __nanosleep(20);
-        if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const uint32_t j = code[u] & ~REP;
-      const bool on = e0 + 32 * u < n;
-      const float* mp = (code[u] & REP) ? a.m_rep + hb * a.K + j : a.m_spec + hb * a.Bud + j;
-      const float* lp = (code[u] & REP) ? a.l_rep + hb * a.K + j : a.l_spec + hb * a.Bud + j;
-      me[u] = on ? __ldcg(mp) : -CUDART_INF_F;
-      le[u] = on ? __ldcg(lp) : 0.f;
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int e = e0 + 32 * u;
-      if (e < n) { ws[e] = me[u]; ls[e] = le[u]; cs[e] = code[u]; mx = fmaxf(mx, me[u]); }
-    }
-  }
-#pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
-  __syncwarp();
-  float lsum = 0.f;
-#pragma unroll 2
-  for (int e = lane; e < n; e += 32) {
-    const float me = ws[e];
-    const float w = me == -CUDART_INF_F ? 0.f : ex2((me - mx) * LOG2E_F);
-    ws[e] = w;
-    lsum = fmaf(w, ls[e], lsum);
-  }
-#pragma unroll
-  for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
-  __syncwarp();
   const int grp = lane >> 3, l8 = lane & 7;
   const float* Os = a.O_spec + hb * a.Bud * D + dq * 32 + l8 * 4;
   const float* Or = a.O_rep + hb * a.K * D + dq * 32 + l8 * 4;
-  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  // Two segments folded by Eq. 6-8: first the speculative entries (their units finished while
+  // selection ran), then the repaired ones -- so only the few repair rows are left to fetch once
+  // the last repair unit has published.
+  float mrun = -CUDART_INF_F, lrun = 0.f;
+  float4 arun = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-  for (int e0 = grp; e0 < n; e0 += 4 * 10) {  // 10 rows per lane (40 entries per warp) in flight
-    float4 x[10];
-    float w[10];
+  for (int seg = 0; seg < 2; ++seg) {
+    const int s0 = seg ? nh : 0, s1 = seg ? n : nh;
+    if (s1 <= s0) continue;
+    float mx = -CUDART_INF_F;
+    // (rolled loops with a run-time trip count serialise their loads: batches with predication instead)
+#pragma unroll 1
+    for (int eb = s0; eb < s1; eb += 4 * 32) {  // warp-uniform trips (votes inside)
+      const int e0 = eb + lane;
+      uint32_t code[4];
+      float me[4], le[4];
 #pragma unroll
-    for (int u = 0; u < 10; ++u) {
-      const int e = e0 + 4 * u;
-      const bool on = e < n;
-      const uint32_t code = on ? cs[e] : 0u;
-      w[u] = on ? ws[e] : 0.f;
-      const float* Op = (code & REP) ? Or + (size_t)(code & ~REP) * D : Os + (size_t)code * D;
-      x[u] = on ? __ldcg(reinterpret_cast<const float4*>(Op)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < s1 ? __ldcg(ms + e0 + 32 * u) : 0u;
+      {  // wait for exactly these entries' units (over-predicted blocks that are not merged are not
+         // waited for); the warp stays converged and exits on a vote
+        uint32_t it = 0;
+#pragma unroll 1
+        for (;;) {
+          bool ok = true;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const uint32_t j = code[u] & ~REP;
+            const uint32_t* fp = (code[u] & REP) ? a.ufr + (size_t)row * a.K + j : a.ufs + (size_t)row * a.Bud + j;
+            if (e0 + 32 * u < s1) ok = ok && (ld_acquire(fp) == ep);
+          }
+          if (__all_sync(FULL, ok)) break;
+          __nanosleep(20);
+          if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const uint32_t j = code[u] & ~REP;
+        const bool on = e0 + 32 * u < s1;
+        const float* mp = (code[u] & REP) ? a.m_rep + hb * a.K + j : a.m_spec + hb * a.Bud + j;
+        const float* lp = (code[u] & REP) ? a.l_rep + hb * a.K + j : a.l_spec + hb * a.Bud + j;
+        me[u] = on ? __ldcg(mp) : -CUDART_INF_F;
+        le[u] = on ? __ldcg(lp) : 0.f;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int e = e0 + 32 * u;
+        if (e < s1) { ws[e] = me[u]; ls[e] = le[u]; cs[e] = code[u]; mx = fmaxf(mx, me[u]); }
+      }
     }
 #pragma unroll
-    for (int u = 0; u < 10; ++u) {
-      acc.x = fmaf(w[u], x[u].x, acc.x); acc.y = fmaf(w[u], x[u].y, acc.y);
-      acc.z = fmaf(w[u], x[u].z, acc.z); acc.w = fmaf(w[u], x[u].w, acc.w);
+    for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
+    __syncwarp();
+    float lsum = 0.f;
+#pragma unroll 2
+    for (int e = s0 + lane; e < s1; e += 32) {
+      const float me = ws[e];
+      const float w = me == -CUDART_INF_F ? 0.f : ex2((me - mx) * LOG2E_F);
+      ws[e] = w;
+      lsum = fmaf(w, ls[e], lsum);
     }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
+    __syncwarp();
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+    for (int e0 = s0 + grp; e0 < s1; e0 += 4 * 10) {  // 10 rows per lane (40 entries per warp) in flight
+      float4 x[10];
+      float w[10];
+#pragma unroll
+      for (int u = 0; u < 10; ++u) {
+        const int e = e0 + 4 * u;
+        const bool on = e < s1;
+        const uint32_t code = on ? cs[e] : 0u;
+        w[u] = on ? ws[e] : 0.f;
+        const float* Op = (code & REP) ? Or + (size_t)(code & ~REP) * D : Os + (size_t)code * D;
+        x[u] = on ? __ldcg(reinterpret_cast<const float4*>(Op)) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int u = 0; u < 10; ++u) {
+        acc.x = fmaf(w[u], x[u].x, acc.x); acc.y = fmaf(w[u], x[u].y, acc.y);
+        acc.z = fmaf(w[u], x[u].z, acc.z); acc.w = fmaf(w[u], x[u].w, acc.w);
+      }
+    }
+    // fold the segment into the running state (Eq. 6-8, unnormalised)
+    const float mnew = fmaxf(mrun, mx);
+    const float fo = mrun == -CUDART_INF_F ? 0.f : ex2((mrun - mnew) * LOG2E_F);
+    const float fn = mx == -CUDART_INF_F ? 0.f : ex2((mx - mnew) * LOG2E_F);
+    arun.x = fo * arun.x + fn * acc.x; arun.y = fo * arun.y + fn * acc.y;
+    arun.z = fo * arun.z + fn * acc.z; arun.w = fo * arun.w + fn * acc.w;
+    lrun = fo * lrun + fn * lsum;
+    mrun = mnew;
   }
 #pragma unroll
   for (int off = 8; off <= 16; off <<= 1) {
-    acc.x += __shfl_xor_sync(FULL, acc.x, off); acc.y += __shfl_xor_sync(FULL, acc.y, off);
-    acc.z += __shfl_xor_sync(FULL, acc.z, off); acc.w += __shfl_xor_sync(FULL, acc.w, off);
+    arun.x += __shfl_xor_sync(FULL, arun.x, off); arun.y += __shfl_xor_sync(FULL, arun.y, off);
+    arun.z += __shfl_xor_sync(FULL, arun.z, off); arun.w += __shfl_xor_sync(FULL, arun.w, off);
   }
   if (grp == 0) {
     float4 o;
-    o.x = lsum > 0.f ? acc.x / lsum : 0.f; o.y = lsum > 0.f ? acc.y / lsum : 0.f;
-    o.z = lsum > 0.f ? acc.z / lsum : 0.f; o.w = lsum > 0.f ? acc.w / lsum : 0.f;
+    o.x = lrun > 0.f ? arun.x / lrun : 0.f; o.y = lrun > 0.f ? arun.y / lrun : 0.f;
+    o.z = lrun > 0.f ? arun.z / lrun : 0.f; o.w = lrun > 0.f ? arun.w / lrun : 0.f;
     *reinterpret_cast<float4*>(a.out + hb * D + dq * 32 + l8 * 4) = o;
   }
   __syncwarp();
@@ -1344,12 +1363,18 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   if (tl && lane == 0) tl[4] = gtime();
 
   // ---- phase 5: merge, claimed by whoever is free ------------------------------------------------
-  if (job_cta || a.J == 0) {
+  {
+    // merge items are dealt out statically: one per job-CTA warp; what is left over goes to the
+    // worker warps from the top (the repair tickets went to the lowest-numbered ones)
     const int NT = a.B * a.Hq * NQ;
-    const int mw = a.J ? ((int)blockIdx.x - NWK) * W + warp : gw;  // merge items are dealt out statically
-    const int nmw = a.J ? a.J * W : NW;
+    const int njw = a.J * W;
+    int t0 = gw, tstep = NW;
+    if (a.J) {
+      if (job_cta) { t0 = ((int)blockIdx.x - NWK) * W + warp; tstep = NT; }
+      else { t0 = njw + (NWS - 1 - gw); tstep = NWS; }
+    }
 #pragma unroll 1
-    for (int t = mw; t < NT; t += nmw) {
+    for (int t = t0; t < NT; t += tstep) {
       const int bh = t / NQ, dq = t - bh * NQ;
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
