@@ -1165,6 +1165,11 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   uint32_t ph = 0;  // parity of the next tile to land in this warp's buffer
   if (lane == 0) { mbar_init(&bars[0], 1); mbar_init(&bars[1], 1); mbar_fence_init(); }
   __syncwarp();
+  // Programmatic dependent launch: let the next step's grid be scheduled now (its CTAs take the SMs
+  // as ours exit and its launch latency hides behind this step), and wait for the previous step's
+  // grid to have completed before the first global access.  No-ops without the launch attribute.
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
   uint32_t* ctl = a.ctl;
   const uint32_t ep = __ldcg(ctl + CTL_EPOCH) + 1u;  // this launch's epoch: the value every flag of the step takes
   const int R = a.B * a.Hkv;
@@ -1448,11 +1453,14 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   cfg.blockDim = dim3(32 * W);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
-  cudaLaunchAttribute at[1];
+  cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeCooperative;
   at[0].val.cooperative = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
-  cfg.numAttrs = 1;
+  static const int pdl = [] { const char* e = getenv("PRR_PDL"); return e ? atoi(e) : 1; }();
+  cfg.numAttrs = pdl ? 2 : 1;
   return cudaLaunchKernelEx(&cfg, k_step<D, BS>, a);
 }
 
