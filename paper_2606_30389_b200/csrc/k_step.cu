@@ -44,7 +44,7 @@ constexpr uint32_t SPIN_LIMIT = 1u << 22;  // ~0.1-0.5 s of polling, then give u
 
 // Dependencies between warps are epoch-valued FLAGS, not counters: a producer publishes with one
 // st.release of the launch's epoch (no atomics, nothing to reset), a consumer polls exactly the
-// flags of the items it needs.  ctl = header, then sel[Rmax], spec-unit flags [Rmax*Bud], repair-
+// flags of the items it needs.  ctl = header, then sel[Rmax] (M published), sel2[Rmax] (merge list published), spec-unit flags [Rmax*Bud], repair-
 // unit flags [Rmax*K], score-chunk flags [Rmax*MB].
 enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_EPOCH = 2, CTL_HDR = 8 };
 
@@ -387,7 +387,7 @@ struct StepArgs {
   // per-step scratch
   uint32_t* maskA; float* pred; uint32_t* msrc; int32_t* mn;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
-  uint32_t* ctl; uint32_t* sel; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
+  uint32_t* ctl; uint32_t* sel; uint32_t* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
   float scale; float pace_ns; double score_c;
@@ -741,7 +741,8 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
 // Ordered emission from the registers (see team_emit for the outputs).
 __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, int k, const Thr& t, const Team& tm,
                                               const TeamMem& m, int32_t* list, int width, uint32_t* mask_g,
-                                              int32_t* Mlist, int widthM, unsigned long long* tl) {
+                                              int32_t* Mlist, int widthM, uint32_t* early, uint32_t ep,
+                                              unsigned long long* tl) {
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
   const int nwd = (n + 31) >> 5, nw32 = tm.nt >> 5;
@@ -782,24 +783,32 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
   }
   tm.sync();
   if (tl && tm.tid == 0) tl[4] = gtime();
+  const uint32_t tot = dec[3];
+  if (Mlist) {
+    // The missed blocks first: the repair units wait for nothing else, so M is published (early)
+    // before A, the bitmask and the merge list are written.
+#pragma unroll
+    for (int e = 0; e < KB; ++e) {
+      const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
+      if (w < nwd && ((mwd[e] >> lane) & 1u)) Mlist[(m.offs[w] & 0xffffu) + __popc(mwd[e] & lt)] = i;
+    }
+#pragma unroll 1
+    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
+    if (early) {
+      tm.sync();
+      if (tm.tid == 0) st_release(early, ep);
+    }
+  }
 #pragma unroll
   for (int e = 0; e < KB; ++e) {
     const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
     if (w < nwd) {
-      const uint32_t off = m.offs[w];
-      if ((bal[e] >> lane) & 1u) {
-        list[(off >> 16) + __popc(bal[e] & lt)] = i;
-        if ((mwd[e] >> lane) & 1u) Mlist[(off & 0xffffu) + __popc(mwd[e] & lt)] = i;
-      }
+      if ((bal[e] >> lane) & 1u) list[(m.offs[w] >> 16) + __popc(bal[e] & lt)] = i;
       if (mask_g && lane == 0) mask_g[w] = bal[e];
     }
   }
-  const uint32_t tot = dec[3];
 #pragma unroll 1
   for (int j = (int)(tot >> 16) + tm.tid; j < width; j += tm.nt) list[j] = -1;
-  if (Mlist)
-#pragma unroll 1
-    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
   tm.sync();
   return tot;
 }
@@ -980,7 +989,8 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   int32_t* list = is_sel ? a.setA + (size_t)row * a.K : Pnext + (size_t)row * a.Bud;
   uint32_t* mask_g = is_sel ? a.maskA + (size_t)row * a.MBw : nullptr;
   int32_t* Mlist = is_sel ? a.setM + (size_t)row * a.K : nullptr;
-  const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K, tl)
+  const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K,
+                                            is_sel ? &a.sel[row] : nullptr, ep, tl)
                             : team_emit(ks, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
   if (!is_sel) return;
@@ -1015,7 +1025,10 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
     }
   }
   tm.sync();  // every thread's stores (A, M, merge list, counts) are ordered before the release
-  if (tm.tid == 0) st_release(&a.sel[row], ep);
+  if (tm.tid == 0) {
+    if (!fast) st_release(&a.sel[row], ep);  // (the fast path published M as soon as it was written)
+    st_release(&a.sel2[row], ep);
+  }
 }
 
 // a7 for one (sequence, query head, 32-channel slice of d): Eq. 6-8 over the listed partial states,
@@ -1383,7 +1396,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       const int bh = t / NQ, dq = t - bh * NQ;
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
-      wait_eq(&a.sel[row], ep, &ctl[CTL_ERR]);
+      wait_eq(&a.sel2[row], ep, &ctl[CTL_ERR]);  // the row's merge list is complete
       job_merge<D>(a, b, hq, dq, buf, ep);
     }
   }
@@ -1528,7 +1541,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.ctl = c->ctl; a.stats = c->stats;
   {
     const size_t rm = (size_t)c->maxB * c->Hkv;
-    a.sel = c->ctl + CTL_HDR; a.ufs = a.sel + rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
+    a.sel = c->ctl + CTL_HDR; a.sel2 = a.sel + rm; a.ufs = a.sel2 + rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
   } a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.Rmax = c->maxB * c->Hkv;
