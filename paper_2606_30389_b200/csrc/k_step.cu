@@ -1184,13 +1184,17 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
   asm volatile("griddepcontrol.wait;\n" ::: "memory");
   uint32_t* ctl = a.ctl;
-  const uint32_t ep = __ldcg(ctl + CTL_EPOCH) + 1u;  // this launch's epoch: the value every flag of the step takes
+  // The epoch and the prediction parity are loaded now and first USED after the warp's summary rows
+  // and queries are in flight (an in-order warp stalls at the first use of a pending load).
+  const uint32_t ep0 = __ldcg(ctl + CTL_EPOCH);
+  const int par_raw = __ldcg(a.parity);
   const int R = a.B * a.Hkv;
-  const int par = *a.parity & 1;
-  const int32_t* Pcur = par ? a.P1 : a.P0;
-  int32_t* Pnext = par ? a.P0 : a.P1;
+  uint32_t ep;  // this launch's epoch: the value every flag of the step takes
+  int par;
+  const int32_t* Pcur;
+  int32_t* Pnext;
   unsigned long long* tl = a.tl ? a.tl + ((size_t)blockIdx.x * W + warp) * 16 : nullptr;
-  if (tl && lane == 0) { tl[0] = gtime(); tl[12] = 0; tl[13] = 0; tl[14] = 0; tl[15] = 0; }
+  if (tl && lane == 0) { tl[0] = gtime(); tl[8] = 0; tl[9] = 0; tl[10] = 0; tl[11] = 0; tl[12] = 0; tl[13] = 0; tl[14] = 0; tl[15] = 0; }
 
   // Roles.  Team mode (J job CTAs at the end of the grid, one row job each): the job CTAs take no
   // score chunk (they stage P / the EMA state and then wait) and are ranked after every worker
@@ -1224,7 +1228,6 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   };
   auto unit_decode = [&](int unit) { unit_decode_a(unit); unit_decode_b(); };
   const bool prefetch = !job_cta && !job_warp && u < U;
-  if (prefetch) unit_decode_a(u);
 
   // ---- phase 1: scores.  The warp's first speculative tile goes in flight only once its summary
   // rows have LANDED: the 25 MB of tile traffic would otherwise queue in front of the 4 MB that
@@ -1245,10 +1248,12 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       }
       if (tl && lane == 0) tl[14] = gtime();
       if (ch * CR >= nb) continue;  // a chunk past the sequence's last block: nobody waits for it
-      signal_set(&a.sfl[(size_t)row * cpr + ch], ep);
+      signal_set(&a.sfl[(size_t)row * cpr + ch], ep0 + 1u);
       if (tl && lane == 0) tl[15] = gtime();
     }
-    if (prefetch) unit_decode_b();
+    ep = ep0 + 1u; par = par_raw & 1;
+    Pcur = par ? a.P1 : a.P0; Pnext = par ? a.P0 : a.P1;
+    if (prefetch) unit_decode(u);
     // No bulk tile traffic from this SM before all of its warps have published their scores: a
     // release waits for the SM's outstanding memory traffic.
     __syncthreads();
@@ -1265,6 +1270,10 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       pend = true;
       if (tl && lane == 0) tl[7] = gtime();
     }
+  }
+  if (job_cta) {
+    ep = ep0 + 1u; par = par_raw & 1;
+    Pcur = par ? a.P1 : a.P0; Pnext = par ? a.P0 : a.P1;
   }
   if (tl && lane == 0) tl[1] = gtime();
 
@@ -1347,6 +1356,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
             uslot = tr / R; urow = tr - uslot * R;
             tr += NWS;
             wait_eq(&a.sel[urow], ep, &ctl[CTL_ERR]);
+            if (tl && lane == 0 && tl[8] == 0) tl[8] = gtime();
             ublk = __ldcg(a.setM + (size_t)urow * a.K + uslot);
             if (ublk >= 0) break;
           }
@@ -1356,8 +1366,10 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
           ulen = seq_len(a, ub);
           uvalid = min(BS, ulen - ublk * BS);
           upage = __ldg(a.table + (size_t)ub * a.MB + ublk);
+          if (tl && lane == 0) tl[9] = gtime() + (unsigned long long)(upage & 0);
         }
         tile_load<D, BS>(Ks, bars, a, upage, uh);
+        if (tl && lane == 0 && urep) tl[10] = gtime();
       }
       const int crow = urow, cslot = uslot;
       const bool patch = a.app && uvalid > 0 && ublk == (ulen - 1) / BS;
@@ -1368,6 +1380,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
                           patch ? a.v_new + ((size_t)ub * a.Hkv + uh) * D : nullptr);
       ph ^= 1u;
       pend = false;
+      if (tl && lane == 0 && crep) tl[11] = gtime();
       if (!crep) {
         u += NWS;
         if (u < U) {  // refill the buffer before publishing: the next tile's latency starts now
