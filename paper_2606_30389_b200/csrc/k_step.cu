@@ -665,15 +665,18 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
     }
     __syncwarp();
   }
+  // Eight rows per trip and per sub-warp.  The 8 per-lane partial sums are folded across the LPR
+  // lanes by a transposed butterfly (each step halves what a lane carries), 7-8 64-bit shuffles
+  // instead of 8 x log2(LPR); every partial sum is exact (Q1), so the order of accumulation is free.
 #pragma unroll 1
-  for (int rr0 = 0; rr0 < nr; rr0 += 4 * RW) {  // warp-uniform trip count (full-mask shuffles below)
-    double acc[4];
+  for (int rr0 = 0; rr0 < nr; rr0 += 8 * RW) {  // warp-uniform trip count (full-mask shuffles below)
+    double acc[8];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
+    for (int e = 0; e < 8; ++e) {
       const int r = rr0 + e * RW + sub;
       const uint4 v = r < nr ? st[r * LPR] : make_uint4(0, 0, 0, 0);
       const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-      double a0 = 0.0, a1 = 0.0;  // every partial sum is exact (Q1), so the order of accumulation is free
+      double a0 = 0.0, a1 = 0.0;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
@@ -681,15 +684,18 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
       }
       acc[e] = a0 + a1;
     }
+    const bool upA = (l & (LPR / 2)) != 0, upB = (l & (LPR / 4)) != 0, upC = (l & (LPR / 8)) != 0;
+    double v4[4], v2[2];
 #pragma unroll
-    for (int off = LPR / 2; off >= 1; off >>= 1)
+    for (int j = 0; j < 4; ++j)
+      v4[j] = (upA ? acc[4 + j] : acc[j]) + __shfl_xor_sync(FULL, upA ? acc[j] : acc[4 + j], LPR / 2);
 #pragma unroll
-      for (int e = 0; e < 4; ++e) acc[e] += __shfl_xor_sync(FULL, acc[e], off);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const int r = rr0 + e * RW + sub;
-      if (l == 0 && r < nr) out[r] = f64_to_score(__dmul_rn(acc[e], a.score_c));
-    }
+    for (int j = 0; j < 2; ++j)
+      v2[j] = (upB ? v4[2 + j] : v4[j]) + __shfl_xor_sync(FULL, upB ? v4[j] : v4[2 + j], LPR / 4);
+    double v1 = (upC ? v2[1] : v2[0]) + __shfl_xor_sync(FULL, upC ? v2[0] : v2[1], LPR / 8);
+    if (LPR == 16) v1 += __shfl_xor_sync(FULL, v1, 1);
+    const int r = rr0 + ((upA ? 4 : 0) + (upB ? 2 : 0) + (upC ? 1 : 0)) * RW + sub;
+    if (r < nr && (LPR == 8 || (l & 1) == 0)) out[r] = f64_to_score(__dmul_rn(v1, a.score_c));
   }
   __syncwarp();
   return nb;
