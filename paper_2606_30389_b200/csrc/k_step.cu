@@ -59,6 +59,14 @@ __device__ __forceinline__ unsigned long long gtime() {
   return t;
 }
 
+__device__ __forceinline__ unsigned long long ld_relaxed64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];\n" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_relaxed64(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;\n" ::"l"(p), "l"(v) : "memory");
+}
 __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
 }
@@ -386,6 +394,9 @@ struct StepArgs {
   int32_t* setA; int32_t* setM; int32_t* counts;
   // per-step scratch
   uint32_t* maskA; float* pred; uint32_t* msrc; int32_t* mn;
+  // M as self-describing words, one per (row, repair slot): epoch << 32 | block + 1 (0 = no such miss).  A
+  // repair warp polls ITS word: no flag, no fence and no second load between selection and the tile request.
+  unsigned long long* mtag;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
   uint32_t* ctl; uint32_t* sel; uint32_t* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
@@ -747,7 +758,7 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
 // Ordered emission from the registers (see team_emit for the outputs).
 __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, int k, const Thr& t, const Team& tm,
                                               const TeamMem& m, int32_t* list, int width, uint32_t* mask_g,
-                                              int32_t* Mlist, int widthM, uint32_t* early, uint32_t ep,
+                                              int32_t* Mlist, int widthM, unsigned long long* mtag, uint32_t ep,
                                               unsigned long long* tl) {
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
@@ -796,13 +807,16 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
 #pragma unroll
     for (int e = 0; e < KB; ++e) {
       const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
-      if (w < nwd && ((mwd[e] >> lane) & 1u)) Mlist[(m.offs[w] & 0xffffu) + __popc(mwd[e] & lt)] = i;
+      if (w < nwd && ((mwd[e] >> lane) & 1u)) {
+        const int pos = (int)(m.offs[w] & 0xffffu) + __popc(mwd[e] & lt);
+        st_relaxed64(mtag + pos, ((unsigned long long)ep << 32) | (uint32_t)(i + 1));
+        Mlist[pos] = i;
+      }
     }
 #pragma unroll 1
-    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
-    if (early) {
-      tm.sync();
-      if (tm.tid == 0) st_release(early, ep);
+    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) {
+      st_relaxed64(mtag + j, (unsigned long long)ep << 32);
+      Mlist[j] = -1;
     }
   }
 #pragma unroll
@@ -996,10 +1010,17 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   uint32_t* mask_g = is_sel ? a.maskA + (size_t)row * a.MBw : nullptr;
   int32_t* Mlist = is_sel ? a.setM + (size_t)row * a.K : nullptr;
   const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K,
-                                            is_sel ? &a.sel[row] : nullptr, ep, tl)
+                                            is_sel ? a.mtag + (size_t)row * a.K : nullptr, ep, tl)
                             : team_emit(ks, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
   if (!is_sel) return;
+  if (!fast) {  // generic path: the tagged words from the list just written (team_emit ended with a barrier)
+    const int nMg = (int)(tot & 0xffffu);
+    for (int j = tm.tid; j < a.K; j += tm.nt) {
+      const int blk = j < nMg ? __ldcg(Mlist + j) : -1;
+      st_relaxed64(a.mtag + (size_t)row * a.K + j, ((unsigned long long)ep << 32) | (uint32_t)(blk + 1));
+    }
+  }
   // ---- publish (select only) ----
   const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
   if (tm.wid == 0) {  // the row's merge list: hit slots (all of P when retained) ascending, then the repair slots
@@ -1032,7 +1053,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   }
   tm.sync();  // every thread's stores (A, M, merge list, counts) are ordered before the release
   if (tm.tid == 0) {
-    if (!fast) st_release(&a.sel[row], ep);  // (the fast path published M as soon as it was written)
+    st_release(&a.sel[row], ep);
     st_release(&a.sel2[row], ep);
   }
 }
@@ -1361,9 +1382,17 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
             if (tr >= NT) { finished = true; break; }
             uslot = tr / R; urow = tr - uslot * R;
             tr += NWS;
-            wait_eq(&a.sel[urow], ep, &ctl[CTL_ERR]);
+            unsigned long long w = 0ull;
+            if (lane == 0) {  // the ticket's own word: tag = this launch's epoch once select(row) knows M
+              const unsigned long long* mp = a.mtag + (size_t)urow * a.K + uslot;
+              uint32_t it = 0;
+              while ((uint32_t)((w = ld_relaxed64(mp)) >> 32) != ep) {
+                __nanosleep(20);
+                if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); w = (unsigned long long)ep << 32; break; }
+              }
+            }
+            ublk = (int)__shfl_sync(FULL, (uint32_t)w, 0) - 1;
             if (tl && lane == 0 && tl[8] == 0) tl[8] = gtime();
-            ublk = __ldcg(a.setM + (size_t)urow * a.K + uslot);
             if (ublk >= 0) break;
           }
           if (finished) break;
@@ -1554,7 +1583,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.theta = c->theta + (size_t)kv->layer * c->maxB * 3;
   a.P0 = c->Pbuf[0] + r * c->Bud; a.P1 = c->Pbuf[1] + r * c->Bud; a.parity = c->parity + kv->layer;
   a.setA = c->setA + r * c->K; a.setM = c->setM + r * c->K; a.counts = c->counts + r * 3;
-  a.maskA = c->maskA; a.pred = c->pred; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
+  a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
   a.ctl = c->ctl; a.stats = c->stats;
