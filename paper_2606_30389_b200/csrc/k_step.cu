@@ -755,11 +755,31 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
   return team_rank(cstar, need, tm, m);
 }
 
+// The row's merge list (warp 0 of the team): hit slots (all of P when retained) ascending, then the
+// repair slots; needs the bitmask of A in m.amask and the predicted blocks by slot in m.plist.
+__device__ __forceinline__ void write_merge_list(const StepArgs& a, int row, int nb, int nM, const TeamMem& m) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* ms = a.msrc + (size_t)row * (a.Bud + a.K);
+  int base = 0;
+  if (a.spec) {
+    for (int j0 = 0; j0 < a.Bud; j0 += 32) {
+      const int j = j0 + lane;
+      const int blk = j < a.Bud ? m.plist[j] : -1;
+      const bool use = blk >= 0 && (a.retain || ((blk >> 5) < ((nb + 31) >> 5) && ((m.amask[blk >> 5] >> (blk & 31)) & 1u)));
+      const uint32_t bal = __ballot_sync(FULL, use);
+      if (use) ms[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)j;
+      base += __popc(bal);
+    }
+  }
+  for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
+  if (lane == 0) a.mn[row] = (base << 16) | (base + nM);  // speculative entries | all entries
+}
+
 // Ordered emission from the registers (see team_emit for the outputs).
 __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, int k, const Thr& t, const Team& tm,
                                               const TeamMem& m, int32_t* list, int width, uint32_t* mask_g,
                                               int32_t* Mlist, int widthM, unsigned long long* mtag, uint32_t ep,
-                                              unsigned long long* tl) {
+                                              const StepArgs& a, int row, int nb, unsigned long long* tl) {
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
   const int nwd = (n + 31) >> 5, nw32 = tm.nt >> 5;
@@ -818,6 +838,11 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
       st_relaxed64(mtag + j, (unsigned long long)ep << 32);
       Mlist[j] = -1;
     }
+    // ... then the merge list, published before A, the bitmask and the counters are written: the
+    // merge of the speculative entries can start while the repairs are in flight
+    if (tm.wid == 0) write_merge_list(a, row, nb, (int)(tot & 0xffffu), m);
+    tm.sync();
+    if (tm.tid == 0) st_release(&a.sel2[row], ep);
   }
 #pragma unroll
   for (int e = 0; e < KB; ++e) {
@@ -1010,7 +1035,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   uint32_t* mask_g = is_sel ? a.maskA + (size_t)row * a.MBw : nullptr;
   int32_t* Mlist = is_sel ? a.setM + (size_t)row * a.K : nullptr;
   const uint32_t tot = fast ? fast_emit(kreg, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K,
-                                            is_sel ? a.mtag + (size_t)row * a.K : nullptr, ep, tl)
+                                            is_sel ? a.mtag + (size_t)row * a.K : nullptr, ep, a, row, nb, tl)
                             : team_emit(ks, n, k, t, tm, m, list, is_sel ? a.K : a.Bud, mask_g, Mlist, a.K);
   if (tl && tm.tid == 0) tl[11] = gtime();
   if (!is_sel) return;
@@ -1023,23 +1048,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   }
   // ---- publish (select only) ----
   const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
-  if (tm.wid == 0) {  // the row's merge list: hit slots (all of P when retained) ascending, then the repair slots
-    const int lane = threadIdx.x & 31;
-    uint32_t* ms = a.msrc + (size_t)row * (a.Bud + a.K);
-    int base = 0;
-    if (a.spec) {
-      for (int j0 = 0; j0 < a.Bud; j0 += 32) {
-        const int j = j0 + lane;
-        const int blk = j < a.Bud ? m.plist[j] : -1;
-        const bool use = blk >= 0 && (a.retain || ((blk >> 5) < ((nb + 31) >> 5) && ((m.amask[blk >> 5] >> (blk & 31)) & 1u)));
-        const uint32_t bal = __ballot_sync(FULL, use);
-        if (use) ms[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)j;
-        base += __popc(bal);
-      }
-    }
-    for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
-    if (lane == 0) a.mn[row] = (base << 16) | (base + nM);  // speculative entries | all entries
-  }
+  if (!fast && tm.wid == 0) write_merge_list(a, row, nb, nM, m);  // (the fast path wrote and published it already)
   if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
     a.counts[row * 3 + 1] = np;
@@ -1054,7 +1063,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   tm.sync();  // every thread's stores (A, M, merge list, counts) are ordered before the release
   if (tm.tid == 0) {
     st_release(&a.sel[row], ep);
-    st_release(&a.sel2[row], ep);
+    if (!fast) st_release(&a.sel2[row], ep);
   }
 }
 
@@ -1065,7 +1074,8 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
 template <int D>
-__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep) {
+__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep,
+                          unsigned long long* tl) {
   constexpr uint32_t REP = 0x80000000u;
   const int lane = threadIdx.x & 31;
   const int h = hq / a.G, row = b * a.Hkv + h;
@@ -1116,6 +1126,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
           if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
         }
       }
+      if (tl && lane == 0) tl[13 + seg] = gtime();
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const uint32_t j = code[u] & ~REP;
@@ -1430,14 +1441,15 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
 
   // ---- phase 5: merge, claimed by whoever is free ------------------------------------------------
   {
-    // merge items are dealt out statically: one per job-CTA warp; what is left over goes to the
-    // worker warps from the top (the repair tickets went to the lowest-numbered ones)
+    // merge items are dealt out statically to the worker warps from the top (the repair tickets went
+    // to the lowest-numbered ones): they have been idle since their speculative unit, while the job
+    // CTAs' warps only come free when their row job ends.  What is left over goes to the job CTAs.
     const int NT = a.B * a.Hq * NQ;
     const int njw = a.J * W;
     int t0 = gw, tstep = NW;
     if (a.J) {
-      if (job_cta) { t0 = ((int)blockIdx.x - NWK) * W + warp; tstep = NT; }
-      else { t0 = njw + (NWS - 1 - gw); tstep = NWS; }
+      if (job_cta) { t0 = NWS + ((int)blockIdx.x - NWK) * W + warp; tstep = njw; }
+      else { t0 = NWS - 1 - gw; tstep = NT; }
     }
 #pragma unroll 1
     for (int t = t0; t < NT; t += tstep) {
@@ -1445,7 +1457,8 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
       wait_eq(&a.sel2[row], ep, &ctl[CTL_ERR]);  // the row's merge list is complete
-      job_merge<D>(a, b, hq, dq, buf, ep);
+      if (tl && lane == 0) tl[12] = gtime();
+      job_merge<D>(a, b, hq, dq, buf, ep, tl);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
