@@ -23,10 +23,10 @@ TB128 = synth.Config("TB128", B=1, L=1, Hq=16, Hkv=1, d=64, ctx_lo=2000, ctx_hi=
 SHAPES = [TINY, T128, T16, TB128]
 
 
-def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None):
+def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None, orchestration=prr.FUSED):
     cfg = cfg if seed is None else cfg.scaled(seed=seed)
     inp = synth.make_layer(cfg, 0, device=DEV, steps=steps)
-    gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget)
+    gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget, orchestration=orchestration)
     ol = H.oracle_layer(cfg, inp, policy=policy, budget=budget)
     return cfg, inp, gl, ol
 
@@ -239,9 +239,9 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
 
 
 def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True,
-               fused_append=False):
+               fused_append=False, orchestration=prr.FUSED):
     steps = cfg.steps if steps is None else steps
-    cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps)
+    cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps, orchestration=orchestration)
     twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget) if seq_check else None
     if calibrate:
         gres = gl.calibrate(inp.q_cal)
@@ -304,6 +304,30 @@ def test_step_append_block_boundary_and_full_size():
     run_decode(T16.scaled(ctx_lo=16 * 5, ctx_hi=16 * 5), steps=20, fused_append=True)   # starts on a boundary
     run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=4, fused_append=True)
     run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=2, seq_check=False, fused_append=True)
+
+
+def test_streams_orchestration_whole_steps():
+    """PRR_STREAMS: the paper's literal two-stream, event-ordered orchestration of the stage kernels
+    (Fig. 1 / Fig. 5), same oracle, same tolerances; prr_step_append falls back to two calls."""
+    run_decode(TINY, orchestration=prr.STREAMS)
+    run_decode(T128, policy=prr.RETAIN, orchestration=prr.STREAMS, fused_append=True)
+
+
+def test_timeline_and_check():
+    """prr_timeline_*: every warp of the fused step stamps its phase boundaries; prr_check is clean."""
+    cfg, inp, gl, ol = make(TINY)
+    gl.calibrate(inp.q_cal)
+    gl.ctx.timeline_enable(True)
+    gl.step_append(0)
+    torch.cuda.synchronize()
+    tl = gl.ctx.timeline_read().astype(np.int64)
+    gl.ctx.timeline_enable(False)
+    assert tl.ndim == 2 and tl.shape[1] == 16 and tl.shape[0] >= 148
+    live = tl[tl[:, 0] > 0]
+    assert len(live) >= 148                                   # one CTA per SM, several warps each
+    assert (live[:, 5] >= live[:, 0]).all()                   # merge-done stamp after the start stamp
+    assert (live[:, 5] - live[:, 0]).max() < 5_000_000        # a step takes microseconds, not milliseconds
+    gl.ctx.check()
 
 
 def test_decode_c0_full():
