@@ -676,27 +676,28 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
     }
     __syncwarp();
   }
-  // Eight rows per trip and per sub-warp.  The 8 per-lane partial sums are folded across the LPR
-  // lanes by a transposed butterfly (each step halves what a lane carries), 7-8 64-bit shuffles
-  // instead of 8 x log2(LPR); every partial sum is exact (Q1), so the order of accumulation is free.
-#pragma unroll 1
-  for (int rr0 = 0; rr0 < nr; rr0 += 8 * RW) {  // warp-uniform trip count (full-mask shuffles below)
-    double acc[8];
+  // Eight rows per trip and per sub-warp (four in a short last trip).  The per-lane partial sums are
+  // folded across the LPR lanes by a transposed butterfly (each step halves what a lane carries): 7-8
+  // 64-bit shuffles instead of 8 x log2(LPR).  Every partial sum is exact (Q1), so the order of
+  // accumulation is free.
+  auto dot = [&](int r) -> double {
+    const uint4 v = r < nr ? st[r * LPR] : make_uint4(0, 0, 0, 0);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    double a0 = 0.0, a1 = 0.0;
 #pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const int r = rr0 + e * RW + sub;
-      const uint4 v = r < nr ? st[r * LPR] : make_uint4(0, 0, 0, 0);
-      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-      double a0 = 0.0, a1 = 0.0;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
-        a1 = fma((double)bf16_hi(w[j]), qs[2 * j + 1], a1);
-      }
-      acc[e] = a0 + a1;
+    for (int j = 0; j < 4; ++j) {
+      a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
+      a1 = fma((double)bf16_hi(w[j]), qs[2 * j + 1], a1);
     }
-    const bool upA = (l & (LPR / 2)) != 0, upB = (l & (LPR / 4)) != 0, upC = (l & (LPR / 8)) != 0;
-    double v4[4], v2[2];
+    return a0 + a1;
+  };
+  const bool upA = (l & (LPR / 2)) != 0, upB = (l & (LPR / 4)) != 0, upC = (l & (LPR / 8)) != 0;
+  int rr0 = 0;
+#pragma unroll 1
+  for (; nr - rr0 > 4 * RW; rr0 += 8 * RW) {  // warp-uniform trip counts (full-mask shuffles below)
+    double acc[8], v4[4], v2[2];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc[e] = dot(rr0 + e * RW + sub);
 #pragma unroll
     for (int j = 0; j < 4; ++j)
       v4[j] = (upA ? acc[4 + j] : acc[j]) + __shfl_xor_sync(FULL, upA ? acc[j] : acc[4 + j], LPR / 2);
@@ -707,6 +708,19 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
     if (LPR == 16) v1 += __shfl_xor_sync(FULL, v1, 1);
     const int r = rr0 + ((upA ? 4 : 0) + (upB ? 2 : 0) + (upC ? 1 : 0)) * RW + sub;
     if (r < nr && (LPR == 8 || (l & 1) == 0)) out[r] = f64_to_score(__dmul_rn(v1, a.score_c));
+  }
+  if (rr0 < nr) {  // at most 4 * RW rows left
+    double acc[4], v2[2];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) acc[e] = dot(rr0 + e * RW + sub);
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+      v2[j] = (upA ? acc[2 + j] : acc[j]) + __shfl_xor_sync(FULL, upA ? acc[j] : acc[2 + j], LPR / 2);
+    double v1 = (upB ? v2[1] : v2[0]) + __shfl_xor_sync(FULL, upB ? v2[0] : v2[1], LPR / 4);
+#pragma unroll
+    for (int off = LPR / 8; off >= 1; off >>= 1) v1 += __shfl_xor_sync(FULL, v1, off);
+    const int r = rr0 + ((upA ? 2 : 0) + (upB ? 1 : 0)) * RW + sub;
+    if (r < nr && (l & (LPR / 4 - 1)) == 0) out[r] = f64_to_score(__dmul_rn(v1, a.score_c));
   }
   __syncwarp();
   return nb;
