@@ -212,7 +212,9 @@ int64_t prr_launch_count(const prr_ctx* ctx);
 /* Profiling aid for the fused step (a9, Fig. 5 timeline).  While enabled, every warp of a
  * fused step launched (or captured) afterwards stores %globaltimer (ns) at its phase boundaries:
  * [0] start, [1] scores done, [2] row job done, [3] speculative units done, [4] repair units done,
- * [5] merge done; words 6-15 are finer marks inside the prologue and the row jobs.  prr_timeline_read copies the stamps of the LAST step,
+ * [5] merge done; words 6-15 are finer marks (score chunk: [6] queries summed, [13] rows landed, [14] computed,
+ * [15] published; row jobs: [8] scores seen, [9] keys, [12] histogram, [13] bucket, [14] candidates, [10] K-th,
+ * [11] emitted; repair units: [8] M seen, [10] tile requested, [11] computed; merge: [12]-[14]).  prr_timeline_read copies the stamps of the LAST step,
  * uint64 [n_warps, 16] with warp index = cta * warps_per_cta + warp, to HOST memory and
  * synchronises `stream`; n_warps_out (host, may be NULL) receives the rows copied (<= max_warps). */
 int32_t prr_timeline_enable(prr_ctx* ctx, int32_t on);

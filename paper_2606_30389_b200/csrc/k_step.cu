@@ -1,30 +1,35 @@
-// k_step — one PRR layer-step (a1-a8) as ONE persistent launch (Fig. 1, :38-42, :115 Fig. 5).
+// k_step — one PRR layer-step (a0-a8) as ONE persistent launch (Fig. 1, :38-42, :115 Fig. 5).
 //
 // The paper overlaps speculative attention with selection on two streams; on B200 a layer-step at
-// batch 1 moves ~30 MB, i.e. ~5 us of HBM time, so kernel boundaries (2 us each) are the cost that
-// matters.  Here the whole step is one grid of #SM CTAs whose WARPS are the workers: each warp owns
-// a private shared-memory tile buffer (K and V tile of one block, padded for ldmatrix) and walks
-// through the phases below.  Dependencies between warps are device-scope counters (release: data
-// stores, __threadfence, atomic; acquire: ld.acquire poll, then L2 (.cg) loads).  Every wait
-// targets an EARLIER phase of other warps, all CTAs are co-resident (cooperative launch), so the
-// schedule cannot deadlock; waits are bounded anyway and raise ctl[CTL_ERR].
+// batch 1 moves ~30 MB, i.e. ~5 us of HBM time, so kernel boundaries and launch gaps (2-3 us each)
+// are the cost that matters.  Here the whole step is one grid of #SM CTAs whose WARPS are the
+// workers: each warp owns a shared-memory tile buffer (K and V tile of one block, filled by TMA in
+// the 128-byte swizzle) and walks through the phases below.  Dependencies between warps are
+// epoch-valued flags in global memory (producer: stores, warp/CTA barrier, one st.release of the
+// launch's epoch; consumer: ld.acquire polls of exactly the flags it needs, whole warps leaving on a
+// vote).  Every wait targets an EARLIER phase of other warps and all CTAs are co-resident
+// (cooperative launch), so the schedule cannot deadlock; waits are bounded anyway and raise
+// ctl[CTL_ERR] (prr_check).  DESIGN.md section 8 has the measured timeline and what shaped it.
 //
-//   phase 1  score chunks (a1): the 16-byte loads of the summary rows are issued FIRST (they head
-//            the critical path), then the warp's first speculative tile is put in flight
-//            (cp.async), then the chunk is finished: exact fp64 accumulation (Q1)
-//   phase 2  row jobs.  When rows are few (2R <= #SM/4) a whole CTA is the team of one job: its
-//            threads hold the row's keys in shared memory and find the exact k-th key by range
-//            narrowing with private counters; otherwise one warp per job does the same.
-//              select(row): wait for the row's scores -> A ascending + bitmask (a2), diff against
-//                           P (a5) -> M list, publish
-//              ema(row):    wait for the row's scores -> Eq. 3 update, Eq. 2 prediction, top-Bud
-//                           -> P of the NEXT step into the other parity buffer (a8, a3)
-//   phase 3  speculative units (a4): per-block partial state (m, l, O) of every block of P
-//   phase 4  repair units (a6), claimed dynamically by whichever warp is free: ticket -> (row,
-//            slot), wait for select(row), same partial-state code over M = A\P
-//   phase 5  merge items (a7), claimed dynamically: wait for the row's units, fold hits u M (DROP)
-//            or P u M (RETAIN) by Eq. 6-8 with one division at the end
-//   exit     last warp resets the counters and flips the layer's P parity
+//   worker CTAs
+//     phase 1  a0 + a1: one chunk of summary rows per warp, copied with cp.async into the warp's idle
+//              tile buffer; exact fp64 accumulation (Q1); the warp whose chunk holds the open block
+//              appends the new token (cache slot, fp64 running sum, summary row) and patches the
+//              staged row; one flag per chunk.  No tile is requested before the SM has published.
+//     phase 3  a4: the warp's speculative units, per-block partial state (m, l, O) of the blocks of P
+//              (first wave paced at the HBM rate so the critical-path accesses are not queued behind it)
+//     phase 4  a6: repair units, dealt out statically as (row, slot) tickets; the ticket's warp polls
+//              its own epoch-tagged word of M and runs the same tile code
+//     phase 5  a7: merge items (query head x 32-channel slice), dealt to the idle worker warps: wait
+//              for the row's merge list, then for exactly the units in it; fold hits u M (DROP) or
+//              P u M (RETAIN) by Eq. 6-8, speculative entries first, one division at the end
+//   job CTAs (one row job each when 2R <= #SM/4; otherwise the highest-numbered warps take the jobs)
+//     phase 2  select(row): P as a bitmask, wait for the row's chunk flags, exact top-K on order-
+//                           preserving keys in registers (a2), M = A\P (a5) published first, then
+//                           the merge list, then A / bitmask / counters
+//              ema(row):    (l, v) staged in shared memory meanwhile; Eq. 3 update, Eq. 2 prediction,
+//                           top-Bud -> P of the NEXT step into the other parity buffer (a8, a3)
+//   exit       the last warp bumps the epoch, flips the layer's P parity and (fused append) seq_lens
 //
 // spec = 0 runs the same kernel as the sequential select-then-attend path: P is
 // treated as empty, every block of A is a "repair" unit that can only start after selection.
@@ -44,8 +49,8 @@ constexpr uint32_t SPIN_LIMIT = 1u << 22;  // ~0.1-0.5 s of polling, then give u
 
 // Dependencies between warps are epoch-valued FLAGS, not counters: a producer publishes with one
 // st.release of the launch's epoch (no atomics, nothing to reset), a consumer polls exactly the
-// flags of the items it needs.  ctl = header, then sel[Rmax] (M published), sel2[Rmax] (merge list published), spec-unit flags [Rmax*Bud], repair-
-// unit flags [Rmax*K], score-chunk flags [Rmax*MB].
+// flags of the items it needs.  ctl = header, then sel[Rmax] (A, M, counters written), sel2[Rmax] (merge
+// list written), spec-unit flags [Rmax*Bud], repair-unit flags [Rmax*K], score-chunk flags [Rmax*MB].
 enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_EPOCH = 2, CTL_HDR = 8 };
 
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
