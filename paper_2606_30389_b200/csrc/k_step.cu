@@ -816,10 +816,27 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
         m.amask[w] = bal[e];
         m.offs[w] = ((uint32_t)__popc(bal[e]) << 16) | (uint32_t)__popc(mwd[e]);
       }
+      // A missed block goes out the moment it is known, in ANY repair slot (a shared-memory ticket):
+      // the repair units and the merge do not care about the order, and the ordered lists (A and M
+      // as the API reports them) are written later, off the critical path.
+      if ((mwd[e] >> lane) & 1u) {
+        const uint32_t pos = atomicAdd(&dec[8], 1u);
+        st_relaxed64(mtag + pos, ((unsigned long long)ep << 32) | (uint32_t)(i + 1));
+      }
     }
   }
   tm.sync();
   if (tl && tm.tid == 0) tl[3] = gtime();
+  if (Mlist) {
+    const int nMq = (int)dec[8];
+#pragma unroll 1
+    for (int j = nMq + tm.tid; j < widthM; j += tm.nt) st_relaxed64(mtag + j, (unsigned long long)ep << 32);  // void tickets
+    // the merge list, published before the ordered lists are written: the merge of the speculative
+    // entries can start while the repairs are in flight
+    if (tm.wid == 0) write_merge_list(a, row, nb, nMq, m);
+    tm.sync();
+    if (tm.tid == 0) st_release(&a.sel2[row], ep);
+  }
   if (tm.wid == 0) {  // exclusive scan of the per-word counts, in block order
     uint32_t carry = 0;
 #pragma unroll 1
@@ -840,39 +857,21 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
   tm.sync();
   if (tl && tm.tid == 0) tl[4] = gtime();
   const uint32_t tot = dec[3];
-  if (Mlist) {
-    // The missed blocks first: the repair units wait for nothing else, so M is published (early)
-    // before A, the bitmask and the merge list are written.
-#pragma unroll
-    for (int e = 0; e < KB; ++e) {
-      const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
-      if (w < nwd && ((mwd[e] >> lane) & 1u)) {
-        const int pos = (int)(m.offs[w] & 0xffffu) + __popc(mwd[e] & lt);
-        st_relaxed64(mtag + pos, ((unsigned long long)ep << 32) | (uint32_t)(i + 1));
-        Mlist[pos] = i;
-      }
-    }
-#pragma unroll 1
-    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) {
-      st_relaxed64(mtag + j, (unsigned long long)ep << 32);
-      Mlist[j] = -1;
-    }
-    // ... then the merge list, published before A, the bitmask and the counters are written: the
-    // merge of the speculative entries can start while the repairs are in flight
-    if (tm.wid == 0) write_merge_list(a, row, nb, (int)(tot & 0xffffu), m);
-    tm.sync();
-    if (tm.tid == 0) st_release(&a.sel2[row], ep);
-  }
 #pragma unroll
   for (int e = 0; e < KB; ++e) {
     const int i = tm.tid + e * tm.nt, w = tm.wid + e * nw32;
     if (w < nwd) {
-      if ((bal[e] >> lane) & 1u) list[(m.offs[w] >> 16) + __popc(bal[e] & lt)] = i;
+      const uint32_t off = m.offs[w];
+      if ((bal[e] >> lane) & 1u) list[(off >> 16) + __popc(bal[e] & lt)] = i;
+      if ((mwd[e] >> lane) & 1u) Mlist[(off & 0xffffu) + __popc(mwd[e] & lt)] = i;
       if (mask_g && lane == 0) mask_g[w] = bal[e];
     }
   }
 #pragma unroll 1
   for (int j = (int)(tot >> 16) + tm.tid; j < width; j += tm.nt) list[j] = -1;
+  if (Mlist)
+#pragma unroll 1
+    for (int j = (int)(tot & 0xffffu) + tm.tid; j < widthM; j += tm.nt) Mlist[j] = -1;
   tm.sync();
   return tot;
 }
@@ -905,7 +904,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   if (is_sel) {
 #pragma unroll 1
     for (int w = tm.tid; w < a.MBw; w += tm.nt) m.pmask[w] = 0u;
-    if (tm.tid == 0) dec[4] = 0u;
+    if (tm.tid == 0) { dec[4] = 0u; dec[8] = 0u; }
     tm.sync();
     if (a.spec) {
       const int32_t* P = Pcur + (size_t)row * a.Bud;
@@ -1352,7 +1351,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
     m.pmask = p; p += a.MBw;
     m.amask = p; p += a.MBw;
     m.offs = p; p += a.MBw;
-    m.red = p; p += tm.nw * 16 + 8;
+    m.red = p; p += tm.nw * 16 + 16;
     m.hist = p; p += 1 << m.hbits;
 #pragma unroll 1
     for (int i = tm.tid; i < (1 << m.hbits); i += tm.nt) m.hist[i] = 0u;
@@ -1514,12 +1513,12 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   a.J = 2 * R <= c->n_sm / 4 ? 2 * R : 0;
   int W = 0, per_warp = 0;
   for (;;) {
-    a.scr_bytes = (3 * a.MBw + 24 + 3 * CAND + 2 + (a.J ? 0 : 256 + c->Bud)) * 4;
+    a.scr_bytes = (3 * a.MBw + 32 + 3 * CAND + 2 + (a.J ? 0 : 256 + c->Bud)) * 4;
     a.scr_bytes += (1024 - (a.buf_bytes + a.scr_bytes) % 1024) % 1024;  // tile buffers stay 1024-byte aligned (swizzle atom)
     per_warp = a.buf_bytes + a.scr_bytes;
     W = std::min(T::WMAX, (c->smem_optin - 1024) / per_warp);
     if (W < 1) return cudaErrorInvalidConfiguration;
-    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 8 + 2048 + 3 * CAND + 2 + 64 + c->Bud;
+    const size_t team_words = (size_t)3 * a.MBw + W * 16 + 16 + 2048 + 3 * CAND + 2 + 64 + c->Bud;
     if (a.J && team_words * 4 > (size_t)W * per_warp) { a.J = 0; continue; }
     break;
   }
