@@ -20,7 +20,7 @@
 //              (first wave paced at the HBM rate so the critical-path accesses are not queued behind it)
 //     phase 4  a6: repair units, dealt out statically as (row, slot) tickets; the ticket's warp polls
 //              its own epoch-tagged word of M and runs the same tile code
-//     phase 5  a7: merge items (query head x 32-channel slice), dealt to the idle worker warps: wait
+//     phase 5  a7: merge items (query head x 16-channel slice), dealt to the idle worker warps: wait
 //              for the row's merge list, then for exactly the units in it; fold hits u M (DROP) or
 //              P u M (RETAIN) by Eq. 6-8, speculative entries first, one division at the end
 //   job CTAs (one row job each when 2R <= #SM/4; otherwise the highest-numbered warps take the jobs)
@@ -1085,10 +1085,10 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   }
 }
 
-// a7 for one (sequence, query head, 32-channel slice of d): Eq. 6-8 over the listed partial states,
-// O unnormalised and one division at the end.  The warp is 4 groups of 8 lanes; a group owns every
-// 4th entry and its lanes one float4 of the 128-byte slice, so a pass has 4 x unroll entries in
-// flight; the groups are folded with two shuffles.  Entry order is fixed (speculative slots
+// a7 for one (sequence, query head, 16-channel slice of d): Eq. 6-8 over the listed partial states,
+// O unnormalised and one division at the end.  The warp is 8 groups of 4 lanes; a group owns every
+// 8th entry and its lanes one float4 of the 64-byte slice, so a pass has 80 entries in flight (the
+// whole speculative segment of a row in one round trip); the groups are folded with three shuffles.  Entry order is fixed (speculative slots
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
 template <int D>
@@ -1106,9 +1106,9 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   const uint32_t pk = (uint32_t)__ldcg(a.mn + row);
   const int n = (int)(pk & 0xffffu), nh = (int)(pk >> 16);
   const uint32_t* ms = a.msrc + (size_t)row * E;
-  const int grp = lane >> 3, l8 = lane & 7;
-  const float* Os = a.O_spec + hb * a.Bud * D + dq * 32 + l8 * 4;
-  const float* Or = a.O_rep + hb * a.K * D + dq * 32 + l8 * 4;
+  const int grp = lane >> 2, l8 = lane & 3;  // 8 entry groups x 4 lanes x float4 = a 16-channel slice
+  const float* Os = a.O_spec + hb * a.Bud * D + dq * 16 + l8 * 4;
+  const float* Or = a.O_rep + hb * a.K * D + dq * 16 + l8 * 4;
   // Two segments folded by Eq. 6-8: first the speculative entries (their units finished while
   // selection ran), then the repaired ones -- so only the few repair rows are left to fetch once
   // the last repair unit has published.
@@ -1176,12 +1176,12 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     __syncwarp();
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-    for (int e0 = s0 + grp; e0 < s1; e0 += 4 * 10) {  // 10 rows per lane (40 entries per warp) in flight
+    for (int e0 = s0 + grp; e0 < s1; e0 += 8 * 10) {  // 10 rows per lane (80 entries per warp) in flight
       float4 x[10];
       float w[10];
 #pragma unroll
       for (int u = 0; u < 10; ++u) {
-        const int e = e0 + 4 * u;
+        const int e = e0 + 8 * u;
         const bool on = e < s1;
         const uint32_t code = on ? cs[e] : 0u;
         w[u] = on ? ws[e] : 0.f;
@@ -1204,7 +1204,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     mrun = mnew;
   }
 #pragma unroll
-  for (int off = 8; off <= 16; off <<= 1) {
+  for (int off = 4; off <= 16; off <<= 1) {
     arun.x += __shfl_xor_sync(FULL, arun.x, off); arun.y += __shfl_xor_sync(FULL, arun.y, off);
     arun.z += __shfl_xor_sync(FULL, arun.z, off); arun.w += __shfl_xor_sync(FULL, arun.w, off);
   }
@@ -1212,7 +1212,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     float4 o;
     o.x = lrun > 0.f ? arun.x / lrun : 0.f; o.y = lrun > 0.f ? arun.y / lrun : 0.f;
     o.z = lrun > 0.f ? arun.z / lrun : 0.f; o.w = lrun > 0.f ? arun.w / lrun : 0.f;
-    *reinterpret_cast<float4*>(a.out + hb * D + dq * 32 + l8 * 4) = o;
+    *reinterpret_cast<float4*>(a.out + hb * D + dq * 16 + l8 * 4) = o;
   }
   __syncwarp();
 }
@@ -1221,7 +1221,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
 template <int D, int BS>
 __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid_constant__ StepArgs a) {
   constexpr int LPR = D / 8;
-  constexpr int NQ = D / 32;                             // merge slices per query head
+  constexpr int NQ = D / 16;                             // merge slices per query head
   const int CR = a.CR;                                   // rows per score chunk
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long bars_all[2 * 12];
