@@ -49,7 +49,7 @@ constexpr uint32_t SPIN_LIMIT = 1u << 22;  // ~0.1-0.5 s of polling, then give u
 
 // Dependencies between warps are epoch-valued FLAGS, not counters: a producer publishes with one
 // st.release of the launch's epoch (no atomics, nothing to reset), a consumer polls exactly the
-// flags of the items it needs.  ctl = header, then sel[Rmax] (A, M, counters written), sel2[Rmax] (merge
+// flags of the items it needs.  ctl = header, then sel[Rmax] (A, M, counters written), sel2[Rmax] x 64 bit (epoch << 32 | list lengths: merge
 // list written), spec-unit flags [Rmax*Bud], repair-unit flags [Rmax*K], score-chunk flags [Rmax*MB].
 enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_EPOCH = 2, CTL_HDR = 8 };
 
@@ -71,6 +71,14 @@ __device__ __forceinline__ unsigned long long ld_relaxed64(const unsigned long l
 }
 __device__ __forceinline__ void st_relaxed64(unsigned long long* p, unsigned long long v) {
   asm volatile("st.relaxed.gpu.global.u64 [%0], %1;\n" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void st_release64(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.release.gpu.global.u64 [%0], %1;\n" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];\n" : "=l"(v) : "l"(p) : "memory");
+  return v;
 }
 __device__ __forceinline__ void st_release(uint32_t* p, uint32_t v) {
   asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
@@ -403,7 +411,7 @@ struct StepArgs {
   // repair warp polls ITS word: no flag, no fence and no second load between selection and the tile request.
   unsigned long long* mtag;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
-  uint32_t* ctl; uint32_t* sel; uint32_t* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
+  uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
   float scale; float pace_ns; double score_c;
@@ -776,7 +784,7 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
 
 // The row's merge list (warp 0 of the team): hit slots (all of P when retained) ascending, then the
 // repair slots; needs the bitmask of A in m.amask and the predicted blocks by slot in m.plist.
-__device__ __forceinline__ void write_merge_list(const StepArgs& a, int row, int nb, int nM, const TeamMem& m) {
+__device__ __forceinline__ uint32_t write_merge_list(const StepArgs& a, int row, int nb, int nM, const TeamMem& m) {
   const int lane = threadIdx.x & 31;
   uint32_t* ms = a.msrc + (size_t)row * (a.Bud + a.K);
   int base = 0;
@@ -791,7 +799,9 @@ __device__ __forceinline__ void write_merge_list(const StepArgs& a, int row, int
     }
   }
   for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
-  if (lane == 0) a.mn[row] = (base << 16) | (base + nM);  // speculative entries | all entries
+  const uint32_t pk = ((uint32_t)base << 16) | (uint32_t)(base + nM);  // speculative entries | all entries
+  if (lane == 0) a.mn[row] = (int32_t)pk;
+  return pk;  // travels with the flag (sel2), so the merge needs no load for it
 }
 
 // Ordered emission from the registers (see team_emit for the outputs).
@@ -833,9 +843,10 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
     for (int j = nMq + tm.tid; j < widthM; j += tm.nt) st_relaxed64(mtag + j, (unsigned long long)ep << 32);  // void tickets
     // the merge list, published before the ordered lists are written: the merge of the speculative
     // entries can start while the repairs are in flight
-    if (tm.wid == 0) write_merge_list(a, row, nb, nMq, m);
+    uint32_t pk = 0;
+    if (tm.wid == 0) pk = write_merge_list(a, row, nb, nMq, m);
     tm.sync();
-    if (tm.tid == 0) st_release(&a.sel2[row], ep);
+    if (tm.tid == 0) st_release64(&a.sel2[row], ((unsigned long long)ep << 32) | pk);
   }
   if (tm.wid == 0) {  // exclusive scan of the per-word counts, in block order
     uint32_t carry = 0;
@@ -1066,7 +1077,8 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   }
   // ---- publish (select only) ----
   const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
-  if (!fast && tm.wid == 0) write_merge_list(a, row, nb, nM, m);  // (the fast path wrote and published it already)
+  uint32_t pkg = 0;
+  if (!fast && tm.wid == 0) pkg = write_merge_list(a, row, nb, nM, m);  // (the fast path wrote and published it already)
   if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
     a.counts[row * 3 + 1] = np;
@@ -1081,7 +1093,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   tm.sync();  // every thread's stores (A, M, merge list, counts) are ordered before the release
   if (tm.tid == 0) {
     st_release(&a.sel[row], ep);
-    if (!fast) st_release(&a.sel2[row], ep);
+    if (!fast) st_release64(&a.sel2[row], ((unsigned long long)ep << 32) | pkg);
   }
 }
 
@@ -1092,7 +1104,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
 template <int D>
-__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep,
+__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep, uint32_t pk,
                           unsigned long long* tl) {
   constexpr uint32_t REP = 0x80000000u;
   const int lane = threadIdx.x & 31;
@@ -1103,7 +1115,6 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   uint32_t* cs = reinterpret_cast<uint32_t*>(buf) + E;   // [E] slot codes (REP bit: repair buffers)
   float* ls = reinterpret_cast<float*>(buf) + 2 * E;     // [E] l
   // the row's merge list was written by select(row): slot codes, speculative slots first
-  const uint32_t pk = (uint32_t)__ldcg(a.mn + row);
   const int n = (int)(pk & 0xffffu), nh = (int)(pk >> 16);
   const uint32_t* ms = a.msrc + (size_t)row * E;
   const int grp = lane >> 2, l8 = lane & 3;  // 8 entry groups x 4 lanes x float4 = a 16-channel slice
@@ -1474,9 +1485,17 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       const int bh = t / NQ, dq = t - bh * NQ;
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
-      wait_eq(&a.sel2[row], ep, &ctl[CTL_ERR]);  // the row's merge list is complete
+      unsigned long long fv = 0ull;  // the row's merge list is complete: its lengths arrive with the flag
+      if (lane == 0) {
+        uint32_t it = 0;
+        while ((uint32_t)((fv = ld_acquire64(&a.sel2[row])) >> 32) != ep) {
+          __nanosleep(20);
+          if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); fv = 0ull; break; }
+        }
+      }
+      const uint32_t pk = __shfl_sync(FULL, (uint32_t)fv, 0);
       if (tl && lane == 0) tl[12] = gtime();
-      job_merge<D>(a, b, hq, dq, buf, ep, tl);
+      job_merge<D>(a, b, hq, dq, buf, ep, pk, tl);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
@@ -1620,7 +1639,8 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.ctl = c->ctl; a.stats = c->stats;
   {
     const size_t rm = (size_t)c->maxB * c->Hkv;
-    a.sel = c->ctl + CTL_HDR; a.sel2 = a.sel + rm; a.ufs = a.sel2 + rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
+    const size_t rme = (rm + 1) & ~(size_t)1;  // sel2 is 64-bit: keep it 8-byte aligned
+    a.sel = c->ctl + CTL_HDR; a.sel2 = (unsigned long long*)(a.sel + rme); a.ufs = a.sel + rme + 2 * rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
   } a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.Rmax = c->maxB * c->Hkv;
