@@ -414,6 +414,7 @@ struct StepArgs {
   uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
+  int msw;  // channels per merge item (16 .. D): the narrowest slice that still gives every merge warp at most one item
   float scale; float pace_ns; double score_c;
 };
 
@@ -1103,7 +1104,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // whole speculative segment of a row in one round trip); the groups are folded with three shuffles.  Entry order is fixed (speculative slots
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
-template <int D>
+template <int D, int MSW>
 __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep, uint32_t pk,
                           unsigned long long* tl) {
   constexpr uint32_t REP = 0x80000000u;
@@ -1117,9 +1118,11 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   // the row's merge list was written by select(row): slot codes, speculative slots first
   const int n = (int)(pk & 0xffffu), nh = (int)(pk >> 16);
   const uint32_t* ms = a.msrc + (size_t)row * E;
-  const int grp = lane >> 2, l8 = lane & 3;  // 8 entry groups x 4 lanes x float4 = a 16-channel slice
-  const float* Os = a.O_spec + hb * a.Bud * D + dq * 16 + l8 * 4;
-  const float* Or = a.O_rep + hb * a.K * D + dq * 16 + l8 * 4;
+  // slice of msw channels: msw / 4 lanes x float4 per entry group, 128 / msw entry groups per warp
+  constexpr int lpg = MSW / 4, ng = 32 / lpg;
+  const int grp = lane / lpg, l8 = lane % lpg;
+  const float* Os = a.O_spec + hb * a.Bud * D + dq * MSW + l8 * 4;
+  const float* Or = a.O_rep + hb * a.K * D + dq * MSW + l8 * 4;
   // Two segments folded by Eq. 6-8: first the speculative entries (their units finished while
   // selection ran), then the repaired ones -- so only the few repair rows are left to fetch once
   // the last repair unit has published.
@@ -1187,12 +1190,12 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     __syncwarp();
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-    for (int e0 = s0 + grp; e0 < s1; e0 += 8 * 10) {  // 10 rows per lane (80 entries per warp) in flight
+    for (int e0 = s0 + grp; e0 < s1; e0 += ng * 10) {  // 10 rows per lane in flight (80 entries per warp at 16 channels)
       float4 x[10];
       float w[10];
 #pragma unroll
       for (int u = 0; u < 10; ++u) {
-        const int e = e0 + 8 * u;
+        const int e = e0 + ng * u;
         const bool on = e < s1;
         const uint32_t code = on ? cs[e] : 0u;
         w[u] = on ? ws[e] : 0.f;
@@ -1215,7 +1218,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     mrun = mnew;
   }
 #pragma unroll
-  for (int off = 4; off <= 16; off <<= 1) {
+  for (int off = lpg; off <= 16; off <<= 1) {
     arun.x += __shfl_xor_sync(FULL, arun.x, off); arun.y += __shfl_xor_sync(FULL, arun.y, off);
     arun.z += __shfl_xor_sync(FULL, arun.z, off); arun.w += __shfl_xor_sync(FULL, arun.w, off);
   }
@@ -1223,7 +1226,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
     float4 o;
     o.x = lrun > 0.f ? arun.x / lrun : 0.f; o.y = lrun > 0.f ? arun.y / lrun : 0.f;
     o.z = lrun > 0.f ? arun.z / lrun : 0.f; o.w = lrun > 0.f ? arun.w / lrun : 0.f;
-    *reinterpret_cast<float4*>(a.out + hb * D + dq * 16 + l8 * 4) = o;
+    *reinterpret_cast<float4*>(a.out + hb * D + dq * MSW + l8 * 4) = o;
   }
   __syncwarp();
 }
@@ -1232,7 +1235,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
 template <int D, int BS>
 __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid_constant__ StepArgs a) {
   constexpr int LPR = D / 8;
-  constexpr int NQ = D / 16;                             // merge slices per query head
+  const int NQ = D / a.msw;                              // merge slices per query head
   const int CR = a.CR;                                   // rows per score chunk
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   __shared__ __align__(8) unsigned long long bars_all[2 * 12];
@@ -1495,7 +1498,8 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       }
       const uint32_t pk = __shfl_sync(FULL, (uint32_t)fv, 0);
       if (tl && lane == 0) tl[12] = gtime();
-      job_merge<D>(a, b, hq, dq, buf, ep, pk, tl);
+      if (a.msw == 16) job_merge<D, 16>(a, b, hq, dq, buf, ep, pk, tl);
+      else job_merge<D, D>(a, b, hq, dq, buf, ep, pk, tl);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
@@ -1544,6 +1548,10 @@ static cudaError_t launch_step_t(prr_ctx* c, const StepArgs& a0, cudaStream_t s)
   if (a.J) {  // worker CTAs: enough warps for one wave of speculative units; the rest also merge
     const int U = a.spec ? R * a.Bud : 0;
     a.J = std::max(a.J, std::min(c->n_sm - (U + W - 1) / W, c->n_sm / 4));
+  }
+  {
+    const long long mw = (long long)W * (c->n_sm - a.J);  // warps that merge (all of them in warp mode)
+    a.msw = (long long)a.B * a.Hq * (D / 16) <= mw ? 16 : D;  // 16-channel slices when every merge warp gets at most one
   }
   const size_t smem = (size_t)W * per_warp;
   {  // score chunk: one per scoring warp (job CTAs do not score), so every warp's summary loads are one batch
