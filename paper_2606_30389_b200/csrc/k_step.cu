@@ -410,6 +410,9 @@ struct StepArgs {
   // M as self-describing words, one per (row, repair slot): epoch << 32 | block + 1 (0 = no such miss).  A
   // repair warp polls ITS word: no flag, no fence and no second load between selection and the tile request.
   unsigned long long* mtag;
+  // the step's scores once more as self-describing words (epoch << 32 | fp32 bits), [Rmax, MB]: a row job in
+  // the fast path polls its own words instead of chunk flags: no producer fence and no flag -> data round trip
+  unsigned long long* sc64;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
   uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
@@ -618,11 +621,12 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
 // each: the group's queries are pre-summed per channel in fp64, products and sums are exact (Q1).
 template <int D>
 __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int r0, int end_ld, unsigned char* stage,
-                                           unsigned long long* tl) {
+                                           uint32_t ep, unsigned long long* tl) {
   constexpr int LPR = D / 8, RW = 32 / LPR;
   const int lane = threadIdx.x & 31, sub = lane / LPR, l = lane % LPR;
   const uint4* rows = a.summ + (((size_t)b * a.Hkv + h) * a.MB + r0) * LPR + l;
   float* out = a.scores + ((size_t)b * a.Hkv + h) * a.MB + r0;
+  unsigned long long* out64 = a.sc64 + ((size_t)b * a.Hkv + h) * a.MB + r0;
   // The copies do not wait for the sequence length: rows up to the chunk's end inside the summary
   // buffer are fetched (rows past the last block hold stale data and are never scored).
   const int nld = end_ld - r0;
@@ -721,7 +725,11 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
     double v1 = (upC ? v2[1] : v2[0]) + __shfl_xor_sync(FULL, upC ? v2[0] : v2[1], LPR / 8);
     if (LPR == 16) v1 += __shfl_xor_sync(FULL, v1, 1);
     const int r = rr0 + ((upA ? 4 : 0) + (upB ? 2 : 0) + (upC ? 1 : 0)) * RW + sub;
-    if (r < nr && (LPR == 8 || (l & 1) == 0)) out[r] = f64_to_score(__dmul_rn(v1, a.score_c));
+    if (r < nr && (LPR == 8 || (l & 1) == 0)) {
+      const float sv = f64_to_score(__dmul_rn(v1, a.score_c));
+      st_relaxed64(out64 + r, ((unsigned long long)ep << 32) | __float_as_uint(sv));
+      out[r] = sv;
+    }
   }
   if (rr0 < nr) {  // at most 4 * RW rows left
     double acc[4], v2[2];
@@ -734,7 +742,11 @@ __device__ __forceinline__ int score_chunk(const StepArgs& a, int b, int h, int 
 #pragma unroll
     for (int off = LPR / 8; off >= 1; off >>= 1) v1 += __shfl_xor_sync(FULL, v1, off);
     const int r = rr0 + ((upA ? 2 : 0) + (upB ? 1 : 0)) * RW + sub;
-    if (r < nr && (l & (LPR / 4 - 1)) == 0) out[r] = f64_to_score(__dmul_rn(v1, a.score_c));
+    if (r < nr && (l & (LPR / 4 - 1)) == 0) {
+      const float sv = f64_to_score(__dmul_rn(v1, a.score_c));
+      st_relaxed64(out64 + r, ((unsigned long long)ep << 32) | __float_as_uint(sv));
+      out[r] = sv;
+    }
   }
   __syncwarp();
   return nb;
@@ -888,6 +900,34 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
   return tot;
 }
 
+// The row's scores for the blocks this thread owns (t, t + nt, ...), polled as epoch-tagged words:
+// every missing word is re-requested each round (all in flight together), the warp leaves on a vote.
+__device__ __forceinline__ void poll_scores(const unsigned long long* s64, int nb, int tid, int nt, uint32_t ep,
+                                            float (&x)[KB], uint32_t* err) {
+  uint32_t pend = 0u;
+#pragma unroll
+  for (int e = 0; e < KB; ++e) {
+    x[e] = 0.f;
+    if (tid + e * nt < nb) pend |= 1u << e;
+  }
+  uint32_t it = 0;
+#pragma unroll 1
+  for (;;) {
+    unsigned long long w[KB];
+#pragma unroll
+    for (int e = 0; e < KB; ++e) w[e] = (pend >> e) & 1u ? ld_relaxed64(s64 + tid + e * nt) : 0ull;
+#pragma unroll
+    for (int e = 0; e < KB; ++e)
+      if (((pend >> e) & 1u) && (uint32_t)(w[e] >> 32) == ep) {
+        x[e] = __uint_as_float((uint32_t)w[e]);
+        pend &= ~(1u << e);
+      }
+    if (__all_sync(FULL, pend == 0u)) break;
+    __nanosleep(20);
+    if (++it > SPIN_LIMIT) { if ((threadIdx.x & 31) == 0) atomicExch(err, 1u); break; }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // One row job by one team (a single code path for both kinds, so the kernel holds ONE copy of the
 // selection code: the instruction cache is 32 KB and this code runs once per step, on the
@@ -954,18 +994,26 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
     }
   }
   const bool in_sm = n <= m.key_cap;
-  // ---- wait for the row's scores ----
+  const bool fast = in_sm && n <= KB * tm.nt;  // (uniform over the team)
+  const unsigned long long* s64 = a.sc64 + (size_t)row * a.MB;
+  // ---- wait for the row's scores (the fast path polls the tagged score words themselves, below) ----
   if (tm.wid == 0) {  // one flag per score chunk of the row, a few per lane
     const int cprs = (a.MB + a.CR - 1) / a.CR, target = (nb + a.CR - 1) / a.CR;
     const uint32_t* f = a.sfl + (size_t)row * cprs;
-    wait_flags(f, target, ep, &ctl[CTL_ERR]);
+    // (fast path: only the row's first chunk flag, as the sign that the scores are about to land --
+    // polling 2048 tagged words per row from the start of the step would load L2 for nothing)
+    wait_flags(f, fast ? min(1, target) : target, ep, &ctl[CTL_ERR]);
   }
   tm.sync();
   if (tl && tm.tid == 0) tl[8] = gtime();
   // ---- keys ----
   uint32_t kmin = 0xffffffffu, kmax = 0u;
   float* pr = a.pred + (size_t)row * a.MB;
-  constexpr int KB = 12;  // scores per thread whose loads are in flight together
+  float xf[KB];
+  if (fast) {  // every thread of the team takes part (votes inside)
+    poll_scores(s64, nb, tm.tid, tm.nt, ep, xf, &ctl[CTL_ERR]);
+    if (tl && tm.tid == 0) tl[8] = gtime();
+  }
   if (is_sel) {
 #pragma unroll 1
     for (int i0 = tm.tid; i0 < nb; i0 += KB * tm.nt) {
@@ -973,7 +1021,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 #pragma unroll
       for (int e = 0; e < KB; ++e) {
         const int i = i0 + e * tm.nt;
-        x[e] = i < nb ? __ldcg(sc + i) : 0.f;
+        x[e] = fast ? xf[e] : (i < nb ? __ldcg(sc + i) : 0.f);
       }
 #pragma unroll
       for (int e = 0; e < KB; ++e) {
@@ -996,7 +1044,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 #pragma unroll
         for (int e = 0; e < KB; ++e) {
           const int i = i0 + e * tm.nt;
-          x[e] = i < nb ? __ldcg(sc + i) : 0.f;
+          x[e] = fast ? xf[e] : (i < nb ? __ldcg(sc + i) : 0.f);
         }
 #pragma unroll
         for (int e = 0; e < KB; ++e) {
@@ -1038,7 +1086,6 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   Keys ks{in_sm ? smem_u32(m.keys) : 0u, is_sel ? sc : pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
-  const bool fast = in_sm && n <= KB * tm.nt;  // (uniform over the team)
   uint32_t kreg[KB];
   if (fast) {
 #pragma unroll
@@ -1313,7 +1360,7 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       int nb = 0;
 #pragma unroll 1
       for (int r0 = ch * CR; r0 < end; r0 += maxr) {
-        nb = score_chunk<D>(a, b, h, r0, min(end, r0 + maxr), Ks, tl);
+        nb = score_chunk<D>(a, b, h, r0, min(end, r0 + maxr), Ks, ep0 + 1u, tl);
         if (r0 + maxr >= nb) break;
       }
       if (tl && lane == 0) tl[14] = gtime();
@@ -1641,7 +1688,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.theta = c->theta + (size_t)kv->layer * c->maxB * 3;
   a.P0 = c->Pbuf[0] + r * c->Bud; a.P1 = c->Pbuf[1] + r * c->Bud; a.parity = c->parity + kv->layer;
   a.setA = c->setA + r * c->K; a.setM = c->setM + r * c->K; a.counts = c->counts + r * 3;
-  a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
+  a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.sc64 = c->sc64; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
   a.ctl = c->ctl; a.stats = c->stats;
