@@ -215,6 +215,7 @@ __device__ void team_pick(uint32_t* hist, int NB, int need, const Team& tm, cons
 // 1 <= k < n, [lo, lo+span] = the exact key range of the row, and a zeroed histogram.
 // ---------------------------------------------------------------------------------------------
 constexpr int CAND = 128;  // survivors that are ranked directly
+constexpr uint32_t MERGE_END = 0x7fffffffu;  // tagged merge list: no entry here
 
 // The need-th (1-based) of the cnt candidates under (key desc, index asc).  A candidate is one
 // 64-bit word (key << 32 | ~index): larger word = better.  All threads work: the comparisons of a
@@ -413,6 +414,9 @@ struct StepArgs {
   // the step's scores once more as self-describing words (epoch << 32 | fp32 bits), [Rmax, MB]: a row job in
   // the fast path polls its own words instead of chunk flags: no producer fence and no flag -> data round trip
   unsigned long long* sc64;
+  // the merge lists once more as self-describing words (epoch << 32 | slot code, MERGE_END past the end),
+  // [Rmax, Bud + K]: a merge warp polls the list itself -- no flag, no producer fence, no second load
+  unsigned long long* ms64;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
   uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
@@ -797,9 +801,12 @@ __device__ __forceinline__ Thr fast_kth(const uint32_t (&key)[KB], const Keys& k
 
 // The row's merge list (warp 0 of the team): hit slots (all of P when retained) ascending, then the
 // repair slots; needs the bitmask of A in m.amask and the predicted blocks by slot in m.plist.
-__device__ __forceinline__ uint32_t write_merge_list(const StepArgs& a, int row, int nb, int nM, const TeamMem& m) {
+__device__ __forceinline__ uint32_t write_merge_list(const StepArgs& a, int row, int nb, int nM, const TeamMem& m,
+                                                     uint32_t ep) {
   const int lane = threadIdx.x & 31;
   uint32_t* ms = a.msrc + (size_t)row * (a.Bud + a.K);
+  unsigned long long* m64 = a.ms64 + (size_t)row * (a.Bud + a.K);
+  const unsigned long long tag = (unsigned long long)ep << 32;
   int base = 0;
   if (a.spec) {
     for (int j0 = 0; j0 < a.Bud; j0 += 32) {
@@ -807,11 +814,19 @@ __device__ __forceinline__ uint32_t write_merge_list(const StepArgs& a, int row,
       const int blk = j < a.Bud ? m.plist[j] : -1;
       const bool use = blk >= 0 && (a.retain || ((blk >> 5) < ((nb + 31) >> 5) && ((m.amask[blk >> 5] >> (blk & 31)) & 1u)));
       const uint32_t bal = __ballot_sync(FULL, use);
-      if (use) ms[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)j;
+      if (use) {
+        const int pos = base + __popc(bal & ((1u << lane) - 1u));
+        ms[pos] = (uint32_t)j;
+        st_relaxed64(m64 + pos, tag | (uint32_t)j);
+      }
       base += __popc(bal);
     }
   }
-  for (int j = lane; j < nM; j += 32) ms[base + j] = (uint32_t)j | 0x80000000u;
+  for (int j = lane; j < nM; j += 32) {
+    ms[base + j] = (uint32_t)j | 0x80000000u;
+    st_relaxed64(m64 + base + j, tag | (uint32_t)j | 0x80000000u);
+  }
+  for (int j = base + nM + lane; j < a.Bud + a.K; j += 32) st_relaxed64(m64 + j, tag | MERGE_END);
   const uint32_t pk = ((uint32_t)base << 16) | (uint32_t)(base + nM);  // speculative entries | all entries
   if (lane == 0) a.mn[row] = (int32_t)pk;
   return pk;  // travels with the flag (sel2), so the merge needs no load for it
@@ -857,7 +872,7 @@ __device__ __forceinline__ uint32_t fast_emit(const uint32_t (&key)[KB], int n, 
     // the merge list, published before the ordered lists are written: the merge of the speculative
     // entries can start while the repairs are in flight
     uint32_t pk = 0;
-    if (tm.wid == 0) pk = write_merge_list(a, row, nb, nMq, m);
+    if (tm.wid == 0) pk = write_merge_list(a, row, nb, nMq, m, ep);
     tm.sync();
     if (tm.tid == 0) st_release64(&a.sel2[row], ((unsigned long long)ep << 32) | pk);
   }
@@ -1126,7 +1141,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
   // ---- publish (select only) ----
   const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
   uint32_t pkg = 0;
-  if (!fast && tm.wid == 0) pkg = write_merge_list(a, row, nb, nM, m);  // (the fast path wrote and published it already)
+  if (!fast && tm.wid == 0) pkg = write_merge_list(a, row, nb, nM, m, ep);  // (the fast path wrote and published it already)
   if (tm.tid == 0) {
     a.counts[row * 3 + 0] = nA;
     a.counts[row * 3 + 1] = np;
@@ -1152,7 +1167,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // ascending, then repair slots ascending) and so is the reduction tree: the result is
 // deterministic; any order is the same real number (Q11).
 template <int D, int MSW>
-__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep, uint32_t pk,
+__device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep,
                           unsigned long long* tl) {
   constexpr uint32_t REP = 0x80000000u;
   const int lane = threadIdx.x & 31;
@@ -1162,9 +1177,43 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   float* ws = reinterpret_cast<float*>(buf);             // [E] m, then weights
   uint32_t* cs = reinterpret_cast<uint32_t*>(buf) + E;   // [E] slot codes (REP bit: repair buffers)
   float* ls = reinterpret_cast<float*>(buf) + 2 * E;     // [E] l
-  // the row's merge list was written by select(row): slot codes, speculative slots first
-  const int n = (int)(pk & 0xffffu), nh = (int)(pk >> 16);
-  const uint32_t* ms = a.msrc + (size_t)row * E;
+  // The row's merge list is written by select(row): slot codes, speculative slots first, as epoch-
+  // tagged words; this warp polls all E of them (MERGE_END past the end) and has list and lengths in
+  // one round trip once they exist.
+  int n = 0, nh = 0;
+  {
+    const unsigned long long* m64 = a.ms64 + (size_t)row * E;
+#pragma unroll 1
+    for (int eb = 0; eb < E; eb += 4 * 32) {  // warp-uniform trips (votes inside)
+      uint32_t c4[4] = {MERGE_END, MERGE_END, MERGE_END, MERGE_END};
+      uint32_t pend = 0u, it = 0;
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (eb + lane + 32 * u < E) pend |= 1u << u;
+#pragma unroll 1
+      for (;;) {
+        unsigned long long w[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) w[u] = (pend >> u) & 1u ? ld_relaxed64(m64 + eb + lane + 32 * u) : 0ull;
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (((pend >> u) & 1u) && (uint32_t)(w[u] >> 32) == ep) { c4[u] = (uint32_t)w[u]; pend &= ~(1u << u); }
+        if (__all_sync(FULL, pend == 0u)) break;
+        __nanosleep(40);
+        if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int e = eb + lane + 32 * u;
+        const bool valid = e < E && c4[u] != MERGE_END;
+        if (e < E) cs[e] = c4[u];
+        n += __popc(__ballot_sync(FULL, valid));
+        nh += __popc(__ballot_sync(FULL, valid && !(c4[u] & REP)));
+      }
+    }
+    __syncwarp();
+  }
+  if (tl && lane == 0) tl[12] = gtime();
   // slice of msw channels: msw / 4 lanes x float4 per entry group, 128 / msw entry groups per warp
   constexpr int lpg = MSW / 4, ng = 32 / lpg;
   const int grp = lane / lpg, l8 = lane % lpg;
@@ -1187,7 +1236,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
       uint32_t code[4];
       float me[4], le[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < s1 ? __ldcg(ms + e0 + 32 * u) : 0u;
+      for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < s1 ? cs[e0 + 32 * u] : 0u;
       {  // wait for exactly these entries' units (over-predicted blocks that are not merged are not
          // waited for); the warp stays converged and exits on a vote
         uint32_t it = 0;
@@ -1218,7 +1267,7 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int e = e0 + 32 * u;
-        if (e < s1) { ws[e] = me[u]; ls[e] = le[u]; cs[e] = code[u]; mx = fmaxf(mx, me[u]); }
+        if (e < s1) { ws[e] = me[u]; ls[e] = le[u]; mx = fmaxf(mx, me[u]); }
       }
     }
 #pragma unroll
@@ -1535,18 +1584,8 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
       const int bh = t / NQ, dq = t - bh * NQ;
       const int b = bh / a.Hq, hq = bh - b * a.Hq;
       const int row = b * a.Hkv + hq / a.G;
-      unsigned long long fv = 0ull;  // the row's merge list is complete: its lengths arrive with the flag
-      if (lane == 0) {
-        uint32_t it = 0;
-        while ((uint32_t)((fv = ld_acquire64(&a.sel2[row])) >> 32) != ep) {
-          __nanosleep(20);
-          if (++it > SPIN_LIMIT) { atomicExch(&ctl[CTL_ERR], 1u); fv = 0ull; break; }
-        }
-      }
-      const uint32_t pk = __shfl_sync(FULL, (uint32_t)fv, 0);
-      if (tl && lane == 0) tl[12] = gtime();
-      if (a.msw == 16) job_merge<D, 16>(a, b, hq, dq, buf, ep, pk, tl);
-      else job_merge<D, D>(a, b, hq, dq, buf, ep, pk, tl);
+      if (a.msw == 16) job_merge<D, 16>(a, b, hq, dq, buf, ep, tl);
+      else job_merge<D, D>(a, b, hq, dq, buf, ep, tl);
     }
   }
   if (tl && lane == 0) tl[5] = gtime();
@@ -1688,7 +1727,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.theta = c->theta + (size_t)kv->layer * c->maxB * 3;
   a.P0 = c->Pbuf[0] + r * c->Bud; a.P1 = c->Pbuf[1] + r * c->Bud; a.parity = c->parity + kv->layer;
   a.setA = c->setA + r * c->K; a.setM = c->setM + r * c->K; a.counts = c->counts + r * 3;
-  a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.sc64 = c->sc64; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
+  a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.sc64 = c->sc64; a.ms64 = c->ms64; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
   a.ctl = c->ctl; a.stats = c->stats;

@@ -129,6 +129,7 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->pred, srows * (size_t)c->MB));
   A(dalloc(c, &c->mtag, srows * (size_t)c->K));
   A(dalloc(c, &c->sc64, srows * (size_t)c->MB));
+  A(dalloc(c, &c->ms64, srows * (size_t)(c->Bud + c->K)));
   A(dalloc(c, &c->ctl, (size_t)10 + srows * ((size_t)3 + c->Bud + c->K + c->MB)));  // header + flag arrays (k_step.cu)
   c->tl_warps = c->n_sm * 32;
   A(dalloc(c, &c->tl, (size_t)c->tl_warps * 16));

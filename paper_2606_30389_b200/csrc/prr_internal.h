@@ -40,6 +40,7 @@ struct prr_ctx {
   float *O_rep = nullptr, *m_rep = nullptr, *l_rep = nullptr;    // [maxB, Hq, K, D]   / [.., K]
   unsigned long long* stats = nullptr; // [4]
   uint32_t* maskA = nullptr;  // [maxB, Hkv, ceil(MB/32)] bitmask of A (fused step)
+  unsigned long long* ms64 = nullptr; // [maxB, Hkv, Bud+K] epoch-tagged merge lists of the running step (fused step)
   unsigned long long* sc64 = nullptr; // [maxB, Hkv, MB] epoch-tagged scores of the running step (fused step)
   unsigned long long* mtag = nullptr; // [maxB, Hkv, K] epoch-tagged missed blocks of the running step (fused step)
   float* pred = nullptr;      // [maxB, Hkv, MB] Eq. 2 predictions of the row being ranked (fused step)
