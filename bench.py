@@ -230,6 +230,9 @@ def main():
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0 and args.impl != "reference":
+        from paper_2606_30389_b200 import build as _b       # incremental: a no-op when libprr.so is up to date
+        _b.build()
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = synth.CONFIGS[args.config]
