@@ -233,6 +233,12 @@ def main():
     if int(os.environ.get("LOCAL_RANK", "0")) == 0 and args.impl != "reference":
         from paper_2606_30389_b200 import build as _b       # incremental: a no-op when libprr.so is up to date
         _b.build()
+    elif args.impl != "reference":                          # the other ranks wait for rank 0's build
+        from paper_2606_30389_b200 import build as _b
+        for _ in range(600):
+            if os.path.exists(_b.LIB) and not os.path.exists(_b.LIB + ".lock"):
+                break
+            time.sleep(0.5)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = synth.CONFIGS[args.config]

@@ -54,7 +54,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=min(8, max(1, len(jobs)))) as ex:
         list(ex.map(run, jobs))
     if jobs or not os.path.exists(LIB):
-        run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs, "-o", LIB])
+        lock = LIB + ".lock"                                 # seen by processes waiting for this build
+        open(lock, "w").close()
+        try:
+            run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs, "-o", LIB])
+        finally:
+            os.remove(lock)
     return LIB
 
 
