@@ -145,12 +145,13 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->l_rep, qrows * c->K, false));
   A(dalloc(c, &c->stats, (size_t)4));
   A(dalloc(c, &c->cal_acc, (size_t)2 * 80 * c->Hkv + 80 + 2));
-  uint16_t *sq = nullptr, *sk = nullptr, *sv = nullptr;
-  A(dalloc(c, &sq, qrows * c->D));
-  A(dalloc(c, &sk, srows * c->D));
-  A(dalloc(c, &sv, srows * c->D));
+  // host-buffer entry point: q | k_new | v_new are staged in ONE pinned buffer and cross PCIe as ONE copy
+  uint16_t* sq = nullptr;
+  const size_t st_elems = (qrows + 2 * srows) * c->D;   // (every part is a multiple of 16 bytes: D >= 64)
+  A(dalloc(c, &sq, st_elems));
   A(dalloc(c, &c->st_out, qrows * c->D));
-  c->st_q = sq; c->st_k = sk; c->st_v = sv;
+  c->st_q = sq; c->st_k = sq ? sq + qrows * c->D : nullptr; c->st_v = sq ? sq + (qrows + srows) * c->D : nullptr;
+  if (e == cudaSuccess) e = cudaHostAlloc(&c->st_pin, st_elems * sizeof(uint16_t), cudaHostAllocDefault);
   if (e == cudaSuccess) {
     // P lists start empty (-1); theta defaults to (1, 1, 0): "reuse the last step's top-K" (S1)
     e = cudaMemset(c->P_next, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
@@ -184,6 +185,7 @@ extern "C" int32_t prr_destroy(prr_ctx* c) {
   if (!c) return PRR_E_INVALID;
   cudaDeviceSynchronize();
   for (void* p : c->allocs) cudaFree(p);
+  if (c->st_pin) cudaFreeHost(c->st_pin);
   if (c->cal_state) cudaFree(c->cal_state);
   if (c->cal_mask) cudaFree(c->cal_mask);
   if (c->cal_den) cudaFree(c->cal_den);
@@ -553,9 +555,22 @@ extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, co
     PRR_FAIL(ctx, PRR_E_INVALID, "prr_decode_step_host: null argument");
   cudaStream_t s = (cudaStream_t)stream;
   const size_t qb = (size_t)kv->batch * ctx->Hq * ctx->D, kb = (size_t)kv->batch * ctx->Hkv * ctx->D;
-  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_q, q_host, qb * 2, cudaMemcpyHostToDevice, s));
-  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_k, k_new_host, kb * 2, cudaMemcpyHostToDevice, s));
-  PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_v, v_new_host, kb * 2, cudaMemcpyHostToDevice, s));
+  // one host->device copy: the three inputs are packed (at the layout of a full batch: the device
+  // pointers st_q / st_k / st_v are fixed offsets) into the pinned staging buffer first.  The call
+  // synchronises the stream before it returns, so the buffer is free again on the next call.
+  const size_t qfull = (size_t)ctx->maxB * ctx->Hq * ctx->D, kfull = (size_t)ctx->maxB * ctx->Hkv * ctx->D;
+  uint16_t* pin = (uint16_t*)ctx->st_pin;
+  memcpy(pin, q_host, qb * 2);
+  memcpy(pin + qfull, k_new_host, kb * 2);
+  memcpy(pin + qfull + kfull, v_new_host, kb * 2);
+  const size_t span = kv->batch == ctx->maxB ? qfull + 2 * kfull : 0;
+  if (span) {
+    PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_q, pin, span * 2, cudaMemcpyHostToDevice, s));
+  } else {  // partial batch: the three parts are not contiguous on the device side
+    PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_q, pin, qb * 2, cudaMemcpyHostToDevice, s));
+    PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_k, pin + qfull, kb * 2, cudaMemcpyHostToDevice, s));
+    PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_v, pin + qfull + kfull, kb * 2, cudaMemcpyHostToDevice, s));
+  }
   const int r = prr_step_append(ctx, kv, ctx->st_q, ctx->st_k, ctx->st_v, summaries, ctx->st_out, 0, stream);
   if (r) return r;
   PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));

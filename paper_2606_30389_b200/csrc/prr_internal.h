@@ -55,6 +55,7 @@ struct prr_ctx {
   double* cal_acc = nullptr;  // [80, Hkv] + counts [80, Hkv] + H [80] + best[1]
   // ---- host staging for prr_decode_step_host ----
   void *st_q = nullptr, *st_k = nullptr, *st_v = nullptr; float* st_out = nullptr;
+  void* st_pin = nullptr;  // pinned host image of [q | k_new | v_new] for one copy across PCIe
 
   cudaStream_t side_spec = nullptr, side_ema = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_spec = nullptr, ev_sel = nullptr;
