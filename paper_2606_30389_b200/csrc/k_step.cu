@@ -21,7 +21,7 @@
 //     phase 4  a6: repair units, dealt out statically as (row, slot) tickets; the ticket's warp polls
 //              its own epoch-tagged word of M and runs the same tile code
 //     phase 5  a7: merge items (query head x 16-channel slice), dealt to the idle worker warps: wait
-//              for the row's merge list, then for exactly the units in it; fold hits u M (DROP) or
+//              for the row's merge list, then for exactly the units in it (their tagged m words); fold hits u M (DROP) or
 //              P u M (RETAIN) by Eq. 6-8, speculative entries first, one division at the end
 //   job CTAs (one row job each when 2R <= #SM/4; otherwise the highest-numbered warps take the jobs)
 //     phase 2  select(row): P as a bitmask, wait for the row's chunk flags, exact top-K on order-
@@ -418,6 +418,9 @@ struct StepArgs {
   // [Rmax, Bud + K]: a merge warp polls the list itself -- no flag, no producer fence, no second load
   unsigned long long* ms64;
   float* O_spec; float* m_spec; float* l_spec; float* O_rep; float* m_rep; float* l_rep;
+  // a unit's block-local maxima as self-describing words (epoch << 32 | fp32 bits of m), one per (query head,
+  // slot), written with st.release after the unit's partial rows and l: the word is the unit's "done" flag AND m
+  unsigned long long* mt_spec; unsigned long long* mt_rep;
   uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
@@ -471,9 +474,9 @@ __device__ __forceinline__ void tile_load(unsigned char* Ks, unsigned long long*
 // it was computed speculatively, as a repair, or by the sequential path.
 template <int D, int BS>
 __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long long* bars, uint32_t phase,
-                                             const StepArgs& a, int b, int h, int valid, float* O, float* Mo,
+                                             const StepArgs& a, int b, int h, int valid, float* O, unsigned long long* Mt,
                                              float* Lo, int width, int slot, const uint16_t* patch_k,
-                                             const uint16_t* patch_v) {
+                                             const uint16_t* patch_v, uint32_t ep) {
   using T = Tile<D, BS>;
   constexpr int SUB = T::SUB, NT8 = SUB / 8;
   unsigned char* Vs = Ks + T::HALF;
@@ -607,15 +610,21 @@ __device__ __forceinline__ void tile_compute(unsigned char* Ks, unsigned long lo
 #pragma unroll
     for (int dt = 0; dt < D / 8; ++dt)
       *reinterpret_cast<float2*>(O + st * D + dt * 8 + tq * 2) = make_float2(o[dt][0], o[dt][1]);
-    if (tq == 0) { Mo[st] = mrun0 * a.scale; Lo[st] = l0; }
+    if (tq == 0) Lo[st] = l0;
   }
   if (r0 + 8 < G) {
     const size_t st = (hb + r0 + 8) * width + slot;
 #pragma unroll
     for (int dt = 0; dt < D / 8; ++dt)
       *reinterpret_cast<float2*>(O + st * D + dt * 8 + tq * 2) = make_float2(o[dt][2], o[dt][3]);
-    if (tq == 0) { Mo[st] = mrun1 * a.scale; Lo[st] = l1; }
+    if (tq == 0) Lo[st] = l1;
   }
+  // publish: every lane's partial rows and l are ordered before the releases by the warp barrier (the
+  // release is cumulative over it); the tagged m IS the unit's completion flag for that query head
+  __syncwarp();
+  const unsigned long long tag = (unsigned long long)ep << 32;
+  if (tq == 0 && r0 < G) st_release64(Mt + (hb + r0) * width + slot, tag | __float_as_uint(mrun0 * a.scale));
+  if (tq == 0 && r0 + 8 < G) st_release64(Mt + (hb + r0 + 8) * width + slot, tag | __float_as_uint(mrun1 * a.scale));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1221,97 +1230,100 @@ __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned cha
   const float* Or = a.O_rep + hb * a.K * D + dq * MSW + l8 * 4;
   // Two segments folded by Eq. 6-8: first the speculative entries (their units finished while
   // selection ran), then the repaired ones -- so only the few repair rows are left to fetch once
-  // the last repair unit has published.
+  // the last repair unit has published.  A segment is processed in trips of <= 128 entries: poll the
+  // entries' tagged m words (acquire: flag and m in one), request l and the partial rows together,
+  // weights from m, fold the trip into the running state.
+  const unsigned long long* Ms = a.mt_spec + hb * a.Bud;
+  const unsigned long long* Mr = a.mt_rep + hb * a.K;
   float mrun = -CUDART_INF_F, lrun = 0.f;
   float4 arun = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
   for (int seg = 0; seg < 2; ++seg) {
-    const int s0 = seg ? nh : 0, s1 = seg ? n : nh;
-    if (s1 <= s0) continue;
-    float mx = -CUDART_INF_F;
-    // (rolled loops with a run-time trip count serialise their loads: batches with predication instead)
+    const int sb = seg ? nh : 0, se = seg ? n : nh;
 #pragma unroll 1
-    for (int eb = s0; eb < s1; eb += 4 * 32) {  // warp-uniform trips (votes inside)
-      const int e0 = eb + lane;
+    for (int s0 = sb; s0 < se; s0 += 4 * 32) {  // warp-uniform trips (votes inside)
+      const int s1 = min(se, s0 + 4 * 32);
+      const int e0 = s0 + lane;
       uint32_t code[4];
       float me[4], le[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) code[u] = e0 + 32 * u < s1 ? cs[e0 + 32 * u] : 0u;
+      for (int u = 0; u < 4; ++u) {
+        code[u] = e0 + 32 * u < s1 ? cs[e0 + 32 * u] : 0u;
+        me[u] = -CUDART_INF_F;
+      }
       {  // wait for exactly these entries' units (over-predicted blocks that are not merged are not
          // waited for); the warp stays converged and exits on a vote
-        uint32_t it = 0;
+        uint32_t pend = 0u, it = 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (e0 + 32 * u < s1) pend |= 1u << u;
 #pragma unroll 1
         for (;;) {
-          bool ok = true;
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const uint32_t j = code[u] & ~REP;
-            const uint32_t* fp = (code[u] & REP) ? a.ufr + (size_t)row * a.K + j : a.ufs + (size_t)row * a.Bud + j;
-            if (e0 + 32 * u < s1) ok = ok && (ld_acquire(fp) == ep);
-          }
-          if (__all_sync(FULL, ok)) break;
+          for (int u = 0; u < 4; ++u)
+            if ((pend >> u) & 1u) {
+              const uint32_t j = code[u] & ~REP;
+              const unsigned long long w = ld_acquire64((code[u] & REP) ? Mr + j : Ms + j);
+              if ((uint32_t)(w >> 32) == ep) { me[u] = __uint_as_float((uint32_t)w); pend &= ~(1u << u); }
+            }
+          if (__all_sync(FULL, pend == 0u)) break;
           __nanosleep(20);
           if (++it > SPIN_LIMIT) { if (lane == 0) atomicExch(a.ctl + CTL_ERR, 1u); break; }
         }
       }
       if (tl && lane == 0) tl[13 + seg] = gtime();
+      float mx = -CUDART_INF_F;
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < 4; ++u) {  // l is requested now and used after the partial rows are in flight
         const uint32_t j = code[u] & ~REP;
         const bool on = e0 + 32 * u < s1;
-        const float* mp = (code[u] & REP) ? a.m_rep + hb * a.K + j : a.m_spec + hb * a.Bud + j;
-        const float* lp = (code[u] & REP) ? a.l_rep + hb * a.K + j : a.l_spec + hb * a.Bud + j;
-        me[u] = on ? __ldcg(mp) : -CUDART_INF_F;
-        le[u] = on ? __ldcg(lp) : 0.f;
+        le[u] = on ? __ldcg((code[u] & REP) ? a.l_rep + hb * a.K + j : a.l_spec + hb * a.Bud + j) : 0.f;
+        mx = fmaxf(mx, me[u]);
       }
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
+      float wl[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        const int e = e0 + 32 * u;
-        if (e < s1) { ws[e] = me[u]; ls[e] = le[u]; mx = fmaxf(mx, me[u]); }
+        wl[u] = me[u] == -CUDART_INF_F ? 0.f : ex2((me[u] - mx) * LOG2E_F);
+        if (e0 + 32 * u < s1) ws[e0 + 32 * u] = wl[u];
       }
-    }
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
-    __syncwarp();
-    float lsum = 0.f;
-#pragma unroll 2
-    for (int e = s0 + lane; e < s1; e += 32) {
-      const float me = ws[e];
-      const float w = me == -CUDART_INF_F ? 0.f : ex2((me - mx) * LOG2E_F);
-      ws[e] = w;
-      lsum = fmaf(w, ls[e], lsum);
-    }
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
-    __syncwarp();
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      __syncwarp();
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
-    for (int e0 = s0 + grp; e0 < s1; e0 += ng * 10) {  // 10 rows per lane in flight (80 entries per warp at 16 channels)
-      float4 x[10];
-      float w[10];
+      for (int g0 = s0 + grp; g0 < s1; g0 += ng * 10) {  // 10 rows per lane in flight (80 entries per warp at 16 channels)
+        float4 x[10];
+        float w[10];
 #pragma unroll
-      for (int u = 0; u < 10; ++u) {
-        const int e = e0 + ng * u;
-        const bool on = e < s1;
-        const uint32_t code = on ? cs[e] : 0u;
-        w[u] = on ? ws[e] : 0.f;
-        const float* Op = (code & REP) ? Or + (size_t)(code & ~REP) * D : Os + (size_t)code * D;
-        x[u] = on ? __ldcg(reinterpret_cast<const float4*>(Op)) : make_float4(0.f, 0.f, 0.f, 0.f);
-      }
+        for (int u = 0; u < 10; ++u) {
+          const int e = g0 + ng * u;
+          const bool on = e < s1;
+          const uint32_t cd = on ? cs[e] : 0u;
+          w[u] = on ? ws[e] : 0.f;
+          const float* Op = (cd & REP) ? Or + (size_t)(cd & ~REP) * D : Os + (size_t)cd * D;
+          x[u] = on ? __ldcg(reinterpret_cast<const float4*>(Op)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
 #pragma unroll
-      for (int u = 0; u < 10; ++u) {
-        acc.x = fmaf(w[u], x[u].x, acc.x); acc.y = fmaf(w[u], x[u].y, acc.y);
-        acc.z = fmaf(w[u], x[u].z, acc.z); acc.w = fmaf(w[u], x[u].w, acc.w);
+        for (int u = 0; u < 10; ++u) {
+          acc.x = fmaf(w[u], x[u].x, acc.x); acc.y = fmaf(w[u], x[u].y, acc.y);
+          acc.z = fmaf(w[u], x[u].z, acc.z); acc.w = fmaf(w[u], x[u].w, acc.w);
+        }
       }
+      float lsum = 0.f;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) lsum = fmaf(wl[u], le[u], lsum);
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) lsum += __shfl_xor_sync(FULL, lsum, off);
+      __syncwarp();  // ws[] of this trip is consumed
+      // fold the trip into the running state (Eq. 6-8, unnormalised)
+      const float mnew = fmaxf(mrun, mx);
+      const float fo = mrun == -CUDART_INF_F ? 0.f : ex2((mrun - mnew) * LOG2E_F);
+      const float fn = mx == -CUDART_INF_F ? 0.f : ex2((mx - mnew) * LOG2E_F);
+      arun.x = fo * arun.x + fn * acc.x; arun.y = fo * arun.y + fn * acc.y;
+      arun.z = fo * arun.z + fn * acc.z; arun.w = fo * arun.w + fn * acc.w;
+      lrun = fo * lrun + fn * lsum;
+      mrun = mnew;
     }
-    // fold the segment into the running state (Eq. 6-8, unnormalised)
-    const float mnew = fmaxf(mrun, mx);
-    const float fo = mrun == -CUDART_INF_F ? 0.f : ex2((mrun - mnew) * LOG2E_F);
-    const float fn = mx == -CUDART_INF_F ? 0.f : ex2((mx - mnew) * LOG2E_F);
-    arun.x = fo * arun.x + fn * acc.x; arun.y = fo * arun.y + fn * acc.y;
-    arun.z = fo * arun.z + fn * acc.z; arun.w = fo * arun.w + fn * acc.w;
-    lrun = fo * lrun + fn * lsum;
-    mrun = mnew;
   }
 #pragma unroll
   for (int off = lpg; off <= 16; off <<= 1) {
@@ -1545,13 +1557,12 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
         tile_load<D, BS>(Ks, bars, a, upage, uh);
         if (tl && lane == 0 && urep) tl[10] = gtime();
       }
-      const int crow = urow, cslot = uslot;
       const bool patch = a.app && uvalid > 0 && ublk == (ulen - 1) / BS;
       const bool crep = urep;
-      tile_compute<D, BS>(Ks, bars, ph, a, ub, uh, uvalid, crep ? a.O_rep : a.O_spec, crep ? a.m_rep : a.m_spec,
+      tile_compute<D, BS>(Ks, bars, ph, a, ub, uh, uvalid, crep ? a.O_rep : a.O_spec, crep ? a.mt_rep : a.mt_spec,
                           crep ? a.l_rep : a.l_spec, crep ? a.K : a.Bud, uslot,
                           patch ? a.k_new + ((size_t)ub * a.Hkv + uh) * D : nullptr,
-                          patch ? a.v_new + ((size_t)ub * a.Hkv + uh) * D : nullptr);
+                          patch ? a.v_new + ((size_t)ub * a.Hkv + uh) * D : nullptr, ep);
       ph ^= 1u;
       pend = false;
       if (tl && lane == 0 && crep) tl[11] = gtime();
@@ -1562,7 +1573,6 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
           if (ublk >= 0) { tile_load<D, BS>(Ks, bars, a, upage, uh); pend = true; }
         }
       }
-      signal_set(crep ? &a.ufr[(size_t)crow * a.K + cslot] : &a.ufs[(size_t)crow * a.Bud + cslot], ep);
     }
   }
   if (tl && lane == 0) tl[4] = gtime();
@@ -1730,6 +1740,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.maskA = c->maskA; a.pred = c->pred; a.mtag = c->mtag; a.sc64 = c->sc64; a.ms64 = c->ms64; a.msrc = (uint32_t*)c->merge_src; a.mn = c->merge_n;
   a.O_spec = c->O_spec; a.m_spec = c->m_spec; a.l_spec = c->l_spec;
   a.O_rep = c->O_rep; a.m_rep = c->m_rep; a.l_rep = c->l_rep;
+  a.mt_spec = c->mt_spec; a.mt_rep = c->mt_rep;
   a.ctl = c->ctl; a.stats = c->stats;
   {
     const size_t rm = (size_t)c->maxB * c->Hkv;

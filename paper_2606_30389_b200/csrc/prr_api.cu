@@ -143,6 +143,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->O_rep, qrows * c->K * c->D, false));
   A(dalloc(c, &c->m_rep, qrows * c->K, false));
   A(dalloc(c, &c->l_rep, qrows * c->K, false));
+  A(dalloc(c, &c->mt_spec, qrows * (size_t)(c->Bud + 1)));
+  A(dalloc(c, &c->mt_rep, qrows * (size_t)c->K));
   A(dalloc(c, &c->stats, (size_t)4));
   A(dalloc(c, &c->cal_acc, (size_t)2 * 80 * c->Hkv + 80 + 2));
   // host-buffer entry point: q | k_new | v_new are staged in ONE pinned buffer and cross PCIe as ONE copy

@@ -40,6 +40,7 @@ struct prr_ctx {
   float *O_rep = nullptr, *m_rep = nullptr, *l_rep = nullptr;    // [maxB, Hq, K, D]   / [.., K]
   unsigned long long* stats = nullptr; // [4]
   uint32_t* maskA = nullptr;  // [maxB, Hkv, ceil(MB/32)] bitmask of A (fused step)
+  unsigned long long *mt_spec = nullptr, *mt_rep = nullptr; // [maxB, Hq, Bud+1] / [maxB, Hq, K] epoch-tagged block maxima (fused step)
   unsigned long long* ms64 = nullptr; // [maxB, Hkv, Bud+K] epoch-tagged merge lists of the running step (fused step)
   unsigned long long* sc64 = nullptr; // [maxB, Hkv, MB] epoch-tagged scores of the running step (fused step)
   unsigned long long* mtag = nullptr; // [maxB, Hkv, K] epoch-tagged missed blocks of the running step (fused step)
