@@ -220,6 +220,23 @@ int64_t prr_launch_count(const prr_ctx* ctx);
 int32_t prr_timeline_enable(prr_ctx* ctx, int32_t on);
 int32_t prr_timeline_read(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps, int32_t* n_warps_out,
                           void* stream);
+/* Same copy WITHOUT synchronising: the stamps live in pinned host memory that the device writes directly,
+ * so they can be looked at while a step is still running (or after a fault). */
+int32_t prr_timeline_peek(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps, int32_t* n_warps_out);
+
+/* Tuning / introspection of the fused step (k_row.cu).  Options are per ctx and take effect at the next
+ * launch (or capture).  PRR_OPT_PDL: 1 (default) = consecutive fused steps are linked by programmatic
+ * dependent launch, so the next step's launch latency hides behind the running one.  PRR_OPT_CLUSTER:
+ * 0 (default) = the library picks the largest cluster (1, 2, 4 or 8 CTAs per (sequence, KV head) row)
+ * that still runs every row at once; 1/2/4/8 force a size.  PRR_OPT_CUT: 1 (default) = once A is known,
+ * predicted blocks that missed and whose tile has not been requested yet are not requested (PRR_DROP
+ * only; the output is attention over A either way); 0 = every block of P is fetched.  Read-only:
+ * PRR_OPT_LAST_CLUSTER / _LAST_RING / _LAST_GRID = cluster size, ring depth and grid of the last fused
+ * launch.  Unknown option or bad value -> PRR_E_INVALID. */
+enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
+       PRR_OPT_LAST_GRID = 18 };
+int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value);
+int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* value_out /* host */);
 
 /* --- CUDA-graph helpers (so callers need no CUDA runtime of their own) ------------------------ */
 typedef struct prr_graph prr_graph;

@@ -1,0 +1,1322 @@
+// k_row — one PRR layer-step (a0-a8) as ONE launch of thread-block CLUSTERS, one cluster per
+// (sequence, KV head) row (Fig. 1, :38-42, :115 Fig. 5).
+//
+// A row -- its summaries, scores, A, P, EMA state, KV blocks and its G query heads -- is independent
+// of every other row (selection is per KV head and shared only inside the group), so
+// the row is the unit of parallelism and everything BETWEEN the stages of a row stays on chip:
+//
+//   * the CS CTAs of a cluster split the row's blocks into slices.  Each CTA streams its slice of the
+//     summary buffer through its ring of shared-memory buffers (cp.async.bulk), scores it exactly
+//     (a1, Q1), applies Eq. 3 / Eq. 2 to its blocks (a8) and sends the order-preserving score keys
+//     to EVERY CTA of the cluster and the prediction keys to one (st.async into distributed shared
+//     memory, counted by an mbarrier).  No global-memory flag sits between scoring and selection.
+//   * every CTA runs the same exact top-K on the gathered keys (a2; redundantly, so nobody has to
+//     wait for a broadcast) and therefore knows A, P, hits and M = A\P (a5) without communication.
+//   * meanwhile the tile warps compute the CTA's share of the speculative units (a4: predicted
+//     blocks dealt round-robin over the CTAs; K and V tiles by TMA in the 128-byte swizzle, one
+//     partial state (m, l, O) per block from mma.sync bf16 with the TOKENS as the M dimension).  A
+//     partial whose fate is not known yet is parked in a shared-memory slot; once A is known a hit is
+//     folded straight into the warp's running state, an over-predicted block is dropped (PRR_DROP)
+//     and predicted blocks whose tile has not been requested yet are not requested at all.
+//   * missed blocks are repaired (a6) by the CTA that owns their slice: same tile code.
+//   * merge (a7): each CTA folds its hit slots and its warps' running states per query head (Eq. 6-8),
+//     sends the result to the head's reducer CTA (st.async again), which normalises and writes out.
+//   * one CTA of the cluster ranks the prediction keys: P of the next step (a3), off the critical path.
+//
+// spec = 0 runs the same kernel as the sequential select-then-attend path: P is
+// treated as empty and every block of A is a "repair" unit that can only start after selection.
+#include <cuda.h>
+#include <math_constants.h>
+
+#include <algorithm>
+#include <cstring>
+
+#include "prr_dev.cuh"
+#include "prr_internal.h"
+
+namespace prr {
+
+constexpr float LOG2E_F = 1.4426950408889634f;
+constexpr int NWARP = 12, NTHR = 32 * NWARP;
+constexpr int NTW = 5;             // tile warps 0 .. 4
+constexpr int GA0 = 5, GAW = 4;    // group A (true top-K, lists, merge): warps 5 .. 8, named barrier 1
+constexpr int GE0 = 9, GEW = 2;    // group E (next prediction): warps 9 .. 10, named barrier 2
+constexpr int LDW = 11;            // loader warp: predicted-set staging, then every bulk / TMA request
+constexpr int NSCW = 11;           // warps 0 .. 10 score
+constexpr int NBMAX = 12;          // ring buffers at most
+constexpr int HB = 1024;           // histogram buckets of a selection pass
+constexpr int CAND = 128;          // survivors that are ranked directly
+constexpr unsigned long long WAIT_NS = 200000000ull;  // every wait gives up loudly after 0.2 s
+
+enum { CTL_EXIT = 0, CTL_ERR = 1, CTL_EPOCH = 2, CTL_SITE = 4 };
+
+struct RowArgs {
+  alignas(64) CUtensorMap mapK;  // bf16 [rows = n_pages*Hkv*bs, d], box [ST, 64], 128-byte swizzle
+  alignas(64) CUtensorMap mapV;
+  const int32_t* table; const int32_t* seq_lens;
+  // fused append (a0): app = 1 -> seq_lens holds the lengths BEFORE the append, every length below is +1
+  const uint16_t* k_new; const uint16_t* v_new; uint16_t* kp_w; uint16_t* vp_w; uint4* summ_w; double* open_sum;
+  int32_t* seq_lens_w; int app;
+  const uint16_t* q; const uint4* summ; float* out;
+  // layer state (already offset to the layer)
+  float* scores; double* ema_l; double* ema_v; int32_t* n_state; const double* theta;
+  int32_t* P0; int32_t* P1; int32_t* parity;
+  int32_t* setA; int32_t* setM; int32_t* counts;
+  uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
+  int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, retain, spec, cut;
+  int CS, NBUF, NSLOT, UCAP, HL, SLMAX;
+  // dynamic shared memory offsets (bytes)
+  int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
+      o_slots, o_slotblk, o_recv, o_end;
+  float scale; double score_c;
+};
+
+// ---------------------------------------------------------------------------------------------
+// cluster / distributed-shared-memory primitives
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;\n" ::: "memory"); }
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+// store into another CTA's shared memory; the bytes are counted by that CTA's mbarrier (complete_tx)
+__device__ __forceinline__ void st_async_v4(uint32_t raddr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t rbar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1,%2,%3,%4}, [%5];\n"
+               ::"r"(raddr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait_cl(unsigned long long* bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{ .reg .pred p; mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }\n"
+      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return done != 0;
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
+  uint32_t d;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;\n" : "=r"(d) : "r"(a));
+  return d;
+}
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
+  return t;
+}
+// Bounded waits: a dependency that never arrives raises ctl[CTL_ERR] (prr_check) instead of hanging; the
+// first site that gave up is kept in ctl[CTL_SITE] (site code | CTA << 8 | warp << 20).
+__device__ __noinline__ void wait_fail(uint32_t* err, uint32_t site) {
+  atomicCAS(err + (CTL_SITE - CTL_ERR), 0u, site | (blockIdx.x << 8) | ((threadIdx.x >> 5) << 20));
+  atomicExch(err, 1u);
+}
+__device__ __forceinline__ void wait_bar(unsigned long long* bar, uint32_t parity, uint32_t* err, uint32_t site) {
+  if (mbar_try_wait_cl(bar, parity)) return;
+  const unsigned long long t0 = gtime();
+  uint32_t it = 0;
+  while (!mbar_try_wait_cl(bar, parity))
+    if ((++it & 1023u) == 0 && (long long)(gtime() - t0) > (long long)WAIT_NS) { wait_fail(err, site); return; }
+}
+__device__ __forceinline__ void wait_flag(const volatile int* f, uint32_t* err, uint32_t site) {
+  if (*f) return;
+  const unsigned long long t0 = gtime();
+  uint32_t it = 0;
+  while (!*f) {
+    __nanosleep(32);
+    if ((++it & 1023u) == 0 && (long long)(gtime() - t0) > (long long)WAIT_NS) { wait_fail(err, site); return; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exact selection by a GROUP of warps (a named barrier): the k-th largest of n keys under the order
+// (key desc, index asc) as a threshold pair; integer-only, hence order-independent and bit-exact (Q4).
+// ---------------------------------------------------------------------------------------------
+struct Thr { uint32_t key; int idx; };  // selected(i) <=> key_i > key || (key_i == key && i <= idx)
+__device__ __forceinline__ bool selected(uint32_t key, int i, const Thr& t) {
+  return key > t.key || (key == t.key && i <= t.idx);
+}
+struct Grp {
+  int tid, nt, wid, nw, bar;
+  __device__ __forceinline__ void sync() const { asm volatile("bar.sync %0, %1;\n" ::"r"(bar), "r"(nt) : "memory"); }
+};
+struct SelMem {
+  uint32_t* hist;            // [HB], zero on entry to and exit from grp_kth
+  uint32_t* red;             // [nw * 2 + 16]: per-warp slots, then 16 decision words
+  unsigned long long* cand;  // [CAND]
+  uint32_t* offs;            // [MBw] emission offsets
+};
+
+// Highest bucket b with  sum_{b' >= b} hist[b'] >= need  (1 <= need <= total); `above` = the count
+// in the buckets over b.  Thread t owns the buckets [HB-(t+1)per, HB-t*per): a prefix scan over
+// threads is a suffix scan over buckets.  Every thread zeroes what it read and returns the triple.
+__device__ void grp_pick(const Grp& g, const SelMem& m, int need, int& bstar, int& cstar, int& above) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + g.nw * 2;
+  const int per = (HB + g.nt - 1) / g.nt;
+  const int hi = max(0, HB - g.tid * per), lo = max(0, hi - per);
+  uint32_t sum = 0;
+#pragma unroll 4
+  for (int b = lo; b < hi; ++b) sum += m.hist[b];
+  uint32_t incl = sum;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const uint32_t x = __shfl_up_sync(FULL, incl, off);
+    if (lane >= off) incl += x;
+  }
+  if (lane == 31) m.red[g.wid] = incl;
+  g.sync();
+#pragma unroll 1
+  for (int w = 0; w < g.wid; ++w) incl += m.red[w];
+  const uint32_t excl = incl - sum;
+  if ((int)excl < need && need <= (int)incl) {  // the crossing is in this thread's buckets (exactly one thread)
+    uint32_t acc = excl;
+#pragma unroll 1
+    for (int b = hi - 1; b >= lo; --b) {
+      const uint32_t c = m.hist[b];
+      if ((int)(acc + c) >= need) { dec[0] = (uint32_t)b; dec[1] = c; dec[2] = acc; break; }
+      acc += c;
+    }
+  }
+#pragma unroll 1
+  for (int b = lo; b < hi; ++b) m.hist[b] = 0u;
+  g.sync();
+  bstar = (int)dec[0]; cstar = (int)dec[1]; above = (int)dec[2];
+  g.sync();  // dec and red are reused by the caller
+}
+
+// keys[0 .. n), 1 <= k < n.
+__device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const SelMem& m) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + g.nw * 2;
+  // the exact key range of the row
+  uint32_t kmin = 0xffffffffu, kmax = 0u;
+#pragma unroll 4
+  for (int i = g.tid; i < n; i += g.nt) { const uint32_t x = keys[i]; kmin = min(kmin, x); kmax = max(kmax, x); }
+  kmin = __reduce_min_sync(FULL, kmin);
+  kmax = __reduce_max_sync(FULL, kmax);
+  if (lane == 0) { m.red[g.wid * 2] = kmin; m.red[g.wid * 2 + 1] = kmax; }
+  g.sync();
+#pragma unroll 1
+  for (int w = 0; w < g.nw; ++w) { kmin = min(kmin, m.red[w * 2]); kmax = max(kmax, m.red[w * 2 + 1]); }
+  g.sync();
+  uint32_t lo = kmin, span = kmax - kmin;
+  int need = k, cnt_in = n;
+  Thr r;
+  // invariant: the threshold key lies in [lo, lo+span]; `need` of the cnt_in keys in that range are
+  // selected, every key above it is
+  for (;;) {
+    if (span == 0) {  // all survivors share one key: the `need` lowest indices win
+      if (g.wid == 0) {
+        int base = 0, idx = n - 1;
+#pragma unroll 1
+        for (int j0 = 0; j0 < n; j0 += 32) {
+          const int i = j0 + lane;
+          const uint32_t bal = __ballot_sync(FULL, i < n && keys[i] == lo);
+          const int c = __popc(bal);
+          if (base + c >= need) { idx = j0 + (int)__fns(bal, 0, need - base); break; }
+          base += c;
+        }
+        if (lane == 0) { dec[5] = lo; dec[6] = (uint32_t)idx; }
+      }
+      g.sync();
+      r.key = dec[5]; r.idx = (int)dec[6];
+      g.sync();
+      return r;
+    }
+    if (cnt_in <= CAND) {  // collect the survivors (any order) and rank them: word = key << 32 | ~index
+      if (g.tid == 0) dec[7] = 0u;
+      g.sync();
+#pragma unroll 4
+      for (int i = g.tid; i < n; i += g.nt) {
+        const uint32_t key = keys[i];
+        if ((key - lo) <= span) {
+          const uint32_t pos = atomicAdd(&dec[7], 1u);
+          m.cand[pos] = ((unsigned long long)key << 32) | (uint32_t)~i;
+        }
+      }
+      g.sync();
+#pragma unroll 1
+      for (int e = g.tid; e < cnt_in; e += g.nt) {
+        const unsigned long long ce = m.cand[e];
+        uint32_t rank = 0;
+#pragma unroll 4
+        for (int f = 0; f < cnt_in; ++f) rank += m.cand[f] > ce;
+        if ((int)rank == need - 1) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }  // exactly one
+      }
+      g.sync();
+      r.key = dec[5]; r.idx = (int)dec[6];
+      g.sync();
+      return r;
+    }
+    const int sh = max(0, (32 - __clz(span)) - 10);  // (span >> sh) < HB
+#pragma unroll 4
+    for (int i = g.tid; i < n; i += g.nt) {
+      const uint32_t d = keys[i] - lo;
+      if (d <= span) atomicAdd(&m.hist[d >> sh], 1u);
+    }
+    g.sync();
+    int bstar, cstar, above;
+    grp_pick(g, m, need, bstar, cstar, above);
+    need -= above;
+    cnt_in = cstar;
+    const uint32_t off = (uint32_t)bstar << sh;
+    const uint32_t width = sh ? ((1u << sh) - 1u) : 0u;
+    lo += off;
+    span = min(span - off, width);
+    if (need == cnt_in) { r.key = lo; r.idx = 0x7fffffff; return r; }  // the whole sub-range is selected
+  }
+}
+
+// Bitmask of the selected blocks into mask[0 .. nwd) (shared), one ballot per 32 blocks.
+__device__ __forceinline__ void grp_mask(const uint32_t* keys, int n, int k, const Thr& t, const Grp& g, uint32_t* mask) {
+  const int lane = threadIdx.x & 31;
+  const int nwd = (n + 31) >> 5;
+#pragma unroll 2
+  for (int w = g.wid; w < nwd; w += g.nw) {
+    const int i = w * 32 + lane;
+    const bool sel = i < n && k > 0 && selected(keys[i], i, t);
+    const uint32_t bal = __ballot_sync(FULL, sel);
+    if (lane == 0) mask[w] = bal;
+  }
+}
+
+// Ordered emission from a bitmask: the set bits ascending into list[width] (padded with -1); with
+// Mlist != null also the set bits NOT in pmask (ascending, padded to widthM).  Returns (nA << 16) | nM.
+__device__ uint32_t grp_emit(const uint32_t* mask, const uint32_t* pmask, int n, const Grp& g, const SelMem& m,
+                             int32_t* list, int width, int32_t* Mlist, int widthM) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t lt = (1u << lane) - 1u;
+  const int nwd = (n + 31) >> 5;
+  uint32_t* dec = m.red + g.nw * 2;
+  if (g.wid == 0) {
+    uint32_t carry = 0;
+#pragma unroll 1
+    for (int w0 = 0; w0 < nwd; w0 += 32) {
+      const int w = w0 + lane;
+      const uint32_t aw = w < nwd ? mask[w] : 0u;
+      const uint32_t mw = (Mlist && w < nwd) ? (aw & ~pmask[w]) : 0u;
+      const uint32_t v = ((uint32_t)__popc(aw) << 16) | (uint32_t)__popc(mw);
+      uint32_t incl = v;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const uint32_t x = __shfl_up_sync(FULL, incl, off);
+        if (lane >= off) incl += x;
+      }
+      if (w < nwd) m.offs[w] = carry + incl - v;
+      carry += __shfl_sync(FULL, incl, 31);
+    }
+    if (lane == 0) dec[3] = carry;
+  }
+  g.sync();
+#pragma unroll 2
+  for (int w = g.wid; w < nwd; w += g.nw) {
+    const uint32_t aw = mask[w];
+    const uint32_t off = m.offs[w];
+    const int i = w * 32 + lane;
+    if ((aw >> lane) & 1u) {
+      list[(off >> 16) + __popc(aw & lt)] = i;
+      if (Mlist) {
+        const uint32_t mw = aw & ~pmask[w];
+        if ((mw >> lane) & 1u) Mlist[(off & 0xffffu) + __popc(mw & lt)] = i;
+      }
+    }
+  }
+  const uint32_t tot = dec[3];
+#pragma unroll 1
+  for (int j = (int)(tot >> 16) + g.tid; j < width; j += g.nt) list[j] = -1;
+  if (Mlist)
+#pragma unroll 1
+    for (int j = (int)(tot & 0xffffu) + g.tid; j < widthM; j += g.nt) Mlist[j] = -1;
+  g.sync();
+  return tot;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Tiles.  Shared-memory image of one (block, KV head, sub-tile) as the copy engine writes it: the
+// K half then the V half, each D/64 boxes of [ST rows x 128 bytes] in the 128-byte swizzle (the
+// 16-byte chunk c of row r sits at chunk c ^ (r & 7)), so ldmatrix is conflict-free without padding.
+// ---------------------------------------------------------------------------------------------
+template <int D, int ST>
+struct Tile {
+  static constexpr int NBOX = D / 64;
+  static constexpr int BOX_BYTES = ST * 128;
+  static constexpr int HALF = NBOX * BOX_BYTES;  // = ST * D * 2
+  static constexpr int BYTES = 2 * HALF;         // K tile + V tile
+  static constexpr int CHR = BYTES / (D * 2);    // summary rows one buffer holds (= 2 ST)
+  __device__ static __forceinline__ const unsigned char* at(const unsigned char* half, int r, int c) {
+    return half + (c >> 3) * BOX_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+  }
+};
+
+// Partial state of one landed tile for the (<= 8) query heads of one pass (the forward
+// also writes l and m), by ONE warp: S^T = K Q^T on mma.sync m16n8k16 with the TOKENS as the M rows
+// (a 16-token slab of the tile is the A operand straight from the swizzled image, the query heads
+// are the 8 columns of B, zero padded), tile-local max / sum over the token dimension with
+// shuffles, then O^T = V^T P^T with V^T through ldmatrix.trans and P^T from the score fragments by
+// movmatrix (P as a two-term bf16 split).  Per thread: heads g = 2 (lane % 4) + {0, 1};
+// o[dt] = O^T[d = 16 dt + lane / 4 (+ 8)][g].  m in log2 units of the scaled logit.
+template <int D, int ST>
+__device__ __forceinline__ void tile_partial(const unsigned char* Ks, unsigned long long* barK, unsigned long long* barV,
+                                             uint32_t par, const uint32_t (&qb)[D / 16][2], int valid, float sl2,
+                                             const uint16_t* patch_k, const uint16_t* patch_v, bool first_pass,
+                                             float (&o)[D / 16][4], float (&mt)[2], float (&lt)[2], uint32_t* err) {
+  using T = Tile<D, ST>;
+  constexpr int NM = ST / 16;
+  const unsigned char* Vs = Ks + T::HALF;
+  const int lane = threadIdx.x & 31;
+  const int r0 = lane >> 2;
+  float s[NM][4];
+#pragma unroll
+  for (int m = 0; m < NM; ++m)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) s[m][e] = 0.f;
+#pragma unroll
+  for (int dt = 0; dt < D / 16; ++dt)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) o[dt][e] = 0.f;
+
+  if (first_pass) {
+    wait_bar(barK, par, err, 1);  // K landed
+    if (patch_k) {  // fused append: the token appended by this launch is not in the cache yet
+      if (lane < D / 8)
+        *reinterpret_cast<uint4*>(const_cast<unsigned char*>(T::at(Ks, valid - 1, lane))) =
+            __ldg(reinterpret_cast<const uint4*>(patch_k) + lane);
+      __syncwarp();
+    }
+  }
+  {
+    const int arow = (lane & 7) + ((lane >> 3) & 1) * 8, acol = lane >> 4;
+#pragma unroll
+    for (int m = 0; m < NM; ++m)
+#pragma unroll
+      for (int k16 = 0; k16 < D / 16; ++k16) {
+        uint32_t a[4];
+        ldmatrix_x4(a[0], a[1], a[2], a[3], T::at(Ks, m * 16 + arow, k16 * 2 + acol));
+        mma_bf16_16816(s[m], a, qb[k16][0], qb[k16][1]);
+      }
+  }
+  float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
+#pragma unroll
+  for (int m = 0; m < NM; ++m) {
+    const int t0 = m * 16 + r0;
+    if (t0 >= valid) { s[m][0] = -CUDART_INF_F; s[m][1] = -CUDART_INF_F; }
+    if (t0 + 8 >= valid) { s[m][2] = -CUDART_INF_F; s[m][3] = -CUDART_INF_F; }
+    mx0 = fmaxf(mx0, fmaxf(s[m][0], s[m][2]));
+    mx1 = fmaxf(mx1, fmaxf(s[m][1], s[m][3]));
+  }
+#pragma unroll
+  for (int off = 4; off <= 16; off <<= 1) {
+    mx0 = fmaxf(mx0, __shfl_xor_sync(FULL, mx0, off));
+    mx1 = fmaxf(mx1, __shfl_xor_sync(FULL, mx1, off));
+  }
+  const float off0 = mx0 * sl2, off1 = mx1 * sl2;  // valid >= 1: the maxima are finite
+  mt[0] = off0; mt[1] = off1;
+  if (first_pass) {
+    wait_bar(barV, par, err, 2);  // V landed
+    if (patch_v) {
+      if (lane < D / 8)
+        *reinterpret_cast<uint4*>(const_cast<unsigned char*>(T::at(Vs, valid - 1, lane))) =
+            __ldg(reinterpret_cast<const uint4*>(patch_v) + lane);
+    }
+    if (valid < ST) {  // open block: 0 * (whatever an unwritten slot holds) must not reach P V
+      for (int i = lane; i < (ST - valid) * T::NBOX * 8; i += 32) {
+        const int r = valid + i / (T::NBOX * 8), c = i % (T::NBOX * 8);
+        *reinterpret_cast<uint4*>(const_cast<unsigned char*>(Vs) + (c >> 3) * T::BOX_BYTES + r * 128 + ((c & 7) << 4)) =
+            make_uint4(0, 0, 0, 0);
+      }
+    }
+    __syncwarp();
+  }
+  float ls0 = 0.f, ls1 = 0.f;
+  const int vrow = (lane & 7) + ((lane >> 4) & 1) * 8, vcol = (lane >> 3) & 1;
+#pragma unroll
+  for (int kk = 0; kk < NM; ++kk) {
+    const float p0 = ex2(fmaf(s[kk][0], sl2, -off0)), p1 = ex2(fmaf(s[kk][1], sl2, -off1));
+    const float p2 = ex2(fmaf(s[kk][2], sl2, -off0)), p3 = ex2(fmaf(s[kk][3], sl2, -off1));
+    ls0 += p0 + p2;
+    ls1 += p1 + p3;
+    const uint32_t h01 = pack_bf16x2(p0, p1), h23 = pack_bf16x2(p2, p3);
+    const uint32_t l01 = pack_bf16x2(p0 - bf16_lo(h01), p1 - bf16_hi(h01));
+    const uint32_t l23 = pack_bf16x2(p2 - bf16_lo(h23), p3 - bf16_hi(h23));
+    const uint32_t bh0 = movmatrix_trans(h01), bh1 = movmatrix_trans(h23);
+    const uint32_t bl0 = movmatrix_trans(l01), bl1 = movmatrix_trans(l23);
+#pragma unroll
+    for (int dt = 0; dt < D / 16; ++dt) {
+      uint32_t a[4];
+      ldmatrix_x4_trans(a[0], a[1], a[2], a[3], T::at(Vs, kk * 16 + vrow, dt * 2 + vcol));
+      mma_bf16_16816(o[dt], a, bh0, bh1);
+      mma_bf16_16816(o[dt], a, bl0, bl1);
+    }
+  }
+#pragma unroll
+  for (int off = 4; off <= 16; off <<= 1) {
+    ls0 += __shfl_xor_sync(FULL, ls0, off);
+    ls1 += __shfl_xor_sync(FULL, ls1, off);
+  }
+  lt[0] = ls0; lt[1] = ls1;
+}
+
+// State image in shared memory (slots, warp running states, received partials): per query head
+// [m, l, -, -, O[D]] = D + 4 floats; the stride keeps the fragment stores conflict-free.
+// Fold a tile partial into a state (Eq. 6-8, unnormalised) or overwrite the state with it.
+template <int D>
+__device__ __forceinline__ void state_put(float* st, int G, int pass, const float (&o)[D / 16][4], const float (&mt)[2],
+                                          const float (&lt)[2], bool fold) {
+  const int lane = threadIdx.x & 31, r0 = lane >> 2, tq = lane & 3;
+  float al[2] = {0.f, 0.f}, be[2] = {1.f, 1.f}, mn[2], ln[2];
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const int g = pass * 8 + tq * 2 + j;
+    mn[j] = mt[j]; ln[j] = lt[j];
+    if (fold && g < G) {
+      const float mo = st[g * (D + 4)], lo = st[g * (D + 4) + 1];
+      mn[j] = fmaxf(mo, mt[j]);
+      al[j] = mo == -CUDART_INF_F ? 0.f : ex2(mo - mn[j]);
+      be[j] = ex2(mt[j] - mn[j]);
+      ln[j] = al[j] * lo + be[j] * lt[j];
+    }
+  }
+  __syncwarp();  // every lane has read the old m, l
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const int g = pass * 8 + tq * 2 + j;
+    if (g < G) {
+      float* row = st + g * (D + 4) + 4;
+#pragma unroll
+      for (int dt = 0; dt < D / 16; ++dt) {
+        const int d0 = dt * 16 + r0;
+        if (fold) {
+          row[d0] = al[j] * row[d0] + be[j] * o[dt][j];
+          row[d0 + 8] = al[j] * row[d0 + 8] + be[j] * o[dt][2 + j];
+        } else {
+          row[d0] = o[dt][j];
+          row[d0 + 8] = o[dt][2 + j];
+        }
+      }
+      if (r0 == 0) { st[g * (D + 4)] = mn[j]; st[g * (D + 4) + 1] = ln[j]; }
+    }
+  }
+  __syncwarp();
+}
+
+struct Sh {  // static shared memory
+  unsigned long long fullK[NBMAX], fullV[NBMAX], empty[NBMAX];
+  unsigned long long bar_keys, bar_pred, bar_red, bar_tw;
+  volatile int q_issued, q_total, q_final, sel_done, spec_ready, n_rep;
+  int q_next, n_slots, rep_cnt, ring_pos;
+  int chunk_cnt[NBMAX];
+  volatile int pos_unit[NBMAX];
+};
+
+// ---------------------------------------------------------------------------------------------
+template <int D, int ST>
+__global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs a) {
+  using T = Tile<D, ST>;
+  constexpr int LPR = D / 8, RW = 32 / LPR;  // lanes per summary row, rows per warp trip
+  constexpr int CHR = T::CHR;                // summary rows per ring buffer
+  constexpr int RPW = ((CHR + NSCW - 1) / NSCW + 3) & ~3;  // rows of a chunk per scoring warp (multiple of 4)
+  constexpr int SW = D + 4;                  // state row stride (floats)
+  static_assert(RPW * NSCW >= CHR && RPW <= 32, "chunk rows must fit the scoring warps");
+  extern __shared__ __align__(1024) unsigned char smem[];
+  __shared__ Sh sh;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int CS = a.CS, NBUF = a.NBUF;
+  const uint32_t rank = CS > 1 ? cluster_ctarank() : 0u;
+  uint32_t* err = a.ctl + CTL_ERR;
+
+  unsigned char* ring = smem;
+  uint32_t* keys = reinterpret_cast<uint32_t*>(smem + a.o_keys);
+  uint32_t* pkeys = reinterpret_cast<uint32_t*>(smem + a.o_pkeys);
+  uint32_t* hist = reinterpret_cast<uint32_t*>(smem + a.o_hist);  // [2][HB]
+  int32_t* plist = reinterpret_cast<int32_t*>(smem + a.o_plist);
+  uint32_t* pmask = reinterpret_cast<uint32_t*>(smem + a.o_pmask);
+  uint32_t* amask = reinterpret_cast<uint32_t*>(smem + a.o_amask);
+  uint32_t* offs = reinterpret_cast<uint32_t*>(smem + a.o_offs);  // [2][MBw]
+  int32_t* tslice = reinterpret_cast<int32_t*>(smem + a.o_tslice);
+  float* scs = reinterpret_cast<float*>(smem + a.o_sc);
+  int2* units = reinterpret_cast<int2*>(smem + a.o_units);
+  unsigned long long* cand = reinterpret_cast<unsigned long long*>(smem + a.o_cand);  // [2][CAND]
+  uint32_t* red = reinterpret_cast<uint32_t*>(smem + a.o_red);                        // [2][32]
+  float* slots = reinterpret_cast<float*>(smem + a.o_slots);  // [NSLOT + NTW][G][SW]
+  int32_t* slotblk = reinterpret_cast<int32_t*>(smem + a.o_slotblk);
+  float* recv = reinterpret_cast<float*>(smem + a.o_recv);    // [CS][HL][SW]
+  const int SLOTF = a.G * SW;  // floats per state image
+
+  if (tid == 0) {
+    for (int i = 0; i < NBUF; ++i) { mbar_init(&sh.fullK[i], 1); mbar_init(&sh.fullV[i], 1); mbar_init(&sh.empty[i], 1); }
+    mbar_init(&sh.bar_keys, 1); mbar_init(&sh.bar_pred, 1); mbar_init(&sh.bar_red, 1); mbar_init(&sh.bar_tw, NTW);
+    mbar_fence_init();
+    sh.ring_pos = 0;
+    for (int i = 0; i < NBMAX; ++i) sh.chunk_cnt[i] = 0;
+  }
+  for (int i = tid; i < 2 * HB; i += NTHR) hist[i] = 0u;
+  __syncthreads();
+  if (CS > 1) cluster_arrive();
+  // Programmatic dependent launch: let the next step's grid be scheduled (its CTAs take the SMs as
+  // ours exit and its launch latency hides behind this step); wait for the previous step's grid to
+  // have completed before the first global access.  No-ops without the launch attribute.
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");
+  unsigned long long* tl = a.tl ? a.tl + ((size_t)blockIdx.x * NWARP + warp) * 16 : nullptr;
+#define MARK(code) do { if (tl && lane == 0) tl[15] = (unsigned long long)(code); } while (0)
+  if (tl && lane == 0) {
+#pragma unroll
+    for (int i = 1; i < 16; ++i) tl[i] = 0;
+    tl[0] = gtime();
+  }
+  const int R = a.B * a.Hkv;
+  const int par_raw = __ldcg(a.parity);
+  const int32_t* Pcur = (par_raw & 1) ? a.P1 : a.P0;
+  int32_t* Pnext = (par_raw & 1) ? a.P0 : a.P1;
+  const int ncl = gridDim.x / CS;
+  bool waited = CS == 1;
+
+#pragma unroll 1
+  for (int it = 0, row = blockIdx.x / CS; row < R; ++it, row += ncl) {
+    const uint32_t ipar = it & 1;  // phase of the once-per-row barriers
+    const int b = row / a.Hkv, h = row - b * a.Hkv;
+    const int len = __ldcg(a.seq_lens + b) + a.app;
+    const int nb = max(0, min(a.MB, (len + a.bs - 1) / a.bs));
+    const int nb4 = (nb + 3) & ~3;
+    const int slice = ((nb4 + CS - 1) / CS + 3) & ~3;
+    const int s0 = min(nb4, (int)rank * slice), s1 = min(nb4, s0 + slice);
+    const int nrows = s1 - s0;                // rows of the summary buffer this CTA scores (multiple of 4)
+    const int NCH = (nrows + CHR - 1) / CHR;  // ring positions taken by summary chunks
+    const int pos0 = sh.ring_pos;             // ring position of chunk 0 (same in every thread: read after a barrier)
+    const int ob = len > 0 ? (len - 1) / a.bs : -1;  // the open block
+    const int ema_rank = CS - 1;
+    const int HLmine = (int)rank < a.G ? (a.G - (int)rank + CS - 1) / CS : 0;  // query heads this CTA reduces
+    const int n_spec = a.spec ? (a.Bud - (int)rank + CS - 1) / CS : 0;         // predicted slots dealt to this CTA
+    const int UREP0 = (a.Bud + CS - 1) / CS;                                   // first repair descriptor
+    const int NSUB = (a.bs + ST - 1) / ST;
+    const size_t rowoff = (size_t)row * a.MB;
+
+    if (tid == 0) {
+      sh.q_issued = pos0; sh.q_total = 0; sh.q_final = 0; sh.sel_done = 0; sh.spec_ready = 0; sh.n_rep = 0;
+      sh.q_next = pos0 + NCH; sh.n_slots = 0; sh.rep_cnt = 0;
+    }
+    // the table entries of the slice (repair units) and the initial warp states
+    for (int i = tid; i < nrows; i += NTHR) tslice[i] = s0 + i < nb ? __ldg(a.table + (size_t)b * a.MB + s0 + i) : 0;
+    for (int i = tid; i < NTW * SLOTF; i += NTHR) {
+      float* st = slots + (size_t)a.NSLOT * SLOTF;
+      const int c = i % SW;
+      st[i] = c == 0 ? -CUDART_INF_F : 0.f;
+    }
+    for (int i = tid; i < a.MBw; i += NTHR) { pmask[i] = 0u; amask[i] = 0u; }
+    __syncthreads();
+    if (!waited) { cluster_wait(); waited = true; }  // every CTA of the cluster has initialised its barriers
+
+    // =========================================================================================
+    MARK(100);
+    if (warp == LDW) {
+      // ---- loader warp: barriers armed, first summary chunks requested, then the predicted set is
+      // staged (list, bitmask, unit descriptors), then lane 0 feeds the ring until the row is done
+      int pos = pos0;
+      auto buf_acquire = [&](int p) -> int {  // (lane 0) ring position p -> buffer, once its previous tenant is consumed
+        const int bi = p % NBUF;
+        if (p >= NBUF) wait_bar(&sh.empty[bi], ((p / NBUF) - 1) & 1, err, 3);
+        return bi;
+      };
+      auto issue_chunk = [&](int c) {
+        const int bi = buf_acquire(pos);
+        const int rows = min(CHR, nrows - c * CHR);
+        const int rows_ld = max(0, min(rows, nb - (s0 + c * CHR)));  // rows past the last block are never scored
+        const uint32_t bytes = (uint32_t)rows_ld * D * 2;
+        fence_proxy_async();
+        mbar_expect_tx(&sh.fullV[bi], 0u);  // (both barriers of a buffer complete once per tenant)
+        mbar_expect_tx(&sh.fullK[bi], bytes);
+        if (bytes) bulk_load(ring + (size_t)bi * T::BYTES, a.summ + (rowoff + s0 + (size_t)c * CHR) * LPR, bytes, &sh.fullK[bi]);
+        sh.pos_unit[bi] = -1;
+        ++pos;
+      };
+      int cnext = 0;
+      if (lane == 0) {
+        mbar_expect_tx(&sh.bar_keys, (uint32_t)nb4 * 4u);
+        if ((int)rank == ema_rank) mbar_expect_tx(&sh.bar_pred, a.Bud > 0 ? (uint32_t)nb4 * 4u : 0u);
+        else mbar_arrive(&sh.bar_pred);
+        mbar_expect_tx(&sh.bar_red, (uint32_t)(CS * HLmine * SW * 4));
+        for (; cnext < NCH && cnext < NBUF; ++cnext) issue_chunk(cnext);
+      }
+      // the predicted set P (a3 of the previous step): list, bitmask, this CTA's unit descriptors
+      if (a.spec) {
+        const int32_t* P = Pcur + (size_t)row * a.Bud;
+#pragma unroll 1
+        for (int j0 = 0; j0 < a.Bud; j0 += 32) {
+          const int j = j0 + lane;
+          int blk = j < a.Bud ? __ldcg(P + j) : -1;
+          if (blk >= nb) blk = -1;
+          if (j < a.Bud) {
+            plist[j] = blk;
+            if (blk >= 0) atomicOr(&pmask[blk >> 5], 1u << (blk & 31));
+            if (j % CS == (int)rank) {
+              const int page = blk >= 0 ? __ldg(a.table + (size_t)b * a.MB + blk) : 0;
+              units[j / CS] = make_int2(blk, page);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) {
+        __threadfence_block();
+        sh.spec_ready = 1;
+        for (; cnext < NCH; ++cnext) issue_chunk(cnext);
+        auto issue_unit = [&](int u, bool rep) {
+          const int2 d = units[u];
+          for (int sub = 0; sub < NSUB; ++sub) {
+            const int valid = min(ST, len - d.x * a.bs - sub * ST);
+            if (valid <= 0) break;
+            const int bi = buf_acquire(pos);
+            unsigned char* Ks = ring + (size_t)bi * T::BYTES;
+            const int y = (d.y * a.Hkv + h) * a.bs + sub * ST;
+            sh.pos_unit[bi] = u | (sub << 20) | (rep ? 0x40000000 : 0);
+            fence_proxy_async();
+            mbar_expect_tx(&sh.fullK[bi], T::HALF);
+#pragma unroll
+            for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + i * T::BOX_BYTES, &a.mapK, i * 64, y, &sh.fullK[bi]);
+            mbar_expect_tx(&sh.fullV[bi], T::HALF);
+#pragma unroll
+            for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + T::HALF + i * T::BOX_BYTES, &a.mapV, i * 64, y, &sh.fullV[bi]);
+            ++pos;
+            __threadfence_block();
+            sh.q_issued = pos;
+          }
+        };
+        // speculative units (a4); once A is known a predicted block that missed is not requested (PRR_DROP)
+#pragma unroll 1
+        for (int u = 0; u < n_spec; ++u) {
+          const int blk = units[u].x;
+          if (blk < 0) continue;
+          if (a.cut && !a.retain && sh.sel_done) {
+            __threadfence_block();
+            if (!((amask[blk >> 5] >> (blk & 31)) & 1u)) continue;
+          }
+          issue_unit(u, false);
+        }
+        MARK(110);
+        wait_flag(&sh.sel_done, err, 4);
+        MARK(111);
+        __threadfence_block();
+        const int nrep = sh.n_rep;
+#pragma unroll 1
+        for (int i = 0; i < nrep; ++i) issue_unit(UREP0 + i, true);  // repair units (a6)
+        sh.q_total = pos;
+        __threadfence_block();
+        sh.q_final = 1;
+        MARK(112);
+      }
+      __syncwarp();
+      if (lane == 0) sh.ring_pos = pos;  // (read by everyone after the row's last barrier)
+    } else {
+      // ---- a0 + a1 + a8: score the slice, chunk by chunk ------------------------------------------
+      const int sub = lane / LPR, l = lane % LPR;
+      double qs[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) qs[j] = 0.0;
+      {
+        const uint16_t* qb = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D + l * 8;
+#pragma unroll 1
+        for (int g0 = 0; g0 < a.G; g0 += 4) {  // four query rows per batch of loads (zeros add nothing)
+          uint4 t[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            t[e] = g0 + e < a.G ? __ldg(reinterpret_cast<const uint4*>(qb + (size_t)(g0 + e) * D)) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const uint32_t w[4] = {t[e].x, t[e].y, t[e].z, t[e].w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              qs[2 * j] += (double)bf16_lo(w[j]);
+              qs[2 * j + 1] += (double)bf16_hi(w[j]);
+            }
+          }
+        }
+      }
+      const double alpha = a.theta[b * 3 + 0], beta = a.theta[b * 3 + 1], gamma = a.theta[b * 3 + 2];
+      const double oma = __dsub_rn(1.0, alpha), omb = __dsub_rn(1.0, beta);
+      const int n_old = a.n_state[row];
+      double* Lg = a.ema_l + rowoff;
+      double* Vg = a.ema_v + rowoff;
+      const uint32_t keys_a = smem_u32(keys), pkeys_a = smem_u32(pkeys);
+      const uint32_t bk_a = smem_u32(&sh.bar_keys), bp_a = smem_u32(&sh.bar_pred);
+      // EMA state of this lane's row of the NEXT chunk is requested one chunk ahead
+      auto my_row = [&](int c) { return s0 + c * CHR + warp * RPW + lane; };  // global block index (lane < RPW)
+      double el = 0.0, ev = 0.0;
+      if (NCH > 0 && lane < RPW) {
+        const int i = my_row(0);
+        if (warp * RPW + lane < min(CHR, nrows) && i < min(nb, n_old)) { el = Lg[i]; ev = Vg[i]; }
+      }
+#pragma unroll 1
+      for (int c = 0; c < NCH; ++c) {
+        const int p = pos0 + c, bi = p % NBUF;
+        const int rows_c = min(CHR, nrows - c * CHR);
+        const int w_lo = min(rows_c, warp * RPW), w_hi = min(rows_c, w_lo + RPW);
+        double nl = 0.0, nv = 0.0;
+        if (c + 1 < NCH && lane < RPW) {
+          const int i = my_row(c + 1);
+          if (warp * RPW + lane < min(CHR, nrows - (c + 1) * CHR) && i < min(nb, n_old)) { nl = Lg[i]; nv = Vg[i]; }
+        }
+        MARK(200 + c);
+        wait_bar(&sh.fullK[bi], (p / NBUF) & 1, err, 5);
+        if (tl && lane == 0 && c == 0) tl[6] = gtime();
+        uint4* st = reinterpret_cast<uint4*>(ring + (size_t)bi * T::BYTES);
+        if (a.app && ob >= s0 + c * CHR + w_lo && ob < s0 + c * CHR + w_hi) {
+          // a0: the warp that scores the block the new token falls in appends it: cache slot, running
+          // sum and mean-key summary (exact fp64 sum, one division, one RNE to bf16, Q2) -- and patches
+          // the summary row it has staged, so the score below is the score after the append.
+          if (sub == 0) {
+            const int pos_t = len - 1, slot = pos_t - ob * a.bs;
+            const size_t ch = ((size_t)b * a.Hkv + h) * D + l * 8;
+            const uint4 kn = __ldg(reinterpret_cast<const uint4*>(a.k_new + ch));
+            const uint4 vn = __ldg(reinterpret_cast<const uint4*>(a.v_new + ch));
+            const size_t page = (size_t)tslice[ob - s0];
+            const size_t dst = ((page * a.Hkv + h) * a.bs + slot) * (size_t)D + l * 8;
+            *reinterpret_cast<uint4*>(a.kp_w + dst) = kn;
+            *reinterpret_cast<uint4*>(a.vp_w + dst) = vn;
+            const uint32_t w[4] = {kn.x, kn.y, kn.z, kn.w};
+            uint32_t o[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const double x0 = (double)bf16_lo(w[j]), x1 = (double)bf16_hi(w[j]);
+              const double a0 = slot == 0 ? x0 : __dadd_rn(a.open_sum[ch + 2 * j], x0);
+              const double a1 = slot == 0 ? x1 : __dadd_rn(a.open_sum[ch + 2 * j + 1], x1);
+              a.open_sum[ch + 2 * j] = a0;
+              a.open_sum[ch + 2 * j + 1] = a1;
+              o[j] = (uint32_t)f64_to_bf16_rne(__ddiv_rn(a0, (double)(slot + 1))) |
+                     ((uint32_t)f64_to_bf16_rne(__ddiv_rn(a1, (double)(slot + 1))) << 16);
+            }
+            const uint4 rowv = make_uint4(o[0], o[1], o[2], o[3]);
+            st[(ob - s0 - c * CHR) * LPR + l] = rowv;
+            a.summ_w[(rowoff + ob) * LPR + l] = rowv;
+          }
+          __syncwarp();
+        }
+        // exact dot products (Q1): every partial sum is exact in fp64, so the order is free
+#pragma unroll 1
+        for (int r = w_lo + sub; r < w_lo + RPW; r += RW) {  // warp-uniform trip count (full-mask shuffles)
+          const uint4 v = r < w_hi ? st[r * LPR + l] : make_uint4(0, 0, 0, 0);
+          const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+          double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
+            a1 = fma((double)bf16_hi(w[j]), qs[2 * j + 1], a1);
+          }
+          double acc = a0 + a1;
+#pragma unroll
+          for (int off = LPR / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(FULL, acc, off);
+          if (l == 0 && r < w_hi) scs[c * CHR + r] = s0 + c * CHR + r < nb ? f64_to_score(__dmul_rn(acc, a.score_c)) : 0.f;
+        }
+        __syncwarp();
+        // this warp is done with the buffer
+        if (lane == 0) {
+          const int old = atomicAdd(&sh.chunk_cnt[bi], 1);
+          if (old == NSCW - 1) { sh.chunk_cnt[bi] = 0; mbar_arrive(&sh.empty[bi]); }
+        }
+        // a8 (Eq. 3) and the prediction for the next step (Eq. 2) for this lane's row; keys out
+        uint32_t key = 0u, pkey = 0u;
+        if (lane < w_hi - w_lo) {
+          const int i = s0 + c * CHR + w_lo + lane;
+          if (i < nb) {
+            const float sv = scs[c * CHR + w_lo + lane];
+            a.scores[rowoff + i] = sv;
+            key = score_key(sv);
+            const double xd = (double)sv;
+            double ln = xd, vn = 0.0;
+            if (i < n_old) {  // non-contracted fp64, both lines use l^{t-1} (Q5)
+              vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, el)), __dmul_rn(omb, ev));
+              ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, el));
+            }
+            Lg[i] = ln;
+            Vg[i] = vn;
+            pkey = score_key(f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn))));
+          }
+        }
+        el = nl; ev = nv;
+        {  // four consecutive keys per st.async: lane 4j gathers the keys of lanes 4j .. 4j+3
+          const uint32_t k1 = __shfl_down_sync(FULL, key, 1), k2 = __shfl_down_sync(FULL, key, 2), k3 = __shfl_down_sync(FULL, key, 3);
+          const uint32_t p1 = __shfl_down_sync(FULL, pkey, 1), p2 = __shfl_down_sync(FULL, pkey, 2), p3 = __shfl_down_sync(FULL, pkey, 3);
+          if ((lane & 3) == 0 && lane < w_hi - w_lo) {
+            const uint32_t off = (uint32_t)(s0 + c * CHR + w_lo + lane) * 4u;
+            if (CS > 1) {
+#pragma unroll 1
+              for (int r = 0; r < CS; ++r) st_async_v4(mapa(keys_a + off, r), key, k1, k2, k3, mapa(bk_a, r));
+              if (a.Bud > 0) st_async_v4(mapa(pkeys_a + off, ema_rank), pkey, p1, p2, p3, mapa(bp_a, ema_rank));
+            } else {
+              st_async_v4(keys_a + off, key, k1, k2, k3, bk_a);
+              if (a.Bud > 0) st_async_v4(pkeys_a + off, pkey, p1, p2, p3, bp_a);
+            }
+          }
+        }
+      }
+      if (tl && lane == 0) tl[1] = gtime();
+      MARK(300);
+
+      // =======================================================================================
+      if (warp < NTW) {
+        // ---- tile warps: a4 + a6.  Ring positions are claimed in order; a speculative partial whose
+        // fate is unknown is parked in a slot, everything else is folded into this warp's running state.
+        float* wst = slots + (size_t)(a.NSLOT + warp) * SLOTF;
+        const float sl2 = a.scale * LOG2E_F;
+        const int NG = (a.G + 7) >> 3;
+        uint32_t qb[2][D / 16][2];
+        {
+          const uint16_t* qg = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D;
+          const int r0 = lane >> 2, tq = lane & 3;
+#pragma unroll
+          for (int ps = 0; ps < 2; ++ps) {
+            const int g = ps * 8 + r0;
+#pragma unroll
+            for (int k16 = 0; k16 < D / 16; ++k16) {
+              const int col = k16 * 16 + tq * 2;
+              qb[ps][k16][0] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col)) : 0u;
+              qb[ps][k16][1] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col + 8)) : 0u;
+            }
+          }
+        }
+#pragma unroll 1
+        for (;;) {
+          int p = 0;
+          if (lane == 0) p = atomicAdd(&sh.q_next, 1);
+          p = __shfl_sync(FULL, p, 0);
+          bool done = false;
+          MARK(400 + (p & 63));
+          if (lane == 0) {  // wait until position p is in flight, or the queue is final and shorter
+            const unsigned long long t0 = gtime();
+            uint32_t itw = 0;
+            for (;;) {
+              if (p < sh.q_issued) break;
+              if (sh.q_final) { __threadfence_block(); if (p >= sh.q_total) { done = true; } break; }
+              __nanosleep(32);
+              if ((++itw & 1023u) == 0 && (long long)(gtime() - t0) > (long long)WAIT_NS) { wait_fail(err, 14); done = true; break; }
+            }
+          }
+          done = __shfl_sync(FULL, (int)done, 0) != 0;
+          if (done) break;
+          __threadfence_block();
+          const int bi = p % NBUF;
+          const uint32_t par = (p / NBUF) & 1;
+          const int pu = sh.pos_unit[bi];
+          const bool rep = (pu & 0x40000000) != 0;
+          const int u = pu & 0xfffff, sub_t = (pu >> 20) & 0x3ff;
+          const int2 d = units[u];
+          const int blk = d.x;
+          const int valid = min(ST, len - blk * a.bs - sub_t * ST);
+          unsigned char* Ks = ring + (size_t)bi * T::BYTES;
+          const bool patch = a.app && blk == ob && (len - 1 - ob * a.bs) / ST == sub_t;
+          const uint16_t* pk = patch ? a.k_new + ((size_t)b * a.Hkv + h) * D : nullptr;
+          const uint16_t* pv = patch ? a.v_new + ((size_t)b * a.Hkv + h) * D : nullptr;
+          // fate of a speculative unit: 1 merge, 0 drop, -1 unknown (park)
+          // (read by ONE lane and broadcast: the flag may flip between two lanes' reads, and the warp
+          // must take one path through the warp-synchronous tile code)
+          auto fate = [&]() -> int {
+            if (rep || a.retain) return 1;
+            int f = -1;
+            if (lane == 0 && sh.sel_done) {
+              __threadfence_block();
+              f = (int)((amask[blk >> 5] >> (blk & 31)) & 1u);
+            }
+            return __shfl_sync(FULL, f, 0);
+          };
+          MARK(500 + (p & 63));
+          int f = fate();
+          if (f == 0) {  // already known to be over-predicted: let the tile land, free the buffer
+            wait_bar(&sh.fullK[bi], par, err, 6);
+            wait_bar(&sh.fullV[bi], par, err, 7);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sh.empty[bi]);
+            continue;
+          }
+          float* dst = wst;
+          bool fold = true;
+          int slot = -1;
+#pragma unroll
+          for (int ps = 0; ps < 2; ++ps) {  // (unrolled: the query fragments stay in registers)
+            if (ps >= NG) break;
+            float o[D / 16][4], mt[2], lt[2];
+            tile_partial<D, ST>(Ks, &sh.fullK[bi], &sh.fullV[bi], par, qb[ps], valid, sl2, pk, pv, ps == 0, o, mt, lt, err);
+            if (ps == NG - 1) {  // every lane is done with the tile: the buffer may be refilled
+              __syncwarp();
+              if (lane == 0) mbar_arrive(&sh.empty[bi]);
+            }
+            if (ps == 0) {
+              f = fate();
+              if (f < 0) {  // park it, if a slot is left; else wait for A
+                if (lane == 0) slot = atomicAdd(&sh.n_slots, 1);
+                slot = __shfl_sync(FULL, slot, 0);
+                if (slot < a.NSLOT) {
+                  dst = slots + (size_t)slot * SLOTF;
+                  fold = false;
+                  if (lane == 0) slotblk[slot] = blk | (sub_t << 20);
+                } else {
+                  if (lane == 0) wait_flag(&sh.sel_done, err, 8);
+                  __syncwarp();
+                  f = fate();
+                }
+              }
+            }
+            if (f != 0) state_put<D>(dst, a.G, ps, o, mt, lt, fold);
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sh.bar_tw);
+        MARK(600);
+        if (tl && lane == 0) tl[4] = gtime();
+      } else if (warp < GA0 + GAW) {
+        // ---- group A: true top-K (a2), diff (a5), repair units, lists, merge (a7) ----------------------
+        const Grp g{tid - GA0 * 32, GAW * 32, warp - GA0, GAW, 1};
+        const SelMem m{hist, red, cand, offs};
+        MARK(700);
+        wait_bar(&sh.bar_keys, ipar, err, 9);
+        MARK(701);  // every CTA's keys have landed
+        if (tl && lane == 0) tl[7] = gtime();
+        if (g.tid == 0) wait_flag(&sh.spec_ready, err, 10);
+        g.sync();
+        const int k = min(a.K, nb);
+        Thr t;
+        t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
+        MARK(702);
+        if (k < nb) t = grp_kth(keys, nb, k, g, m);
+        MARK(703);
+        if (tl && lane == 0) tl[8] = gtime();
+        grp_mask(keys, nb, k, t, g, amask);
+        g.sync();
+        // repair units: the missed blocks of this CTA's slice (all of A's in the sequential path)
+        for (int i = s0 + g.tid; i < min(s1, nb); i += g.nt) {
+          const uint32_t bit = 1u << (i & 31);
+          if ((amask[i >> 5] & bit) && !(pmask[i >> 5] & bit)) {
+            const int pos = atomicAdd(&sh.rep_cnt, 1);
+            units[UREP0 + pos] = make_int2(i, tslice[i - s0]);
+          }
+        }
+        g.sync();
+        if (g.tid == 0) {
+          sh.n_rep = sh.rep_cnt;
+          __threadfence_block();
+          sh.sel_done = 1;
+        }
+        if (tl && lane == 0) tl[2] = gtime();
+        if (rank == 0) {  // the row's lists as the API reports them, off the critical path
+          const uint32_t tot = grp_emit(amask, pmask, nb, g, m, a.setA + (size_t)row * a.K, a.K,
+                                        a.setM + (size_t)row * a.K, a.K);
+          if (g.tid == 0) {
+            int np = 0;
+            for (int j = 0; j < (a.spec ? a.Bud : 0); ++j) np += plist[j] >= 0;
+            const int nA = (int)(tot >> 16), nM = (int)(tot & 0xffffu);
+            a.counts[row * 3 + 0] = nA;
+            a.counts[row * 3 + 1] = np;
+            a.counts[row * 3 + 2] = nM;
+            a.n_state[row] = nb;
+            if (a.stats) {
+              atomicAdd(&a.stats[0], (unsigned long long)nA);
+              atomicAdd(&a.stats[1], (unsigned long long)(nA - nM));
+              atomicAdd(&a.stats[2], (unsigned long long)nM);
+              atomicAdd(&a.stats[3], (unsigned long long)np);
+            }
+          }
+        }
+        // ---- merge: this CTA's hit slots and warp states per query head, then to the head's reducer
+        MARK(710);
+        wait_bar(&sh.bar_tw, ipar, err, 11);
+        MARK(711);
+        __threadfence_block();
+        if (tl && lane == 0) tl[3] = gtime();
+        const int nsl = min(sh.n_slots, a.NSLOT);
+        const uint32_t recv_a = smem_u32(recv), br_a = smem_u32(&sh.bar_red);
+#pragma unroll 1
+        for (int gq = g.wid; gq < a.G; gq += GAW) {
+          float mrun = -CUDART_INF_F, lrun = 0.f;
+          float4 acc[D / 128 > 0 ? D / 128 : 1];
+          constexpr int NV = D / 128 > 0 ? D / 128 : 1;
+          const bool on = lane * 4 < D;
+#pragma unroll
+          for (int v = 0; v < NV; ++v) acc[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+          for (int e = 0; e < nsl + NTW; ++e) {
+            if (e < nsl) {
+              const int blk = slotblk[e] & 0xfffff;
+              if (!a.retain && !((amask[blk >> 5] >> (blk & 31)) & 1u)) continue;
+            }
+            const float* st = slots + (size_t)(e < nsl ? e : a.NSLOT + (e - nsl)) * SLOTF + gq * SW;
+            const float me = st[0], le = st[1];
+            if (me == -CUDART_INF_F) continue;
+            const float mn = fmaxf(mrun, me);
+            const float fo = mrun == -CUDART_INF_F ? 0.f : ex2(mrun - mn), fn = ex2(me - mn);
+            lrun = fo * lrun + fn * le;
+            mrun = mn;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+              const float4 x = on ? *reinterpret_cast<const float4*>(st + 4 + v * 128 + lane * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+              acc[v].x = fo * acc[v].x + fn * x.x; acc[v].y = fo * acc[v].y + fn * x.y;
+              acc[v].z = fo * acc[v].z + fn * x.z; acc[v].w = fo * acc[v].w + fn * x.w;
+            }
+          }
+          const int rr = gq % CS, hl = gq / CS;
+          const uint32_t dsta = recv_a + (uint32_t)((rank * a.HL + hl) * SW) * 4u;
+          const uint32_t ra = CS > 1 ? mapa(dsta, rr) : dsta, rb = CS > 1 ? mapa(br_a, rr) : br_a;
+          if (lane == 0) st_async_v4(ra, __float_as_uint(mrun), __float_as_uint(lrun), 0u, 0u, rb);
+#pragma unroll
+          for (int v = 0; v < NV; ++v)
+            if (on) st_async_v4(ra + 16u + (uint32_t)(v * 128 + lane * 4) * 4u, __float_as_uint(acc[v].x), __float_as_uint(acc[v].y),
+                                __float_as_uint(acc[v].z), __float_as_uint(acc[v].w), rb);
+        }
+        // ---- reducer: fold the cluster's partials of this CTA's query heads, normalise, write out
+        if (HLmine > 0) {
+          MARK(720);
+          wait_bar(&sh.bar_red, ipar, err, 12);
+          MARK(721);
+#pragma unroll 1
+          for (int hl = g.wid; hl < HLmine; hl += GAW) {
+            const int gq = hl * CS + (int)rank;
+            constexpr int NV = D / 128 > 0 ? D / 128 : 1;
+            const bool on = lane * 4 < D;
+            float mrun = -CUDART_INF_F, lrun = 0.f;
+            float4 acc[NV];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) acc[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
+            for (int r = 0; r < CS; ++r) {
+              const float* st = recv + (size_t)(r * a.HL + hl) * SW;
+              const float me = st[0], le = st[1];
+              if (me == -CUDART_INF_F) continue;
+              const float mn = fmaxf(mrun, me);
+              const float fo = mrun == -CUDART_INF_F ? 0.f : ex2(mrun - mn), fn = ex2(me - mn);
+              lrun = fo * lrun + fn * le;
+              mrun = mn;
+#pragma unroll
+              for (int v = 0; v < NV; ++v) {
+                const float4 x = on ? *reinterpret_cast<const float4*>(st + 4 + v * 128 + lane * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+                acc[v].x = fo * acc[v].x + fn * x.x; acc[v].y = fo * acc[v].y + fn * x.y;
+                acc[v].z = fo * acc[v].z + fn * x.z; acc[v].w = fo * acc[v].w + fn * x.w;
+              }
+            }
+            const float inv = lrun > 0.f ? 1.f / lrun : 0.f;
+            float* op = a.out + ((size_t)b * a.Hq + (size_t)h * a.G + gq) * D;
+#pragma unroll
+            for (int v = 0; v < NV; ++v)
+              if (on) *reinterpret_cast<float4*>(op + v * 128 + lane * 4) =
+                  make_float4(acc[v].x * inv, acc[v].y * inv, acc[v].z * inv, acc[v].w * inv);
+          }
+        }
+        if (tl && lane == 0) tl[5] = gtime();
+      } else if ((int)rank == ema_rank && a.Bud > 0) {
+        // ---- group E: P of the next step = top-min(Bud, #stateful) of the Eq. 2 predictions (a3) -------
+        const Grp g{tid - GE0 * 32, GEW * 32, warp - GE0, GEW, 2};
+        const SelMem m{hist + HB, red + 32, cand + CAND, offs + a.MBw};
+        uint32_t* emask = offs + 2 * a.MBw;  // [MBw]
+        MARK(800);
+        wait_bar(&sh.bar_pred, ipar, err, 13);
+        MARK(801);
+        const int k = min(a.Bud, nb);
+        Thr t;
+        t.key = 0u; t.idx = 0x7fffffff;
+        if (k < nb) t = grp_kth(pkeys, nb, k, g, m);
+        grp_mask(pkeys, nb, k, t, g, emask);
+        g.sync();
+        grp_emit(emask, nullptr, nb, g, m, Pnext + (size_t)row * a.Bud, a.Bud, nullptr, 0);
+        if (tl && lane == 0) tl[9] = gtime();
+      }
+    }
+    MARK(900);
+    __syncthreads();  // the row is done in this CTA
+    MARK(901);
+    if (tl && lane == 0 && tl[5] == 0) tl[5] = gtime();
+  }
+  if (!waited) cluster_wait();
+  if (CS > 1) {  // nobody leaves while a peer may still be storing into the cluster's shared memory
+    cluster_arrive();
+    cluster_wait();
+    MARK(902);
+  }
+
+  // ---- exit: the last CTA of the grid flips the parity and bumps the lengths -------------------
+  if (tid == 0) {
+    __threadfence();
+    const uint32_t last = atomicAdd(&a.ctl[CTL_EXIT], 1u) == gridDim.x - 1 ? 1u : 0u;
+    if (last) {
+      a.ctl[CTL_EXIT] = 0u;
+      *a.parity = par_raw ^ 1;
+      if (a.app)
+        for (int b = 0; b < a.B; ++b) a.seq_lens_w[b] += 1;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+struct RowPlan { int CS, NBUF, NSLOT, smem; };
+
+template <int D, int ST>
+static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
+  using T = Tile<D, ST>;
+  const int R = a.B * a.Hkv;
+  const void* fn = (const void*)k_row<D, ST>;
+  const int key = (D == 128 ? 0 : 1) * 3 + (ST == 64 ? 0 : ST == 32 ? 1 : 2);
+  if (!c->row_attr[key]) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return e;
+    c->row_dyn[key] = c->smem_optin - (int)fa.sharedSizeBytes;
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->row_dyn[key]);
+    if (e != cudaSuccess) return e;
+    // clusters of 1, 2, 4, 8 CTAs that can be co-resident with the whole shared memory of an SM each
+    for (int i = 0; i < 4; ++i) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((1 << i) * 8); cfg.blockDim = dim3(NTHR);
+      cfg.dynamicSmemBytes = c->row_dyn[key];
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 1 << i; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      int n = 0;
+      if (cudaOccupancyMaxActiveClusters(&n, fn, &cfg) != cudaSuccess) { cudaGetLastError(); n = i == 0 ? c->n_sm : 0; }
+      c->row_maxcl[key][i] = n;
+    }
+    c->row_attr[key] = 1;
+  }
+  // the largest cluster that still gives every row its own cluster in one wave
+  int CS = 1;
+  for (int i = 3; i >= 0; --i)
+    if (c->row_maxcl[key][i] >= R) { CS = 1 << i; break; }
+  if (c->force_cs > 0) CS = c->force_cs;
+  int li = 0; while ((1 << li) < CS) ++li;
+  const int ncl = std::max(1, std::min(R, c->row_maxcl[key][li] > 0 ? c->row_maxcl[key][li] : 1));
+  if (CS > 1 && ncl < R) return cudaErrorInvalidConfiguration;
+  a.CS = CS;
+  a.HL = (a.G + CS - 1) / CS;
+  a.UCAP = (a.Bud + CS - 1) / CS + a.K;
+  a.SLMAX = ((((a.MB + 3) & ~3) + CS - 1) / CS + 3 + 4) & ~3;
+  const int SW = D + 4, SLOTF = a.G * SW;
+  a.NSLOT = 8;
+  const int budget = c->row_dyn[key];
+  int NBUF = NBMAX;
+  for (;;) {
+    int o = NBUF * T::BYTES;
+    auto take = [&](int bytes) { const int at = o; o += (bytes + 15) & ~15; return at; };
+    a.o_keys = take((a.MB + 8) * 4);
+    a.o_pkeys = take((a.MB + 8) * 4);
+    a.o_hist = take(2 * HB * 4);
+    a.o_plist = take(std::max(1, a.Bud) * 4);
+    a.o_pmask = take(a.MBw * 4);
+    a.o_amask = take(a.MBw * 4);
+    a.o_offs = take(3 * a.MBw * 4);
+    a.o_tslice = take(a.SLMAX * 4);
+    a.o_sc = take((a.SLMAX + T::CHR) * 4);
+    a.o_units = take(a.UCAP * 8);
+    a.o_cand = take(2 * CAND * 8);
+    a.o_red = take(2 * 32 * 4);
+    a.o_slots = take((a.NSLOT + NTW) * SLOTF * 4);
+    a.o_slotblk = take(a.NSLOT * 4);
+    a.o_recv = take(CS * a.HL * SW * 4);
+    a.o_end = o;
+    if (o <= budget) break;
+    if (NBUF > 2) { --NBUF; continue; }
+    if (a.NSLOT > 1) { a.NSLOT /= 2; NBUF = NBMAX; continue; }
+    return cudaErrorInvalidConfiguration;
+  }
+  a.NBUF = NBUF;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(ncl * CS);
+  cfg.blockDim = dim3(NTHR);
+  cfg.dynamicSmemBytes = a.o_end;
+  cfg.stream = s;
+  cudaLaunchAttribute at[2];
+  int na = 0;
+  {  // (also for one CTA per row: st.async needs a cluster launch)
+    at[na].id = cudaLaunchAttributeClusterDimension;
+    at[na].val.clusterDim.x = CS; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
+    ++na;
+  }
+  if (c->pdl) {
+    at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  cfg.attrs = at; cfg.numAttrs = na;
+  c->last_cs = CS; c->last_nbuf = NBUF; c->last_grid = ncl * CS;
+  return cudaLaunchKernelEx(&cfg, k_row<D, ST>, a);
+}
+
+// Tensor map of a K or V page pool for the copy engine: bf16 [rows, d] with rows = page * Hkv * bs
+// (the library is not told n_pages; tile coordinates are int32, so the row extent is 2^31), box =
+// [ST rows, 64 channels = 128 bytes], 128-byte swizzle.  Encoded on the host, cached per pointer.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess) p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+static int page_map(prr_ctx* c, const void* base, int box_rows, CUtensorMap* out) {
+  static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap is 128 bytes");
+  auto it = c->tmaps.find(base);
+  if (it == c->tmaps.end()) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return (int)cudaErrorNotSupported;
+    alignas(64) CUtensorMap m;
+    const cuuint64_t dims[2] = {(cuuint64_t)c->D, (cuuint64_t)1 << 31};
+    const cuuint64_t strides[1] = {(cuuint64_t)c->D * 2};
+    const cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
+    const cuuint32_t es[2] = {1u, 1u};
+    if (fn(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return (int)cudaErrorInvalidValue;
+    std::array<uint64_t, 16> blob;
+    memcpy(blob.data(), &m, 128);
+    if (c->tmaps.size() > 4096) c->tmaps.clear();
+    it = c->tmaps.emplace(base, blob).first;
+  }
+  memcpy(out, it->second.data(), 128);
+  return 0;
+}
+
+int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
+                int spec, cudaStream_t s, const void* k_new, const void* v_new) {
+  const size_t r = (size_t)kv->layer * c->maxB * c->Hkv;
+  const int ST = std::min(c->bs, 64);
+  RowArgs a{};
+  if (int e = page_map(c, kv->k_pages, ST, &a.mapK)) return e;
+  if (int e = page_map(c, kv->v_pages, ST, &a.mapV)) return e;
+  a.table = kv->block_table; a.seq_lens = kv->seq_lens;
+  a.app = (k_new && v_new) ? 1 : 0;
+  a.k_new = (const uint16_t*)k_new; a.v_new = (const uint16_t*)v_new;
+  a.kp_w = (uint16_t*)kv->k_pages; a.vp_w = (uint16_t*)kv->v_pages; a.summ_w = (uint4*)summaries;
+  a.open_sum = c->open_sum + (size_t)kv->layer * c->maxB * c->Hkv * c->D; a.seq_lens_w = (int32_t*)kv->seq_lens;
+  a.q = (const uint16_t*)q; a.summ = (const uint4*)summaries; a.out = out;
+  a.scores = c->scores + r * c->MB;
+  a.ema_l = c->ema_l + r * c->MB; a.ema_v = c->ema_v + r * c->MB;
+  a.n_state = c->n_state + r;
+  a.theta = c->theta + (size_t)kv->layer * c->maxB * 3;
+  a.P0 = c->Pbuf[0] + r * c->Bud; a.P1 = c->Pbuf[1] + r * c->Bud; a.parity = c->parity + kv->layer;
+  a.setA = c->setA + r * c->K; a.setM = c->setM + r * c->K; a.counts = c->counts + r * 3;
+  a.ctl = c->ctl; a.stats = c->stats;
+  a.tl = c->tl_on ? c->tl : nullptr;
+  a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32 + 1;
+  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud;
+  a.retain = c->lay.overpredict_policy == PRR_RETAIN;
+  a.spec = (spec && c->Bud > 0) ? 1 : 0;
+  a.cut = c->cut;
+  a.scale = c->sm_scale; a.score_c = c->score_c;
+  cudaError_t e = cudaErrorInvalidValue;
+#define PRR_CASE(DD, SS) if (c->D == DD && ST == SS) e = plan_and_launch<DD, SS>(c, a, s);
+  PRR_CASE(128, 64) PRR_CASE(128, 32) PRR_CASE(128, 16)
+  PRR_CASE(64, 64) PRR_CASE(64, 32) PRR_CASE(64, 16)
+#undef PRR_CASE
+  c->launches++;
+  return e == cudaSuccess ? 0 : (int)e;
+}
+
+}  // namespace prr

@@ -132,7 +132,11 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->ms64, srows * (size_t)(c->Bud + c->K)));
   A(dalloc(c, &c->ctl, (size_t)10 + srows * ((size_t)3 + c->Bud + c->K + c->MB)));  // header + flag arrays (k_step.cu)
   c->tl_warps = c->n_sm * 32;
-  A(dalloc(c, &c->tl, (size_t)c->tl_warps * 16));
+  {  // phase stamps live in pinned, device-mapped HOST memory: readable while a step runs or after a fault
+    void* p = nullptr;
+    if (e == cudaSuccess) e = cudaHostAlloc(&p, (size_t)c->tl_warps * 16 * sizeof(unsigned long long), cudaHostAllocMapped);
+    if (e == cudaSuccess) { memset(p, 0, (size_t)c->tl_warps * 16 * sizeof(unsigned long long)); c->tl = (unsigned long long*)p; }
+  }
   A(dalloc(c, &c->merge_src, srows * (c->Bud + c->K)));
   A(dalloc(c, &c->merge_n, srows));
   A(dalloc(c, &c->nblk, (size_t)c->maxB));
@@ -188,6 +192,7 @@ extern "C" int32_t prr_destroy(prr_ctx* c) {
   cudaDeviceSynchronize();
   for (void* p : c->allocs) cudaFree(p);
   if (c->st_pin) cudaFreeHost(c->st_pin);
+  if (c->tl) cudaFreeHost(c->tl);
   if (c->cal_state) cudaFree(c->cal_state);
   if (c->cal_mask) cudaFree(c->cal_mask);
   if (c->cal_den) cudaFree(c->cal_den);
@@ -643,11 +648,37 @@ extern "C" int32_t prr_check(prr_ctx* ctx, void* stream) {
   if (!ctx) return PRR_E_INVALID;
   cudaStream_t s = (cudaStream_t)stream;
   join_updates(ctx, s);
-  uint32_t err = 0;
-  PRR_CUDA(ctx, cudaMemcpyAsync(&err, ctx->ctl + 1, sizeof(err), cudaMemcpyDeviceToHost, s));
+  uint32_t err[4] = {0, 0, 0, 0};  // ctl[1] error flag ... ctl[4] first wait site that gave up (k_row.cu)
+  PRR_CUDA(ctx, cudaMemcpyAsync(err, ctx->ctl + 1, sizeof(err), cudaMemcpyDeviceToHost, s));
   PRR_CUDA(ctx, cudaStreamSynchronize(s));
-  if (err) PRR_FAIL(ctx, PRR_E_STATE, "prr_check: a fused step gave up waiting on a dependency counter");
+  if (err[0])
+    PRR_FAIL(ctx, PRR_E_STATE, "prr_check: a fused step gave up waiting on a dependency (site %u, CTA %u, warp %u)",
+             err[3] & 0xffu, (err[3] >> 8) & 0xfffu, err[3] >> 20);
   return check_launch(ctx, "prr_check");
+}
+
+extern "C" int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value) {
+  if (!ctx) return PRR_E_INVALID;
+  switch (option) {
+    case PRR_OPT_PDL: if (value != 0 && value != 1) break; ctx->pdl = value; return PRR_OK;
+    case PRR_OPT_CLUSTER: if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break; ctx->force_cs = value; return PRR_OK;
+    case PRR_OPT_CUT: if (value != 0 && value != 1) break; ctx->cut = value; return PRR_OK;
+    default: break;
+  }
+  PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_option: unknown option %d or bad value %d", option, value);
+}
+
+extern "C" int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* value_out) {
+  if (!ctx || !value_out) return PRR_E_INVALID;
+  switch (option) {
+    case PRR_OPT_PDL: *value_out = ctx->pdl; return PRR_OK;
+    case PRR_OPT_CLUSTER: *value_out = ctx->force_cs; return PRR_OK;
+    case PRR_OPT_CUT: *value_out = ctx->cut; return PRR_OK;
+    case PRR_OPT_LAST_CLUSTER: *value_out = ctx->last_cs; return PRR_OK;
+    case PRR_OPT_LAST_RING: *value_out = ctx->last_nbuf; return PRR_OK;
+    case PRR_OPT_LAST_GRID: *value_out = ctx->last_grid; return PRR_OK;
+    default: return PRR_E_INVALID;
+  }
 }
 
 extern "C" int32_t prr_timeline_enable(prr_ctx* ctx, int32_t on) {
@@ -662,8 +693,17 @@ extern "C" int32_t prr_timeline_read(prr_ctx* ctx, uint64_t* stamps_host, int32_
   if (!stamps_host || max_warps < 1) PRR_FAIL(ctx, PRR_E_INVALID, "prr_timeline_read: bad argument");
   cudaStream_t s = (cudaStream_t)stream;
   const int n = max_warps < ctx->tl_warps ? max_warps : ctx->tl_warps;
-  PRR_CUDA(ctx, cudaMemcpyAsync(stamps_host, ctx->tl, (size_t)n * 16 * sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  memcpy(stamps_host, ctx->tl, (size_t)n * 16 * sizeof(uint64_t));
+  if (n_warps_out) *n_warps_out = n;
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_timeline_peek(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps, int32_t* n_warps_out) {
+  if (!ctx) return PRR_E_INVALID;
+  if (!stamps_host || max_warps < 1) PRR_FAIL(ctx, PRR_E_INVALID, "prr_timeline_peek: bad argument");
+  const int n = max_warps < ctx->tl_warps ? max_warps : ctx->tl_warps;
+  memcpy(stamps_host, ctx->tl, (size_t)n * 16 * sizeof(uint64_t));
   if (n_warps_out) *n_warps_out = n;
   return PRR_OK;
 }

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libprr.so")
 
 OK, E_INVALID, E_UNSUPPORTED, E_STATE, E_CUDA, E_NOMEM = range(6)
 DROP, RETAIN = 0, 1
+OPT_PDL, OPT_CLUSTER, OPT_CUT, OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID = 0, 1, 2, 16, 17, 18
 FUSED, STREAMS = 0, 1
 
 SYMBOLS = [
@@ -23,7 +24,7 @@ SYMBOLS = [
     "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_step_append",
     "prr_decode_step_host",
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
-    "prr_timeline_enable", "prr_timeline_read",
+    "prr_timeline_enable", "prr_timeline_read", "prr_timeline_peek", "prr_set_option", "prr_get_option",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
 ]
 
@@ -244,6 +245,14 @@ class Context:
     def launch_count(self) -> int:
         return int(lib().prr_launch_count(self._h))
 
+    def set_option(self, option: int, value: int):
+        self._chk(lib().prr_set_option(self._h, int(option), int(value)))
+
+    def get_option(self, option: int) -> int:
+        v = C.c_int32(0)
+        self._chk(lib().prr_get_option(self._h, int(option), C.byref(v)))
+        return int(v.value)
+
     def timeline_enable(self, on=True):
         self._chk(lib().prr_timeline_enable(self._h, int(on)))
 
@@ -254,6 +263,14 @@ class Context:
         n = C.c_int32(0)
         self._chk(lib().prr_timeline_read(self._h, buf.ctypes.data_as(C.c_void_p), max_warps, C.byref(n),
                                           C.c_void_p(_stream(stream))))
+        return buf[:n.value]
+
+    def timeline_peek(self, max_warps=8192):
+        """timeline_read without synchronising (the stamps live in pinned host memory)."""
+        import numpy as np
+        buf = np.zeros((max_warps, 16), dtype=np.uint64)
+        n = C.c_int32(0)
+        self._chk(lib().prr_timeline_peek(self._h, buf.ctypes.data_as(C.c_void_p), max_warps, C.byref(n)))
         return buf[:n.value]
 
     # -- graphs ------------------------------------------------------------------------------

@@ -402,8 +402,8 @@ def test_graph_replay_matches_eager():
         graph = g2.ctx.graph_end(s)
         graph.launch(s)
     s.synchronize()
-    for t in range(4):
-        assert torch.equal(outs_e[t], outs_g[t]), t
+    for t in range(4):   # (the fold order of the partial states follows the tile arrival order: equal to fp32 rounding, not bitwise)
+        assert (outs_e[t] - outs_g[t]).abs().max().item() <= 2e-6, t
     assert g2.seq_lens.tolist() == gl.seq_lens.tolist()
     graph.destroy()
 
@@ -418,7 +418,7 @@ def test_host_buffer_step_matches_device_step():
                                 inp.k_new[t].cpu().contiguous().pin_memory(),
                                 inp.v_new[t].cpu().contiguous().pin_memory(), g2.summ, out_h)
         torch.cuda.synchronize()
-        assert torch.equal(o.cpu(), out_h)
+        assert (o.cpu() - out_h).abs().max().item() <= 2e-6
 
 
 def test_errors_are_reported_not_raised_in_c():
