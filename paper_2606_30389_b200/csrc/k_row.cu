@@ -38,11 +38,11 @@ namespace prr {
 
 constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr int NWARP = 12, NTHR = 32 * NWARP;
-constexpr int NTW = 5;             // tile warps 0 .. 4
-constexpr int GA0 = 5, GAW = 4;    // group A (true top-K, lists, merge): warps 5 .. 8, named barrier 1
-constexpr int GE0 = 9, GEW = 2;    // group E (next prediction): warps 9 .. 10, named barrier 2
+constexpr int SCW = 8;             // warps 0 .. 7 score; afterwards:
+constexpr int GA0 = 0, GAW = 4;    //   group A (true top-K, lists, merge): warps 0 .. 3, named barrier 1
+constexpr int GE0 = 4, GEW = 2;    //   group E (next prediction): warps 4 .. 5, named barrier 2
+constexpr int TW0 = 6, NTW = 5;    // tile warps 6 .. 10 (8 .. 10 from the start, 6 and 7 once they have scored)
 constexpr int LDW = 11;            // loader warp: predicted-set staging, then every bulk / TMA request
-constexpr int NSCW = 11;           // warps 0 .. 10 score
 constexpr int NBMAX = 12;          // ring buffers at most
 constexpr int HB = 1024;           // histogram buckets of a selection pass
 constexpr int CAND = 128;          // survivors that are ranked directly
@@ -64,7 +64,7 @@ struct RowArgs {
   int32_t* setA; int32_t* setM; int32_t* counts;
   uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, retain, spec, cut;
-  int CS, NBUF, NSLOT, UCAP, HL, SLMAX;
+  int CS, NBUF, NSLOT, UCAP, HL, SLMAX, NBH;
   // dynamic shared memory offsets (bytes)
   int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
       o_slots, o_slotblk, o_recv, o_end;
@@ -90,7 +90,7 @@ __device__ __forceinline__ void st_async_v4(uint32_t raddr, uint32_t a, uint32_t
 __device__ __forceinline__ bool mbar_try_wait_cl(unsigned long long* bar, uint32_t parity) {
   uint32_t done;
   asm volatile(
-      "{ .reg .pred p; mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }\n"
+      "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }\n"
       : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
   return done != 0;
 }
@@ -156,7 +156,7 @@ struct SelMem {
 // Highest bucket b with  sum_{b' >= b} hist[b'] >= need  (1 <= need <= total); `above` = the count
 // in the buckets over b.  Thread t owns the buckets [HB-(t+1)per, HB-t*per): a prefix scan over
 // threads is a suffix scan over buckets.  Every thread zeroes what it read and returns the triple.
-__device__ void grp_pick(const Grp& g, const SelMem& m, int need, int& bstar, int& cstar, int& above) {
+__device__ __noinline__ void grp_pick(const Grp& g, const SelMem& m, int need, int& bstar, int& cstar, int& above) {
   const int lane = threadIdx.x & 31;
   uint32_t* dec = m.red + g.nw * 2;
   const int per = (HB + g.nt - 1) / g.nt;
@@ -192,9 +192,10 @@ __device__ void grp_pick(const Grp& g, const SelMem& m, int need, int& bstar, in
 }
 
 // keys[0 .. n), 1 <= k < n.
-__device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const SelMem& m) {
+__device__ __noinline__ Thr grp_kth_cont(const uint32_t* keys, int n, const Grp& g, const SelMem& m, uint32_t lo, uint32_t span,
+                                         int need, int cnt_in, unsigned long long* tl);
+__device__ __noinline__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const SelMem& m, unsigned long long* tl = nullptr) {
   const int lane = threadIdx.x & 31;
-  uint32_t* dec = m.red + g.nw * 2;
   // the exact key range of the row
   uint32_t kmin = 0xffffffffu, kmax = 0u;
 #pragma unroll 4
@@ -206,8 +207,14 @@ __device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const S
 #pragma unroll 1
   for (int w = 0; w < g.nw; ++w) { kmin = min(kmin, m.red[w * 2]); kmax = max(kmax, m.red[w * 2 + 1]); }
   g.sync();
-  uint32_t lo = kmin, span = kmax - kmin;
-  int need = k, cnt_in = n;
+  if (tl && lane == 0) tl[10] = gtime();
+  return grp_kth_cont(keys, n, g, m, kmin, kmax - kmin, k, n, tl);
+}
+// Range narrowing from a known state (see the invariant below).
+__device__ __noinline__ Thr grp_kth_cont(const uint32_t* keys, int n, const Grp& g, const SelMem& m, uint32_t lo, uint32_t span,
+                                         int need, int cnt_in, unsigned long long* tl) {
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + g.nw * 2;
   Thr r;
   // invariant: the threshold key lies in [lo, lo+span]; `need` of the cnt_in keys in that range are
   // selected, every key above it is
@@ -242,6 +249,7 @@ __device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const S
         }
       }
       g.sync();
+      if (tl && lane == 0) tl[13] = gtime();
 #pragma unroll 1
       for (int e = g.tid; e < cnt_in; e += g.nt) {
         const unsigned long long ce = m.cand[e];
@@ -262,8 +270,10 @@ __device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const S
       if (d <= span) atomicAdd(&m.hist[d >> sh], 1u);
     }
     g.sync();
+    if (tl && lane == 0 && tl[11] == 0) tl[11] = gtime();
     int bstar, cstar, above;
     grp_pick(g, m, need, bstar, cstar, above);
+    if (tl && lane == 0 && tl[12] == 0) tl[12] = gtime();
     need -= above;
     cnt_in = cstar;
     const uint32_t off = (uint32_t)bstar << sh;
@@ -275,7 +285,7 @@ __device__ Thr grp_kth(const uint32_t* keys, int n, int k, const Grp& g, const S
 }
 
 // Bitmask of the selected blocks into mask[0 .. nwd) (shared), one ballot per 32 blocks.
-__device__ __forceinline__ void grp_mask(const uint32_t* keys, int n, int k, const Thr& t, const Grp& g, uint32_t* mask) {
+__device__ __noinline__ void grp_mask(const uint32_t* keys, int n, int k, const Thr& t, const Grp& g, uint32_t* mask) {
   const int lane = threadIdx.x & 31;
   const int nwd = (n + 31) >> 5;
 #pragma unroll 2
@@ -287,9 +297,132 @@ __device__ __forceinline__ void grp_mask(const uint32_t* keys, int n, int k, con
   }
 }
 
+__device__ __forceinline__ float key_value(uint32_t key) {  // inverse of score_key (key 0 = NaN -> -inf)
+  if (key == 0u) return -CUDART_INF_F;
+  return __uint_as_float((key & 0x80000000u) ? (key & 0x7fffffffu) : ~key);
+}
+
+// Selection without a histogram, for k <= NT (a group of NT threads, n <= NT * KR keys in registers).
+// Shared-memory atomics run at about one lane per clock, so a histogram over all n keys costs n clocks;
+// plain compares on registers do not.  A LOWER BOUND of the k-th largest key comes from the per-thread
+// maxima: if every warp's r-th largest thread maximum is >= L, with r = ceil(k / #warps), then at least k
+// distinct keys are >= L.  Only the keys >= L (a few more than k) are collected (one atomic per warp)
+// and ranked exactly.  Everything is branch-free predicated code: a lone warp issues a dependent
+// instruction every ~10 clocks, so the instruction count per thread IS the latency.
+constexpr int CANDX = 256;
+__device__ __forceinline__ bool selected_bf(uint32_t key, int i, uint32_t tkey, int tidx) {  // (no short circuit)
+  return (key > tkey) | ((key == tkey) & (i <= tidx));
+}
+#ifndef PRR_SEL_INLINE
+#define PRR_SEL_INLINE __forceinline__
+#endif
+template <int NT, int KR>
+__device__ PRR_SEL_INLINE void grp_select_v3(const uint32_t* keys, int n, int k, const Grp& g, const SelMem& m, uint32_t* mask,
+                                           unsigned long long* tl) {
+  constexpr int NW = NT / 32;
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + NW * 2;
+  uint32_t kr[KR];
+  uint32_t tmax = 0u;
+#pragma unroll
+  for (int e = 0; e < KR; ++e) {
+    const int i = g.tid + e * NT;
+    kr[e] = keys[min(i, n - 1)];
+    kr[e] = i < n ? kr[e] : 0u;
+    tmax = max(tmax, kr[e]);
+  }
+  uint32_t tkey = 0u;
+  int tidx = 0x7fffffff;  // k >= n: everything is selected
+  if (k < n) {            // (uniform)
+    // the warp's r-th largest thread maximum: r rounds of (max, retire its lowest lane)
+    const int r = (k + NW - 1) / NW;  // <= 32
+    uint32_t v = tmax, wl = 0u;
+#pragma unroll 1
+    for (int j = 0; j < r; ++j) {
+      wl = __reduce_max_sync(FULL, v);
+      const uint32_t eq = __ballot_sync(FULL, v == wl);
+      v = lane == __ffs(eq) - 1 ? 0u : v;
+    }
+    if (lane == 0) m.red[g.wid] = wl;
+    if (g.tid == 0) dec[7] = 0u;
+    g.sync();
+    uint32_t L = 0xffffffffu;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) L = min(L, m.red[w]);
+    if (tl && lane == 0) tl[10] = gtime();
+    // survivors: per-thread bitmask, warp prefix, ONE atomic per warp
+    uint32_t cm = 0u;
+#pragma unroll
+    for (int e = 0; e < KR; ++e) cm |= (uint32_t)((g.tid + e * NT < n) & (kr[e] >= L)) << e;
+    const int mine = __popc(cm);
+    int incl = mine;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int x = __shfl_up_sync(FULL, incl, off);
+      incl += lane >= off ? x : 0;
+    }
+    int base = 0;
+    if (lane == 31) base = (int)atomicAdd(&dec[7], (uint32_t)incl);
+    base = __shfl_sync(FULL, base, 31) + incl - mine;
+#pragma unroll
+    for (int e = 0; e < KR; ++e)
+      if ((cm >> e) & 1u) {
+        if (base < CANDX) m.cand[base] = ((unsigned long long)kr[e] << 32) | (uint32_t)~(g.tid + e * NT);
+        ++base;
+      }
+    g.sync();
+    const int c = (int)dec[7];
+    if (tl && lane == 0) tl[11] = gtime();
+    if (c > CANDX) {  // (ties, or rows shorter than the group): the generic narrowing
+      g.sync();
+      const Thr t = grp_kth(keys, n, k, g, m, nullptr);
+      tkey = t.key; tidx = t.idx;
+    } else {
+      // exact rank of every survivor, its c comparisons split over NT / P2 threads (P2 = c rounded up to a power of two)
+      int P2 = 32;
+      while (P2 < c && P2 < NT) P2 <<= 1;
+      if (c > NT) {  // more survivors than threads: a thread ranks several, each against all
+#pragma unroll 1
+        for (int j = g.tid; j < c; j += NT) {
+          const unsigned long long ce = m.cand[j];
+          int rk = 0;
+#pragma unroll 4
+          for (int f = 0; f < c; ++f) rk += m.cand[f] > ce;
+          if (rk == k - 1) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }
+        }
+      }
+      const int parts = NT / P2, j = g.tid & (P2 - 1), part = g.tid / P2;
+      const int per = (c + parts - 1) / parts, f0 = part * per, f1 = min(c, f0 + per);
+      const unsigned long long ce = m.cand[min(j, c - 1)];
+      int rk = 0;
+#pragma unroll 4
+      for (int f = f0; f < f1; ++f) rk += m.cand[f] > ce;
+      if (parts > 1) {  // partial ranks meet in shared memory (offs[] is free until the lists are emitted)
+        if (g.tid < CANDX) m.offs[g.tid] = 0u;
+        g.sync();
+        if (j < c) atomicAdd(&m.offs[j], (uint32_t)rk);
+        g.sync();
+        rk = (int)m.offs[j & (CANDX - 1)];
+      }
+      if ((c <= NT) & (j < c) & (part == 0) & (rk == k - 1)) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }  // exactly one
+      g.sync();
+      tkey = dec[5]; tidx = (int)dec[6];
+    }
+  }
+  if (tl && lane == 0) tl[14] = gtime();
+  const int nwd = (n + 31) >> 5;
+  const bool kpos = k > 0;
+#pragma unroll
+  for (int e = 0; e < KR; ++e) {  // lanes of a warp hold 32 consecutive blocks: one mask word per (warp, e)
+    const int i = g.tid + e * NT, w = e * NW + g.wid;
+    const uint32_t bal = __ballot_sync(FULL, (i < n) & kpos & selected_bf(kr[e], i, tkey, tidx));
+    if ((lane == 0) & (w < nwd)) mask[w] = bal;
+  }
+}
+
 // Ordered emission from a bitmask: the set bits ascending into list[width] (padded with -1); with
 // Mlist != null also the set bits NOT in pmask (ascending, padded to widthM).  Returns (nA << 16) | nM.
-__device__ uint32_t grp_emit(const uint32_t* mask, const uint32_t* pmask, int n, const Grp& g, const SelMem& m,
+__device__ __noinline__ uint32_t grp_emit(const uint32_t* mask, const uint32_t* pmask, int n, const Grp& g, const SelMem& m,
                              int32_t* list, int width, int32_t* Mlist, int widthM) {
   const int lane = threadIdx.x & 31;
   const uint32_t lt = (1u << lane) - 1u;
@@ -510,7 +643,7 @@ struct Sh {  // static shared memory
   unsigned long long fullK[NBMAX], fullV[NBMAX], empty[NBMAX];
   unsigned long long bar_keys, bar_pred, bar_red, bar_tw;
   volatile int q_issued, q_total, q_final, sel_done, spec_ready, n_rep;
-  int q_next, n_slots, rep_cnt, ring_pos;
+  int t_next, n_slots, rep_cnt, ring_pos;
   int chunk_cnt[NBMAX];
   volatile int pos_unit[NBMAX];
 };
@@ -521,9 +654,10 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
   using T = Tile<D, ST>;
   constexpr int LPR = D / 8, RW = 32 / LPR;  // lanes per summary row, rows per warp trip
   constexpr int CHR = T::CHR;                // summary rows per ring buffer
-  constexpr int RPW = ((CHR + NSCW - 1) / NSCW + 3) & ~3;  // rows of a chunk per scoring warp (multiple of 4)
+  constexpr int RPW = CHR / SCW;             // rows of a chunk per scoring warp (4, 8 or 16)
+  constexpr int NV = RPW / RW;               // rows per lane group and chunk
   constexpr int SW = D + 4;                  // state row stride (floats)
-  static_assert(RPW * NSCW >= CHR && RPW <= 32, "chunk rows must fit the scoring warps");
+  static_assert(RPW * SCW == CHR && RPW % 4 == 0 && NV >= 1 && NV <= LPR, "chunk rows must fit the scoring warps");
   extern __shared__ __align__(1024) unsigned char smem[];
   __shared__ Sh sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -555,26 +689,70 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
     mbar_fence_init();
     sh.ring_pos = 0;
     for (int i = 0; i < NBMAX; ++i) sh.chunk_cnt[i] = 0;
+    sh.q_issued = 0;
   }
   for (int i = tid; i < 2 * HB; i += NTHR) hist[i] = 0u;
+  // per-row state; set again at the end of a row if another one follows (nothing here depends on the row,
+  // so the first requests of a row wait for nothing but its length)
+  auto row_init = [&]() {
+    if (tid == 0) {
+      sh.q_total = 0; sh.q_final = 0; sh.sel_done = 0; sh.spec_ready = 0; sh.n_rep = 0;
+      sh.t_next = 0; sh.n_slots = 0; sh.rep_cnt = 0;
+    }
+    for (int i = tid; i < NTW * SLOTF; i += NTHR) slots[(size_t)a.NSLOT * SLOTF + i] = (i % SW) == 0 ? -CUDART_INF_F : 0.f;
+    for (int i = tid; i < a.MBw; i += NTHR) { pmask[i] = 0u; amask[i] = 0u; }
+  };
+  row_init();
   __syncthreads();
   if (CS > 1) cluster_arrive();
   // Programmatic dependent launch: let the next step's grid be scheduled (its CTAs take the SMs as
   // ours exit and its launch latency hides behind this step); wait for the previous step's grid to
   // have completed before the first global access.  No-ops without the launch attribute.
   asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+  {  // While the previous grid drains: prefetch (L2 is the point of coherence, so a line the previous grid
+     // still writes is simply written again) the first row's summary slice, EMA state, table slice and
+     // the control words.  Every one of these is otherwise a TLB miss + HBM miss at the head of the step.
+    const int row = blockIdx.x / CS;
+    if (row < a.B * a.Hkv) {
+      const int b = row / a.Hkv;
+      const int nb4 = (a.NBH + 3) & ~3;
+      const int slice = ((nb4 + CS - 1) / CS + 3) & ~3;
+      const int s0 = min(nb4, (int)rank * slice), s1 = min(min(nb4, s0 + slice), a.MB);
+      const size_t rowoff = (size_t)row * a.MB;
+      auto pf = [](const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); };
+      const char* sp = reinterpret_cast<const char*>(a.summ) + (rowoff + s0) * (size_t)(D * 2);
+      const int nline = max(0, s1 - s0) * (D * 2) / 128;
+#pragma unroll 1
+      for (int i = tid; i < nline; i += NTHR) pf(sp + (size_t)i * 128);
+      const int nl8 = (max(0, s1 - s0) * 8 + 127) / 128;  // lines of a double-per-block slice
+      if (warp == 8)
+#pragma unroll 1
+        for (int i = lane; i < nl8; i += 32) { pf(reinterpret_cast<const char*>(a.ema_l + rowoff + s0) + i * 128); pf(reinterpret_cast<const char*>(a.ema_v + rowoff + s0) + i * 128); }
+      if (warp == 9)
+#pragma unroll 1
+        for (int i = lane; i < (nl8 + 1) / 2; i += 32) pf(reinterpret_cast<const char*>(a.table + (size_t)b * a.MB + s0) + i * 128);
+      if (warp == 10) {
+#pragma unroll 1
+        for (int i = lane; i < (a.Bud * 4 + 127) / 128; i += 32) { pf(reinterpret_cast<const char*>(a.P0 + (size_t)row * a.Bud) + i * 128); pf(reinterpret_cast<const char*>(a.P1 + (size_t)row * a.Bud) + i * 128); }
+        if (lane == 0) { pf(a.seq_lens + b); pf(a.parity); pf(a.theta + b * 3); pf(a.n_state + row); pf(a.ctl); }
+        if (a.app && lane >= 8 && lane < 8 + (D * 8 + 127) / 128) pf(reinterpret_cast<const char*>(a.open_sum + (size_t)row * D) + (lane - 8) * 128);
+      }
+    }
+  }
   asm volatile("griddepcontrol.wait;\n" ::: "memory");
-  unsigned long long* tl = a.tl ? a.tl + ((size_t)blockIdx.x * NWARP + warp) * 16 : nullptr;
-#define MARK(code) do { if (tl && lane == 0) tl[15] = (unsigned long long)(code); } while (0)
+  // phase stamps are collected in shared memory and written out at exit (the buffer is host memory);
+  // the progress mark [15] goes out at once, so it survives a hang
+  __shared__ unsigned long long stamps[NWARP][16];
+  unsigned long long* tlg = a.tl ? a.tl + ((size_t)blockIdx.x * NWARP + warp) * 16 : nullptr;
+  unsigned long long* tl = a.tl ? stamps[warp] : nullptr;
+#define MARK(code) do { if (tlg && lane == 0) tlg[15] = (unsigned long long)(code); } while (0)
   if (tl && lane == 0) {
 #pragma unroll
     for (int i = 1; i < 16; ++i) tl[i] = 0;
     tl[0] = gtime();
   }
   const int R = a.B * a.Hkv;
-  const int par_raw = __ldcg(a.parity);
-  const int32_t* Pcur = (par_raw & 1) ? a.P1 : a.P0;
-  int32_t* Pnext = (par_raw & 1) ? a.P0 : a.P1;
+  const int par_raw = __ldcg(a.parity);  // (in flight: first used when the predicted set is staged)
   const int ncl = gridDim.x / CS;
   bool waited = CS == 1;
 
@@ -582,75 +760,94 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
   for (int it = 0, row = blockIdx.x / CS; row < R; ++it, row += ncl) {
     const uint32_t ipar = it & 1;  // phase of the once-per-row barriers
     const int b = row / a.Hkv, h = row - b * a.Hkv;
-    const int len = __ldcg(a.seq_lens + b) + a.app;
-    const int nb = max(0, min(a.MB, (len + a.bs - 1) / a.bs));
-    const int nb4 = (nb + 3) & ~3;
+    const int len_ld = __ldcg(a.seq_lens + b);  // in flight; first USED below, after the requests that do not need it
+    // The row's blocks are dealt to the CTAs by the STATIC bound NBH >= ceil(len / bs) (the caller's
+    // max_blocks_per_seq or hint), so the summary requests go out without waiting for the length; rows
+    // past the last block are fetched but never scored.
+    const int nb4 = (a.NBH + 3) & ~3;
     const int slice = ((nb4 + CS - 1) / CS + 3) & ~3;
     const int s0 = min(nb4, (int)rank * slice), s1 = min(nb4, s0 + slice);
     const int nrows = s1 - s0;                // rows of the summary buffer this CTA scores (multiple of 4)
     const int NCH = (nrows + CHR - 1) / CHR;  // ring positions taken by summary chunks
     const int pos0 = sh.ring_pos;             // ring position of chunk 0 (same in every thread: read after a barrier)
-    const int ob = len > 0 ? (len - 1) / a.bs : -1;  // the open block
     const int ema_rank = CS - 1;
     const int HLmine = (int)rank < a.G ? (a.G - (int)rank + CS - 1) / CS : 0;  // query heads this CTA reduces
     const int n_spec = a.spec ? (a.Bud - (int)rank + CS - 1) / CS : 0;         // predicted slots dealt to this CTA
     const int UREP0 = (a.Bud + CS - 1) / CS;                                   // first repair descriptor
     const int NSUB = (a.bs + ST - 1) / ST;
     const size_t rowoff = (size_t)row * a.MB;
-
-    if (tid == 0) {
-      sh.q_issued = pos0; sh.q_total = 0; sh.q_final = 0; sh.sel_done = 0; sh.spec_ready = 0; sh.n_rep = 0;
-      sh.q_next = pos0 + NCH; sh.n_slots = 0; sh.rep_cnt = 0;
+    // requests that do not depend on the length, all in flight together (each may be a TLB miss + HBM miss)
+    uint4 qpre[4] = {};
+    double th0 = 0.0, th1 = 0.0, th2 = 0.0;
+    int n_old = 0;
+    if (warp < SCW) {
+      const uint16_t* qb = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D + (lane % LPR) * 8;
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (e < a.G) qpre[e] = __ldg(reinterpret_cast<const uint4*>(qb + (size_t)e * D));
+      th0 = a.theta[b * 3 + 0]; th1 = a.theta[b * 3 + 1]; th2 = a.theta[b * 3 + 2];
+      n_old = a.n_state[row];
     }
-    // the table entries of the slice (repair units) and the initial warp states
-    for (int i = tid; i < nrows; i += NTHR) tslice[i] = s0 + i < nb ? __ldg(a.table + (size_t)b * a.MB + s0 + i) : 0;
-    for (int i = tid; i < NTW * SLOTF; i += NTHR) {
-      float* st = slots + (size_t)a.NSLOT * SLOTF;
-      const int c = i % SW;
-      st[i] = c == 0 ? -CUDART_INF_F : 0.f;
+    int ppre0[4] = {-1, -1, -1, -1}, ppre1[4] = {-1, -1, -1, -1};  // both prediction buffers: the parity is in flight too
+    if (warp == LDW && a.spec) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int j = e * 32 + lane;
+        if (j < a.Bud) { ppre0[e] = __ldcg(a.P0 + (size_t)row * a.Bud + j); ppre1[e] = __ldcg(a.P1 + (size_t)row * a.Bud + j); }
+      }
     }
-    for (int i = tid; i < a.MBw; i += NTHR) { pmask[i] = 0u; amask[i] = 0u; }
-    __syncthreads();
-    if (!waited) { cluster_wait(); waited = true; }  // every CTA of the cluster has initialised its barriers
+    int pos = pos0, cnext = 0;
+    auto buf_acquire = [&](int p) -> int {  // (loader lane 0) ring position p -> buffer, once its previous tenant is consumed
+      const int bi = p % NBUF;
+      if (p >= NBUF) { wait_bar(&sh.empty[bi], ((p / NBUF) - 1) & 1, err, 3); fence_proxy_async(); }
+      return bi;
+    };
+    auto issue_chunk = [&](int c) {
+      const int bi = buf_acquire(pos);
+      const int rows = min(CHR, nrows - c * CHR);
+      const int rows_ld = max(0, min(rows, a.MB - (s0 + c * CHR)));  // (stay inside the row of the summary buffer)
+      const uint32_t bytes = (uint32_t)rows_ld * D * 2;
+      mbar_expect_tx(&sh.fullV[bi], 0u);  // (both barriers of a buffer complete once per tenant)
+      mbar_expect_tx(&sh.fullK[bi], bytes);
+      if (bytes) bulk_load(ring + (size_t)bi * T::BYTES, a.summ + (rowoff + s0 + (size_t)c * CHR) * LPR, bytes, &sh.fullK[bi]);
+      sh.pos_unit[bi] = -1;
+      ++pos;
+    };
+    if (warp == LDW && lane == 0) {
+      mbar_expect_tx(&sh.bar_keys, (uint32_t)nb4 * 4u);
+      if ((int)rank == ema_rank) mbar_expect_tx(&sh.bar_pred, a.Bud > 0 ? (uint32_t)nb4 * 4u : 0u);
+      else mbar_arrive(&sh.bar_pred);
+      mbar_expect_tx(&sh.bar_red, (uint32_t)(CS * HLmine * SW * 4));
+      for (; cnext < NCH && cnext < NBUF; ++cnext) issue_chunk(cnext);
+      if (tl) tl[11] = gtime();
+    }
+    const int len = len_ld + a.app;
+    const int nb = max(0, min(a.NBH, (len + a.bs - 1) / a.bs));
+    const int ob = len > 0 ? (len - 1) / a.bs : -1;  // the open block
+    if (tl && lane == 0 && warp == LDW) tl[10] = gtime();
+    // (every remote store is preceded by the cluster barrier: all CTAs have initialised their mbarriers)
 
     // =========================================================================================
     MARK(100);
     if (warp == LDW) {
-      // ---- loader warp: barriers armed, first summary chunks requested, then the predicted set is
-      // staged (list, bitmask, unit descriptors), then lane 0 feeds the ring until the row is done
-      int pos = pos0;
-      auto buf_acquire = [&](int p) -> int {  // (lane 0) ring position p -> buffer, once its previous tenant is consumed
-        const int bi = p % NBUF;
-        if (p >= NBUF) wait_bar(&sh.empty[bi], ((p / NBUF) - 1) & 1, err, 3);
-        return bi;
-      };
-      auto issue_chunk = [&](int c) {
-        const int bi = buf_acquire(pos);
-        const int rows = min(CHR, nrows - c * CHR);
-        const int rows_ld = max(0, min(rows, nb - (s0 + c * CHR)));  // rows past the last block are never scored
-        const uint32_t bytes = (uint32_t)rows_ld * D * 2;
-        fence_proxy_async();
-        mbar_expect_tx(&sh.fullV[bi], 0u);  // (both barriers of a buffer complete once per tenant)
-        mbar_expect_tx(&sh.fullK[bi], bytes);
-        if (bytes) bulk_load(ring + (size_t)bi * T::BYTES, a.summ + (rowoff + s0 + (size_t)c * CHR) * LPR, bytes, &sh.fullK[bi]);
-        sh.pos_unit[bi] = -1;
-        ++pos;
-      };
-      int cnext = 0;
-      if (lane == 0) {
-        mbar_expect_tx(&sh.bar_keys, (uint32_t)nb4 * 4u);
-        if ((int)rank == ema_rank) mbar_expect_tx(&sh.bar_pred, a.Bud > 0 ? (uint32_t)nb4 * 4u : 0u);
-        else mbar_arrive(&sh.bar_pred);
-        mbar_expect_tx(&sh.bar_red, (uint32_t)(CS * HLmine * SW * 4));
-        for (; cnext < NCH && cnext < NBUF; ++cnext) issue_chunk(cnext);
-      }
+      // ---- loader warp: the barriers are armed and the first summary chunks requested (above); now the
+      // predicted set is staged (list, bitmask, unit descriptors), then lane 0 feeds the ring until the row is done
+      if (!waited) { cluster_wait(); waited = true; }
       // the predicted set P (a3 of the previous step): list, bitmask, this CTA's unit descriptors
       if (a.spec) {
-        const int32_t* P = Pcur + (size_t)row * a.Bud;
+        const int32_t* P = ((par_raw & 1) ? a.P1 : a.P0) + (size_t)row * a.Bud;
 #pragma unroll 1
         for (int j0 = 0; j0 < a.Bud; j0 += 32) {
           const int j = j0 + lane;
-          int blk = j < a.Bud ? __ldcg(P + j) : -1;
+          int blk = -1;
+          if (j0 < 128) {
+            const int e = j0 >> 5;
+            const int v0 = e == 0 ? ppre0[0] : e == 1 ? ppre0[1] : e == 2 ? ppre0[2] : ppre0[3];
+            const int v1 = e == 0 ? ppre1[0] : e == 1 ? ppre1[1] : e == 2 ? ppre1[2] : ppre1[3];
+            blk = (par_raw & 1) ? v1 : v0;
+          } else if (j < a.Bud) {
+            blk = __ldcg(P + j);
+          }
           if (blk >= nb) blk = -1;
           if (j < a.Bud) {
             plist[j] = blk;
@@ -666,6 +863,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
       if (lane == 0) {
         __threadfence_block();
         sh.spec_ready = 1;
+        if (tl) tl[12] = gtime();
         for (; cnext < NCH; ++cnext) issue_chunk(cnext);
         auto issue_unit = [&](int u, bool rep) {
           const int2 d = units[u];
@@ -676,7 +874,6 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             unsigned char* Ks = ring + (size_t)bi * T::BYTES;
             const int y = (d.y * a.Hkv + h) * a.bs + sub * ST;
             sh.pos_unit[bi] = u | (sub << 20) | (rep ? 0x40000000 : 0);
-            fence_proxy_async();
             mbar_expect_tx(&sh.fullK[bi], T::HALF);
 #pragma unroll
             for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + i * T::BOX_BYTES, &a.mapK, i * 64, y, &sh.fullK[bi]);
@@ -714,8 +911,14 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
       __syncwarp();
       if (lane == 0) sh.ring_pos = pos;  // (read by everyone after the row's last barrier)
     } else {
-      // ---- a0 + a1 + a8: score the slice, chunk by chunk ------------------------------------------
+      if (warp < SCW) {
+      // ---- a0 + a1 + a8: score the slice, chunk by chunk (warps 0 .. 7, RPW rows of a chunk each) -----
       const int sub = lane / LPR, l = lane % LPR;
+      // the table entries of the slice, for group A's repair units (its own threads fill them)
+      if (warp < GAW)
+        for (int i = tid; i < nrows; i += GAW * 32) tslice[i] = s0 + i < nb ? __ldg(a.table + (size_t)b * a.MB + s0 + i) : 0;
+      const bool own_ob = a.app && ob >= s0 && ob < s1;  // this CTA appends the new token
+      const int page_ob = own_ob ? __ldg(a.table + (size_t)b * a.MB + ob) : 0;
       double qs[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) qs[j] = 0.0;
@@ -726,7 +929,8 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           uint4 t[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e)
-            t[e] = g0 + e < a.G ? __ldg(reinterpret_cast<const uint4*>(qb + (size_t)(g0 + e) * D)) : make_uint4(0, 0, 0, 0);
+            t[e] = g0 == 0 ? qpre[e]
+                           : (g0 + e < a.G ? __ldg(reinterpret_cast<const uint4*>(qb + (size_t)(g0 + e) * D)) : make_uint4(0, 0, 0, 0));
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const uint32_t w[4] = {t[e].x, t[e].y, t[e].z, t[e].w};
@@ -738,35 +942,25 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           }
         }
       }
-      const double alpha = a.theta[b * 3 + 0], beta = a.theta[b * 3 + 1], gamma = a.theta[b * 3 + 2];
+      const double alpha = th0, beta = th1, gamma = th2;
       const double oma = __dsub_rn(1.0, alpha), omb = __dsub_rn(1.0, beta);
-      const int n_old = a.n_state[row];
       double* Lg = a.ema_l + rowoff;
       double* Vg = a.ema_v + rowoff;
-      const uint32_t keys_a = smem_u32(keys), pkeys_a = smem_u32(pkeys);
-      const uint32_t bk_a = smem_u32(&sh.bar_keys), bp_a = smem_u32(&sh.bar_pred);
-      // EMA state of this lane's row of the NEXT chunk is requested one chunk ahead
-      auto my_row = [&](int c) { return s0 + c * CHR + warp * RPW + lane; };  // global block index (lane < RPW)
-      double el = 0.0, ev = 0.0;
-      if (NCH > 0 && lane < RPW) {
-        const int i = my_row(0);
-        if (warp * RPW + lane < min(CHR, nrows) && i < min(nb, n_old)) { el = Lg[i]; ev = Vg[i]; }
-      }
+      const uint32_t keys_a = smem_u32(keys), bk_a = smem_u32(&sh.bar_keys);
+      const int w_lo = warp * RPW;  // this warp's first row inside a chunk
+      if (!waited) { cluster_wait(); waited = true; }
 #pragma unroll 1
       for (int c = 0; c < NCH; ++c) {
         const int p = pos0 + c, bi = p % NBUF;
-        const int rows_c = min(CHR, nrows - c * CHR);
-        const int w_lo = min(rows_c, warp * RPW), w_hi = min(rows_c, w_lo + RPW);
-        double nl = 0.0, nv = 0.0;
-        if (c + 1 < NCH && lane < RPW) {
-          const int i = my_row(c + 1);
-          if (warp * RPW + lane < min(CHR, nrows - (c + 1) * CHR) && i < min(nb, n_old)) { nl = Lg[i]; nv = Vg[i]; }
-        }
+        const int rows_c = min(CHR, nrows - c * CHR);  // (multiple of 4)
+        const int g0r = s0 + c * CHR;                  // global block index of the chunk's row 0
         MARK(200 + c);
+        if (tl && lane == 0 && c == 0) tl[14] = gtime();
         wait_bar(&sh.fullK[bi], (p / NBUF) & 1, err, 5);
         if (tl && lane == 0 && c == 0) tl[6] = gtime();
+        if (tl && lane == 0 && c == 1 && warp >= 4) tl[12] = gtime();
         uint4* st = reinterpret_cast<uint4*>(ring + (size_t)bi * T::BYTES);
-        if (a.app && ob >= s0 + c * CHR + w_lo && ob < s0 + c * CHR + w_hi) {
+        if (own_ob && ob >= g0r + w_lo && ob < g0r + min(rows_c, w_lo + RPW)) {
           // a0: the warp that scores the block the new token falls in appends it: cache slot, running
           // sum and mean-key summary (exact fp64 sum, one division, one RNE to bf16, Q2) -- and patches
           // the summary row it has staged, so the score below is the score after the append.
@@ -775,8 +969,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             const size_t ch = ((size_t)b * a.Hkv + h) * D + l * 8;
             const uint4 kn = __ldg(reinterpret_cast<const uint4*>(a.k_new + ch));
             const uint4 vn = __ldg(reinterpret_cast<const uint4*>(a.v_new + ch));
-            const size_t page = (size_t)tslice[ob - s0];
-            const size_t dst = ((page * a.Hkv + h) * a.bs + slot) * (size_t)D + l * 8;
+            const size_t dst = (((size_t)page_ob * a.Hkv + h) * a.bs + slot) * (size_t)D + l * 8;
             *reinterpret_cast<uint4*>(a.kp_w + dst) = kn;
             *reinterpret_cast<uint4*>(a.vp_w + dst) = vn;
             const uint32_t w[4] = {kn.x, kn.y, kn.z, kn.w};
@@ -792,15 +985,21 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
                      ((uint32_t)f64_to_bf16_rne(__ddiv_rn(a1, (double)(slot + 1))) << 16);
             }
             const uint4 rowv = make_uint4(o[0], o[1], o[2], o[3]);
-            st[(ob - s0 - c * CHR) * LPR + l] = rowv;
+            st[(ob - g0r) * LPR + l] = rowv;
             a.summ_w[(rowoff + ob) * LPR + l] = rowv;
           }
           __syncwarp();
         }
-        // exact dot products (Q1): every partial sum is exact in fp64, so the order is free
-#pragma unroll 1
-        for (int r = w_lo + sub; r < w_lo + RPW; r += RW) {  // warp-uniform trip count (full-mask shuffles)
-          const uint4 v = r < w_hi ? st[r * LPR + l] : make_uint4(0, 0, 0, 0);
+        // Exact dot products (Q1): every partial sum is exact in fp64, so the order is free.  Lane group
+        // `sub` takes the rows w_lo + e RW + sub, e < NV, all requested and converted before the first
+        // shuffle; the NV partial sums per lane are folded across the LPR lanes by a transposed butterfly
+        // (each step halves what a lane carries), then a plain butterfly over the remaining lanes.
+        if (w_lo < rows_c) {  // (warp-uniform)
+        double acc[NV];
+#pragma unroll
+        for (int e = 0; e < NV; ++e) {
+          const int r = w_lo + e * RW + sub;
+          const uint4 v = r < rows_c ? st[r * LPR + l] : make_uint4(0, 0, 0, 0);
           const uint32_t w[4] = {v.x, v.y, v.z, v.w};
           double a0 = 0.0, a1 = 0.0;
 #pragma unroll
@@ -808,82 +1007,144 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             a0 = fma((double)bf16_lo(w[j]), qs[2 * j], a0);
             a1 = fma((double)bf16_hi(w[j]), qs[2 * j + 1], a1);
           }
-          double acc = a0 + a1;
+          acc[e] = a0 + a1;
+        }
+        int eidx = 0;
+        {
+          int off = LPR / 2;
 #pragma unroll
-          for (int off = LPR / 2; off >= 1; off >>= 1) acc += __shfl_xor_sync(FULL, acc, off);
-          if (l == 0 && r < w_hi) scs[c * CHR + r] = s0 + c * CHR + r < nb ? f64_to_score(__dmul_rn(acc, a.score_c)) : 0.f;
+          for (int nvv = NV; nvv > 1; nvv >>= 1, off >>= 1) {
+            const bool up = (l & off) != 0;
+#pragma unroll
+            for (int j = 0; j < nvv / 2; ++j)
+              acc[j] = (up ? acc[nvv / 2 + j] : acc[j]) + __shfl_xor_sync(FULL, up ? acc[j] : acc[nvv / 2 + j], off);
+            eidx += up ? nvv / 2 : 0;
+          }
+#pragma unroll
+          for (; off >= 1; off >>= 1) acc[0] += __shfl_xor_sync(FULL, acc[0], off);
+        }
+        {
+          const int r = w_lo + eidx * RW + sub;
+          if ((l & (LPR / NV - 1)) == 0 && r < rows_c)
+            scs[c * CHR + r] = g0r + r < nb ? f64_to_score(__dmul_rn(acc[0], a.score_c)) : 0.f;
+        }
         }
         __syncwarp();
+        if (tl && lane == 0 && warp >= 4 && c < 2) tl[c == 0 ? 10 : 13] = gtime();
         // this warp is done with the buffer
         if (lane == 0) {
           const int old = atomicAdd(&sh.chunk_cnt[bi], 1);
-          if (old == NSCW - 1) { sh.chunk_cnt[bi] = 0; mbar_arrive(&sh.empty[bi]); }
+          if (old == SCW - 1) { sh.chunk_cnt[bi] = 0; mbar_arrive(&sh.empty[bi]); }
         }
-        // a8 (Eq. 3) and the prediction for the next step (Eq. 2) for this lane's row; keys out
-        uint32_t key = 0u, pkey = 0u;
-        if (lane < w_hi - w_lo) {
-          const int i = s0 + c * CHR + w_lo + lane;
+        // keys out: one st.async of four consecutive keys per (group of four rows, destination CTA) pair,
+        // one pair per lane
+        uint32_t key = 0u;
+        if (lane < RPW && w_lo + lane < rows_c) {
+          const int i = g0r + w_lo + lane;
           if (i < nb) {
             const float sv = scs[c * CHR + w_lo + lane];
             a.scores[rowoff + i] = sv;
             key = score_key(sv);
-            const double xd = (double)sv;
-            double ln = xd, vn = 0.0;
-            if (i < n_old) {  // non-contracted fp64, both lines use l^{t-1} (Q5)
-              vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, el)), __dmul_rn(omb, ev));
-              ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, el));
-            }
-            Lg[i] = ln;
-            Vg[i] = vn;
-            pkey = score_key(f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn))));
           }
         }
-        el = nl; ev = nv;
-        {  // four consecutive keys per st.async: lane 4j gathers the keys of lanes 4j .. 4j+3
-          const uint32_t k1 = __shfl_down_sync(FULL, key, 1), k2 = __shfl_down_sync(FULL, key, 2), k3 = __shfl_down_sync(FULL, key, 3);
-          const uint32_t p1 = __shfl_down_sync(FULL, pkey, 1), p2 = __shfl_down_sync(FULL, pkey, 2), p3 = __shfl_down_sync(FULL, pkey, 3);
-          if ((lane & 3) == 0 && lane < w_hi - w_lo) {
-            const uint32_t off = (uint32_t)(s0 + c * CHR + w_lo + lane) * 4u;
-            if (CS > 1) {
+        {
+          constexpr int NGRP = RPW / 4;
 #pragma unroll 1
-              for (int r = 0; r < CS; ++r) st_async_v4(mapa(keys_a + off, r), key, k1, k2, k3, mapa(bk_a, r));
-              if (a.Bud > 0) st_async_v4(mapa(pkeys_a + off, ema_rank), pkey, p1, p2, p3, mapa(bp_a, ema_rank));
-            } else {
-              st_async_v4(keys_a + off, key, k1, k2, k3, bk_a);
-              if (a.Bud > 0) st_async_v4(pkeys_a + off, pkey, p1, p2, p3, bp_a);
+          for (int pi0 = 0; pi0 < NGRP * CS; pi0 += 32) {
+            const int pi = pi0 + lane;
+            const int grp = min(pi / CS, NGRP - 1), dest = pi % CS;
+            const uint32_t k0 = __shfl_sync(FULL, key, 4 * grp), k1 = __shfl_sync(FULL, key, 4 * grp + 1);
+            const uint32_t k2 = __shfl_sync(FULL, key, 4 * grp + 2), k3 = __shfl_sync(FULL, key, 4 * grp + 3);
+            if (pi < NGRP * CS && w_lo + 4 * grp < rows_c) {
+              const uint32_t off = (uint32_t)(g0r + w_lo + 4 * grp) * 4u;
+              st_async_v4(mapa(keys_a + off, dest), k0, k1, k2, k3, mapa(bk_a, dest));
             }
           }
         }
+        if (tl && lane == 0 && warp >= 4 && c == 0) tl[11] = gtime();
       }
       if (tl && lane == 0) tl[1] = gtime();
       MARK(300);
-
-      // =======================================================================================
-      if (warp < NTW) {
-        // ---- tile warps: a4 + a6.  Ring positions are claimed in order; a speculative partial whose
-        // fate is unknown is parked in a slot, everything else is folded into this warp's running state.
-        float* wst = slots + (size_t)(a.NSLOT + warp) * SLOTF;
-        const float sl2 = a.scale * LOG2E_F;
-        const int NG = (a.G + 7) >> 3;
-        uint32_t qb[2][D / 16][2];
-        {
-          const uint16_t* qg = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D;
-          const int r0 = lane >> 2, tq = lane & 3;
+      // a8 (Eq. 3) and the prediction for the next step (Eq. 2), OFF the critical path: the slice's scores are
+      // in shared memory; warps 4 and 5 take four consecutive blocks per thread (one st.async of prediction keys)
+      if (warp >= GE0 && warp < GE0 + GEW) {
+        asm volatile("bar.sync 3, %0;\n" ::"n"(SCW * 32) : "memory");
+        const uint32_t pkeys_a = smem_u32(pkeys), bp_a = smem_u32(&sh.bar_pred);
+#pragma unroll 1
+        for (int r4 = (tid - GE0 * 32) * 4; r4 < nrows; r4 += GEW * 32 * 4) {
+          double el[4], ev[4];
 #pragma unroll
-          for (int ps = 0; ps < 2; ++ps) {
-            const int g = ps * 8 + r0;
+          for (int e = 0; e < 4; ++e) {
+            const int i = s0 + r4 + e;
+            const bool has = i < min(nb, n_old);
+            el[e] = has ? Lg[i] : 0.0;
+            ev[e] = has ? Vg[i] : 0.0;
+          }
+          uint32_t pk[4];
 #pragma unroll
-            for (int k16 = 0; k16 < D / 16; ++k16) {
-              const int col = k16 * 16 + tq * 2;
-              qb[ps][k16][0] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col)) : 0u;
-              qb[ps][k16][1] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col + 8)) : 0u;
+          for (int e = 0; e < 4; ++e) {
+            const int i = s0 + r4 + e;
+            pk[e] = 0u;
+            if (i < nb) {
+              const double xd = (double)scs[r4 + e];
+              double ln = xd, vn = 0.0;
+              if (i < n_old) {  // non-contracted fp64, both lines use l^{t-1} (Q5)
+                vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, el[e])), __dmul_rn(omb, ev[e]));
+                ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, el[e]));
+              }
+              Lg[i] = ln;
+              Vg[i] = vn;
+              pk[e] = score_key(f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn))));
             }
           }
+          if (a.Bud > 0) st_async_v4(mapa(pkeys_a + (uint32_t)(s0 + r4) * 4u, ema_rank), pk[0], pk[1], pk[2], pk[3], mapa(bp_a, ema_rank));
         }
+      } else {
+        asm volatile("bar.arrive 3, %0;\n" ::"n"(SCW * 32) : "memory");
+      }
+      }  // scoring warps
+      if (!waited) { cluster_wait(); waited = true; }
+      // ---- a2: the true top-K by ALL EIGHT scoring warps (keys in registers, no histogram) when the row fits
+      const int kA = min(a.K, nb);
+      const bool fastA = nb <= 256 * 18 && kA <= 256;
+      if (warp < SCW && fastA) {
+        const Grp g8{tid, SCW * 32, warp, SCW, 1};
+        const SelMem m8{hist, red, cand, offs};
+        MARK(700);
+        wait_bar(&sh.bar_keys, ipar, err, 9);  // every CTA's keys have landed
+        MARK(701);
+        if (tl && lane == 0) tl[7] = gtime();
+        if (nb <= 256 * 9) grp_select_v3<256, 9>(keys, nb, kA, g8, m8, amask, tl);
+        else grp_select_v3<256, 18>(keys, nb, kA, g8, m8, amask, tl);
+        g8.sync();
+        if (tl && lane == 0) tl[8] = gtime();
+      }
+
+      // =======================================================================================
+      if (warp >= TW0) {
+        // ---- tile warps: a4 + a6.  Ring positions are claimed in order; a speculative partial whose
+        // fate is unknown is parked in a slot, everything else is folded into this warp's running state.
+        float* wst = slots + (size_t)(a.NSLOT + warp - TW0) * SLOTF;
+        const float sl2 = a.scale * LOG2E_F;
+        const int NG = (a.G + 7) >> 3;
+        uint32_t qb[D / 16][2];  // query fragments of pass `qps` (one pass unless G > 8: then reloaded, from L1)
+        int qps = -1;
+        auto load_q = [&](int ps) {
+          const uint16_t* qg = a.q + ((size_t)b * a.Hq + (size_t)h * a.G) * D;
+          const int g = ps * 8 + (lane >> 2), tq = lane & 3;
+#pragma unroll
+          for (int k16 = 0; k16 < D / 16; ++k16) {
+            const int col = k16 * 16 + tq * 2;
+            qb[k16][0] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col)) : 0u;
+            qb[k16][1] = g < a.G ? __ldg(reinterpret_cast<const uint32_t*>(qg + g * D + col + 8)) : 0u;
+          }
+          qps = ps;
+        };
+        load_q(0);
 #pragma unroll 1
         for (;;) {
           int p = 0;
-          if (lane == 0) p = atomicAdd(&sh.q_next, 1);
+          if (lane == 0) p = pos0 + NCH + atomicAdd(&sh.t_next, 1);  // tile positions follow the row's chunks
           p = __shfl_sync(FULL, p, 0);
           bool done = false;
           MARK(400 + (p & 63));
@@ -936,11 +1197,11 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           float* dst = wst;
           bool fold = true;
           int slot = -1;
-#pragma unroll
-          for (int ps = 0; ps < 2; ++ps) {  // (unrolled: the query fragments stay in registers)
-            if (ps >= NG) break;
+#pragma unroll 1
+          for (int ps = 0; ps < NG; ++ps) {  // (one copy of the tile code: the instruction cache is small)
+            if (ps != qps) load_q(ps);
             float o[D / 16][4], mt[2], lt[2];
-            tile_partial<D, ST>(Ks, &sh.fullK[bi], &sh.fullV[bi], par, qb[ps], valid, sl2, pk, pv, ps == 0, o, mt, lt, err);
+            tile_partial<D, ST>(Ks, &sh.fullK[bi], &sh.fullV[bi], par, qb, valid, sl2, pk, pv, ps == 0, o, mt, lt, err);
             if (ps == NG - 1) {  // every lane is done with the tile: the buffer may be refilled
               __syncwarp();
               if (lane == 0) mbar_arrive(&sh.empty[bi]);
@@ -970,22 +1231,20 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         if (tl && lane == 0) tl[4] = gtime();
       } else if (warp < GA0 + GAW) {
         // ---- group A: true top-K (a2), diff (a5), repair units, lists, merge (a7) ----------------------
-        const Grp g{tid - GA0 * 32, GAW * 32, warp - GA0, GAW, 1};
+        const Grp g{tid - GA0 * 32, GAW * 32, warp - GA0, GAW, 2};
         const SelMem m{hist, red, cand, offs};
-        MARK(700);
-        wait_bar(&sh.bar_keys, ipar, err, 9);
-        MARK(701);  // every CTA's keys have landed
-        if (tl && lane == 0) tl[7] = gtime();
+        if (!fastA) {  // long rows or K > 256: the generic narrowing, by this group alone
+          MARK(700);
+          wait_bar(&sh.bar_keys, ipar, err, 9);
+          MARK(701);
+          if (tl && lane == 0) tl[7] = gtime();
+          Thr t;
+          t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
+          if (kA < nb) t = grp_kth(keys, nb, kA, g, m, tl);
+          grp_mask(keys, nb, kA, t, g, amask);
+          if (tl && lane == 0) tl[8] = gtime();
+        }
         if (g.tid == 0) wait_flag(&sh.spec_ready, err, 10);
-        g.sync();
-        const int k = min(a.K, nb);
-        Thr t;
-        t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
-        MARK(702);
-        if (k < nb) t = grp_kth(keys, nb, k, g, m);
-        MARK(703);
-        if (tl && lane == 0) tl[8] = gtime();
-        grp_mask(keys, nb, k, t, g, amask);
         g.sync();
         // repair units: the missed blocks of this CTA's slice (all of A's in the sequential path)
         for (int i = s0 + g.tid; i < min(s1, nb); i += g.nt) {
@@ -1020,6 +1279,28 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
               atomicAdd(&a.stats[3], (unsigned long long)np);
             }
           }
+        }
+        if ((int)rank == ema_rank && a.Bud > 0) {
+          // ---- P of the next step = top-min(Bud, #stateful) of the Eq. 2 predictions (a3): the same group,
+          // the same code (one copy in the instruction cache), while this CTA's repair tiles are in flight
+          uint32_t* emask = offs + 2 * a.MBw;  // [MBw]
+          MARK(800);
+          wait_bar(&sh.bar_pred, ipar, err, 13);
+          MARK(801);
+          const int kp = min(a.Bud, nb);
+          if (nb <= 128 * 18 && kp <= 128) {
+            grp_select_v3<128, 18>(pkeys, nb, kp, g, m, emask, nullptr);
+          } else if (nb <= 128 * 36 && kp <= 128) {
+            grp_select_v3<128, 36>(pkeys, nb, kp, g, m, emask, nullptr);
+          } else {
+            Thr tp;
+            tp.key = 0u; tp.idx = 0x7fffffff;
+            if (kp < nb) tp = grp_kth(pkeys, nb, kp, g, m);
+            grp_mask(pkeys, nb, kp, tp, g, emask);
+          }
+          g.sync();
+          grp_emit(emask, nullptr, nb, g, m, ((par_raw & 1) ? a.P0 : a.P1) + (size_t)row * a.Bud, a.Bud, nullptr, 0);
+          if (tl && lane == 0) tl[9] = gtime();
         }
         // ---- merge: this CTA's hit slots and warp states per query head, then to the head's reducer
         MARK(710);
@@ -1105,27 +1386,15 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           }
         }
         if (tl && lane == 0) tl[5] = gtime();
-      } else if ((int)rank == ema_rank && a.Bud > 0) {
-        // ---- group E: P of the next step = top-min(Bud, #stateful) of the Eq. 2 predictions (a3) -------
-        const Grp g{tid - GE0 * 32, GEW * 32, warp - GE0, GEW, 2};
-        const SelMem m{hist + HB, red + 32, cand + CAND, offs + a.MBw};
-        uint32_t* emask = offs + 2 * a.MBw;  // [MBw]
-        MARK(800);
-        wait_bar(&sh.bar_pred, ipar, err, 13);
-        MARK(801);
-        const int k = min(a.Bud, nb);
-        Thr t;
-        t.key = 0u; t.idx = 0x7fffffff;
-        if (k < nb) t = grp_kth(pkeys, nb, k, g, m);
-        grp_mask(pkeys, nb, k, t, g, emask);
-        g.sync();
-        grp_emit(emask, nullptr, nb, g, m, Pnext + (size_t)row * a.Bud, a.Bud, nullptr, 0);
-        if (tl && lane == 0) tl[9] = gtime();
       }
     }
     MARK(900);
     __syncthreads();  // the row is done in this CTA
     MARK(901);
+    if (row + ncl < R) {  // (one CTA per row and more rows than CTAs)
+      row_init();
+      __syncthreads();
+    }
     if (tl && lane == 0 && tl[5] == 0) tl[5] = gtime();
   }
   if (!waited) cluster_wait();
@@ -1135,6 +1404,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
     MARK(902);
   }
 
+  if (tl && lane < 15) tlg[lane] = tl[lane];
   // ---- exit: the last CTA of the grid flips the parity and bumps the lengths -------------------
   if (tid == 0) {
     __threadfence();
@@ -1206,7 +1476,7 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
     a.o_plist = take(std::max(1, a.Bud) * 4);
     a.o_pmask = take(a.MBw * 4);
     a.o_amask = take(a.MBw * 4);
-    a.o_offs = take(3 * a.MBw * 4);
+    a.o_offs = take(std::max(3 * a.MBw, CANDX) * 4);  // emission offsets (2 groups) + the prediction bitmask; also the 256 partial ranks of a selection
     a.o_tslice = take(a.SLMAX * 4);
     a.o_sc = take((a.SLMAX + T::CHR) * 4);
     a.o_units = take(a.UCAP * 8);
@@ -1305,7 +1575,7 @@ int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* s
   a.ctl = c->ctl; a.stats = c->stats;
   a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32 + 1;
-  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud;
+  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.NBH = c->MB;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.cut = c->cut;
