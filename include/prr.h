@@ -230,10 +230,11 @@ int32_t prr_timeline_peek(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps
  * 0 (default) = the library picks the largest cluster (1, 2, 4 or 8 CTAs per (sequence, KV head) row)
  * that still runs every row at once; 1/2/4/8 force a size.  PRR_OPT_CUT: 1 (default) = once A is known,
  * predicted blocks that missed and whose tile has not been requested yet are not requested (PRR_DROP
- * only; the output is attention over A either way); 0 = every block of P is fetched.  Read-only:
+ * only; the output is attention over A either way); 0 = every block of P is fetched.  PRR_OPT_SUBTILE:
+ * tokens per tile unit of the fused step, 16 / 32 / 64 (default 64; a block larger than that is several units).  Read-only:
  * PRR_OPT_LAST_CLUSTER / _LAST_RING / _LAST_GRID = cluster size, ring depth and grid of the last fused
  * launch.  Unknown option or bad value -> PRR_E_INVALID. */
-enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
+enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_SUBTILE = 3, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
        PRR_OPT_LAST_GRID = 18 };
 int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value);
 int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* value_out /* host */);

@@ -38,13 +38,13 @@ namespace prr {
 
 constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr int NWARP = 12, NTHR = 32 * NWARP;
-constexpr int SCW = 8;             // warps 0 .. 7 score; afterwards:
-constexpr int GA0 = 0, GAW = 4;    //   group A (true top-K, lists, merge): warps 0 .. 3, named barrier 1
-constexpr int GE0 = 4, GEW = 2;    //   group E (next prediction): warps 4 .. 5, named barrier 2
-constexpr int TW0 = 6, NTW = 5;    // tile warps 6 .. 10 (8 .. 10 from the start, 6 and 7 once they have scored)
+constexpr int SCW = 8;             // warps 0 .. 7 score, then rank the true top-K together
+constexpr int GA0 = 0, GAW = 4;    // group A, warps 0 .. 3, then: the true top-K, the diff, Eq. 3 / Eq. 2, the lists, the next
+                                   //   prediction, the merge
+constexpr int TW0 = 4, NTW = 7;    // tile warps 4 .. 10: 8 .. 10 from the start, 4 .. 7 once they have scored and selected
 constexpr int LDW = 11;            // loader warp: predicted-set staging, then every bulk / TMA request
 constexpr int NBMAX = 12;          // ring buffers at most
-constexpr int HB = 1024;           // histogram buckets of a selection pass
+constexpr int HB = 256;            // histogram buckets of a selection pass (shared memory is better spent on slots)
 constexpr int CAND = 128;          // survivors that are ranked directly
 constexpr unsigned long long WAIT_NS = 200000000ull;  // every wait gives up loudly after 0.2 s
 
@@ -91,6 +91,13 @@ __device__ __forceinline__ bool mbar_try_wait_cl(unsigned long long* bar, uint32
   uint32_t done;
   asm volatile(
       "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }\n"
+      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return done != 0;
+}
+__device__ __forceinline__ bool mbar_test_wait(unsigned long long* bar, uint32_t parity) {  // (does not suspend)
+  uint32_t done;
+  asm volatile(
+      "{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }\n"
       : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
   return done != 0;
 }
@@ -263,7 +270,7 @@ __device__ __noinline__ Thr grp_kth_cont(const uint32_t* keys, int n, const Grp&
       g.sync();
       return r;
     }
-    const int sh = max(0, (32 - __clz(span)) - 10);  // (span >> sh) < HB
+    const int sh = max(0, (32 - __clz(span)) - 8);  // (span >> sh) < HB
 #pragma unroll 4
     for (int i = g.tid; i < n; i += g.nt) {
       const uint32_t d = keys[i] - lo;
@@ -309,7 +316,84 @@ __device__ __forceinline__ float key_value(uint32_t key) {  // inverse of score_
 // distinct keys are >= L.  Only the keys >= L (a few more than k) are collected (one atomic per warp)
 // and ranked exactly.  Everything is branch-free predicated code: a lone warp issues a dependent
 // instruction every ~10 clocks, so the instruction count per thread IS the latency.
-constexpr int CANDX = 256;
+constexpr int CANDX = 512;
+// The k-th largest (1-based) of the c <= CANDX survivors in m.cand (key << 32 | ~index), all with keys in
+// [klo, khi]: 256 buckets linear in VALUE over that range (order-preserving keys are logarithmic in value),
+// one atomic per survivor, suffix pick, then the handful of survivors in the crossing bucket are ranked.
+template <int NT>
+__device__ __forceinline__ void cand_kth(int c, int k, uint32_t klo, uint32_t khi, const Grp& g, const SelMem& m,
+                                         uint32_t& tkey, int& tidx) {
+  constexpr int NW = NT / 32, NBK = 256, PER = NBK / NT, CPT = CANDX / NT;
+  static_assert(PER >= 1 && CPT >= 1, "group of at most 256 threads");
+  const int lane = threadIdx.x & 31;
+  uint32_t* dec = m.red + NW * 2;
+  unsigned long long* cand2 = m.cand + CANDX;  // [64]
+  const float vlo = key_value(klo), vhi = key_value(khi);
+  const float inv = (float)NBK / (vhi - vlo);
+  const bool lin = (vhi > vlo) & (inv < CUDART_INF_F) & (vlo > -CUDART_INF_F);  // (uniform) else: one bucket
+  unsigned long long ce[CPT];
+  int bk[CPT];
+#pragma unroll
+  for (int q = 0; q < CPT; ++q) {
+    const int j = g.tid + q * NT;
+    ce[q] = m.cand[min(j, c - 1)];
+    bk[q] = lin ? min(NBK - 1, max(0, (int)((key_value((uint32_t)(ce[q] >> 32)) - vlo) * inv))) : 0;
+    if (j < c) atomicAdd(&m.hist[bk[q]], 1u);
+  }
+  if (g.tid == 0) dec[7] = 0u;
+  g.sync();
+  // suffix pick: thread t owns the buckets [NBK - (t+1) PER, NBK - t PER)
+  const int hb = NBK - g.tid * PER;
+  uint32_t hv[PER], sum = 0;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) { hv[q] = m.hist[hb - 1 - q]; sum += hv[q]; }
+  uint32_t incl = sum;
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const uint32_t x = __shfl_up_sync(FULL, incl, off);
+    incl += lane >= off ? x : 0u;
+  }
+  if (lane == 31) m.red[g.wid] = incl;
+  g.sync();
+#pragma unroll
+  for (int w = 0; w < NW; ++w) incl += w < g.wid ? m.red[w] : 0u;
+  uint32_t acc = incl - sum;
+#pragma unroll
+  for (int q = 0; q < PER; ++q) {
+    if (((int)acc < k) & (k <= (int)(acc + hv[q]))) { dec[0] = (uint32_t)(hb - 1 - q); dec[1] = hv[q]; dec[2] = acc; }  // exactly one
+    acc += hv[q];
+    m.hist[hb - 1 - q] = 0u;
+  }
+  g.sync();
+  const int bstar = (int)dec[0], cstar = (int)dec[1], need = k - (int)dec[2];
+#pragma unroll
+  for (int q = 0; q < CPT; ++q)
+    if ((g.tid + q * NT < c) & (bk[q] == bstar)) {
+      const uint32_t pos = atomicAdd(&dec[7], 1u);
+      if (pos < 64u) cand2[pos] = ce[q];
+    }
+  g.sync();
+  if (cstar <= 64) {
+    if (g.tid < cstar) {
+      const unsigned long long x = cand2[g.tid];
+      int rk = 0;
+#pragma unroll 4
+      for (int f = 0; f < cstar; ++f) rk += cand2[f] > x;
+      if (rk == need - 1) { dec[5] = (uint32_t)(x >> 32); dec[6] = ~(uint32_t)x; }  // exactly one
+    }
+  } else {  // (heavy ties inside one bucket) every survivor against all
+#pragma unroll 1
+    for (int j = g.tid; j < c; j += NT) {
+      const unsigned long long x = m.cand[j];
+      int rk = 0;
+#pragma unroll 4
+      for (int f = 0; f < c; ++f) rk += m.cand[f] > x;
+      if (rk == k - 1) { dec[5] = (uint32_t)(x >> 32); dec[6] = ~(uint32_t)x; }
+    }
+  }
+  g.sync();
+  tkey = dec[5]; tidx = (int)dec[6];
+}
 __device__ __forceinline__ bool selected_bf(uint32_t key, int i, uint32_t tkey, int tidx) {  // (no short circuit)
   return (key > tkey) | ((key == tkey) & (i <= tidx));
 }
@@ -343,18 +427,19 @@ __device__ PRR_SEL_INLINE void grp_select_v3(const uint32_t* keys, int n, int k,
       const uint32_t eq = __ballot_sync(FULL, v == wl);
       v = lane == __ffs(eq) - 1 ? 0u : v;
     }
-    if (lane == 0) m.red[g.wid] = wl;
+    const uint32_t wmax = __reduce_max_sync(FULL, tmax);
+    if (lane == 0) { m.red[g.wid] = wl; m.red[NW + g.wid] = wmax; }
     if (g.tid == 0) dec[7] = 0u;
     g.sync();
-    uint32_t L = 0xffffffffu;
+    uint32_t L = 0xffffffffu, KMAX = 0u;
 #pragma unroll
-    for (int w = 0; w < NW; ++w) L = min(L, m.red[w]);
+    for (int w = 0; w < NW; ++w) { L = min(L, m.red[w]); KMAX = max(KMAX, m.red[NW + w]); }
     if (tl && lane == 0) tl[10] = gtime();
     // survivors: per-thread bitmask, warp prefix, ONE atomic per warp
-    uint32_t cm = 0u;
+    unsigned long long cm = 0ull;
 #pragma unroll
-    for (int e = 0; e < KR; ++e) cm |= (uint32_t)((g.tid + e * NT < n) & (kr[e] >= L)) << e;
-    const int mine = __popc(cm);
+    for (int e = 0; e < KR; ++e) cm |= (unsigned long long)((g.tid + e * NT < n) & (kr[e] >= L)) << e;
+    const int mine = __popcll(cm);
     int incl = mine;
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
@@ -366,7 +451,7 @@ __device__ PRR_SEL_INLINE void grp_select_v3(const uint32_t* keys, int n, int k,
     base = __shfl_sync(FULL, base, 31) + incl - mine;
 #pragma unroll
     for (int e = 0; e < KR; ++e)
-      if ((cm >> e) & 1u) {
+      if ((cm >> e) & 1ull) {
         if (base < CANDX) m.cand[base] = ((unsigned long long)kr[e] << 32) | (uint32_t)~(g.tid + e * NT);
         ++base;
       }
@@ -378,35 +463,8 @@ __device__ PRR_SEL_INLINE void grp_select_v3(const uint32_t* keys, int n, int k,
       const Thr t = grp_kth(keys, n, k, g, m, nullptr);
       tkey = t.key; tidx = t.idx;
     } else {
-      // exact rank of every survivor, its c comparisons split over NT / P2 threads (P2 = c rounded up to a power of two)
-      int P2 = 32;
-      while (P2 < c && P2 < NT) P2 <<= 1;
-      if (c > NT) {  // more survivors than threads: a thread ranks several, each against all
-#pragma unroll 1
-        for (int j = g.tid; j < c; j += NT) {
-          const unsigned long long ce = m.cand[j];
-          int rk = 0;
-#pragma unroll 4
-          for (int f = 0; f < c; ++f) rk += m.cand[f] > ce;
-          if (rk == k - 1) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }
-        }
-      }
-      const int parts = NT / P2, j = g.tid & (P2 - 1), part = g.tid / P2;
-      const int per = (c + parts - 1) / parts, f0 = part * per, f1 = min(c, f0 + per);
-      const unsigned long long ce = m.cand[min(j, c - 1)];
-      int rk = 0;
-#pragma unroll 4
-      for (int f = f0; f < f1; ++f) rk += m.cand[f] > ce;
-      if (parts > 1) {  // partial ranks meet in shared memory (offs[] is free until the lists are emitted)
-        if (g.tid < CANDX) m.offs[g.tid] = 0u;
-        g.sync();
-        if (j < c) atomicAdd(&m.offs[j], (uint32_t)rk);
-        g.sync();
-        rk = (int)m.offs[j & (CANDX - 1)];
-      }
-      if ((c <= NT) & (j < c) & (part == 0) & (rk == k - 1)) { dec[5] = (uint32_t)(ce >> 32); dec[6] = ~(uint32_t)ce; }  // exactly one
-      g.sync();
-      tkey = dec[5]; tidx = (int)dec[6];
+      g.sync();  // (red / dec are reused)
+      cand_kth<NT>(c, k, L, KMAX, g, m, tkey, tidx);
     }
   }
   if (tl && lane == 0) tl[14] = gtime();
@@ -499,7 +557,8 @@ template <int D, int ST>
 __device__ __forceinline__ void tile_partial(const unsigned char* Ks, unsigned long long* barK, unsigned long long* barV,
                                              uint32_t par, const uint32_t (&qb)[D / 16][2], int valid, float sl2,
                                              const uint16_t* patch_k, const uint16_t* patch_v, bool first_pass,
-                                             float (&o)[D / 16][4], float (&mt)[2], float (&lt)[2], uint32_t* err) {
+                                             float (&o)[D / 16][4], float (&mt)[2], float (&lt)[2], uint32_t* err,
+                                             unsigned long long* tl = nullptr) {
   using T = Tile<D, ST>;
   constexpr int NM = ST / 16;
   const unsigned char* Vs = Ks + T::HALF;
@@ -549,6 +608,7 @@ __device__ __forceinline__ void tile_partial(const unsigned char* Ks, unsigned l
     mx0 = fmaxf(mx0, __shfl_xor_sync(FULL, mx0, off));
     mx1 = fmaxf(mx1, __shfl_xor_sync(FULL, mx1, off));
   }
+  const unsigned long long tq1 = tl ? gtime() : 0ull;
   const float off0 = mx0 * sl2, off1 = mx1 * sl2;  // valid >= 1: the maxima are finite
   mt[0] = off0; mt[1] = off1;
   if (first_pass) {
@@ -594,6 +654,7 @@ __device__ __forceinline__ void tile_partial(const unsigned char* Ks, unsigned l
     ls1 += __shfl_xor_sync(FULL, ls1, off);
   }
   lt[0] = ls0; lt[1] = ls1;
+  if (tl && (threadIdx.x & 31) == 0) { const unsigned long long tq2 = gtime(); tl[2] += tq2 - tq1; tl[1] = tq1; }
 }
 
 // State image in shared memory (slots, warp running states, received partials): per query head
@@ -646,6 +707,8 @@ struct Sh {  // static shared memory
   int t_next, n_slots, rep_cnt, ring_pos;
   int chunk_cnt[NBMAX];
   volatile int pos_unit[NBMAX];
+  volatile int patch_ready;  // the open block's new summary row is in patch_row
+  alignas(16) uint32_t patch_row[64];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -697,7 +760,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
   auto row_init = [&]() {
     if (tid == 0) {
       sh.q_total = 0; sh.q_final = 0; sh.sel_done = 0; sh.spec_ready = 0; sh.n_rep = 0;
-      sh.t_next = 0; sh.n_slots = 0; sh.rep_cnt = 0;
+      sh.t_next = 0; sh.n_slots = 0; sh.rep_cnt = 0; sh.patch_ready = 0;
     }
     for (int i = tid; i < NTW * SLOTF; i += NTHR) slots[(size_t)a.NSLOT * SLOTF + i] = (i % SW) == 0 ? -CUDART_INF_F : 0.f;
     for (int i = tid; i < a.MBw; i += NTHR) { pmask[i] = 0u; amask[i] = 0u; }
@@ -736,6 +799,10 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         for (int i = lane; i < (a.Bud * 4 + 127) / 128; i += 32) { pf(reinterpret_cast<const char*>(a.P0 + (size_t)row * a.Bud) + i * 128); pf(reinterpret_cast<const char*>(a.P1 + (size_t)row * a.Bud) + i * 128); }
         if (lane == 0) { pf(a.seq_lens + b); pf(a.parity); pf(a.theta + b * 3); pf(a.n_state + row); pf(a.ctl); }
         if (a.app && lane >= 8 && lane < 8 + (D * 8 + 127) / 128) pf(reinterpret_cast<const char*>(a.open_sum + (size_t)row * D) + (lane - 8) * 128);
+        if (a.app && lane >= 20 && lane < 20 + (D * 2 + 127) / 128) {
+          pf(reinterpret_cast<const char*>(a.k_new + (size_t)row * D) + (lane - 20) * 128);
+          pf(reinterpret_cast<const char*>(a.v_new + (size_t)row * D) + (lane - 20) * 128);
+        }
       }
     }
   }
@@ -865,15 +932,61 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         sh.spec_ready = 1;
         if (tl) tl[12] = gtime();
         for (; cnext < NCH; ++cnext) issue_chunk(cnext);
-        auto issue_unit = [&](int u, bool rep) {
+        // The ring's producer.  Speculative units (a4) go out in order until A is known; from then on the
+        // repair units (a6) go first -- they are the critical path -- and a predicted block that missed is
+        // not requested at all (PRR_DROP with the cut).  A wait for a free buffer is left as soon as A
+        // becomes known, so that the next buffer goes to a repair unit.
+        int u_spec = 0, sub_spec = 0, i_rep = 0, sub_rep = 0, nrep = -1;
+        const unsigned long long t0w = gtime();
+        uint32_t itw = 0;
+#pragma unroll 1
+        for (;;) {
+          if (nrep < 0 && sh.sel_done) {
+            __threadfence_block();
+            nrep = sh.n_rep;
+            if (tl) { tl[13] = gtime(); tl[14] = nrep; }
+          }
+          int u = -1, sub = 0;
+          bool rep = false;
+          if (nrep >= 0 && i_rep < nrep) {
+            u = UREP0 + i_rep; sub = sub_rep; rep = true;
+          } else {
+            while (u_spec < n_spec) {  // next speculative unit worth a request
+              const int blk = units[u_spec].x;
+              bool skip = blk < 0;
+              if (!skip && nrep >= 0 && a.cut && !a.retain) skip = !((amask[blk >> 5] >> (blk & 31)) & 1u);
+              if (!skip) break;
+              ++u_spec; sub_spec = 0;
+            }
+            if (u_spec < n_spec) { u = u_spec; sub = sub_spec; }
+          }
+          if (u < 0) {
+            if (nrep >= 0) break;  // everything is out
+            __nanosleep(64);       // only A is missing
+            if ((++itw & 1023u) == 0 && (long long)(gtime() - t0w) > (long long)WAIT_NS) { wait_fail(err, 4); break; }
+            continue;
+          }
           const int2 d = units[u];
-          for (int sub = 0; sub < NSUB; ++sub) {
-            const int valid = min(ST, len - d.x * a.bs - sub * ST);
-            if (valid <= 0) break;
-            const int bi = buf_acquire(pos);
+          const int valid = min(ST, len - d.x * a.bs - sub * ST);
+          const bool last_sub = sub + 1 >= NSUB || min(ST, len - d.x * a.bs - (sub + 1) * ST) <= 0;
+          if (valid > 0) {
+            const int bi = pos % NBUF;
+            if (pos >= NBUF) {  // the buffer's previous tenant must be consumed
+              const uint32_t par = ((pos / NBUF) - 1) & 1;
+              bool free_ = mbar_try_wait_cl(&sh.empty[bi], par);
+              if (!free_ && nrep < 0) {  // keep an eye on A while waiting
+                while (!(free_ = mbar_test_wait(&sh.empty[bi], par)) && !sh.sel_done)
+                  if ((++itw & 1023u) == 0 && (long long)(gtime() - t0w) > (long long)WAIT_NS) { wait_fail(err, 3); break; }
+                if (!free_) continue;  // A is known now: choose again
+              } else if (!free_) {
+                wait_bar(&sh.empty[bi], par, err, 3);
+              }
+              fence_proxy_async();
+            }
             unsigned char* Ks = ring + (size_t)bi * T::BYTES;
             const int y = (d.y * a.Hkv + h) * a.bs + sub * ST;
             sh.pos_unit[bi] = u | (sub << 20) | (rep ? 0x40000000 : 0);
+            if (tl && rep && tl[8] == 0) tl[8] = gtime();
             mbar_expect_tx(&sh.fullK[bi], T::HALF);
 #pragma unroll
             for (int i = 0; i < T::NBOX; ++i) tma_load_2d(Ks + i * T::BOX_BYTES, &a.mapK, i * 64, y, &sh.fullK[bi]);
@@ -884,28 +997,14 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             __threadfence_block();
             sh.q_issued = pos;
           }
-        };
-        // speculative units (a4); once A is known a predicted block that missed is not requested (PRR_DROP)
-#pragma unroll 1
-        for (int u = 0; u < n_spec; ++u) {
-          const int blk = units[u].x;
-          if (blk < 0) continue;
-          if (a.cut && !a.retain && sh.sel_done) {
-            __threadfence_block();
-            if (!((amask[blk >> 5] >> (blk & 31)) & 1u)) continue;
-          }
-          issue_unit(u, false);
+          if (rep) { if (last_sub || valid <= 0) { ++i_rep; sub_rep = 0; } else ++sub_rep; }
+          else { if (last_sub || valid <= 0) { ++u_spec; sub_spec = 0; } else ++sub_spec; }
         }
-        MARK(110);
-        wait_flag(&sh.sel_done, err, 4);
         MARK(111);
-        __threadfence_block();
-        const int nrep = sh.n_rep;
-#pragma unroll 1
-        for (int i = 0; i < nrep; ++i) issue_unit(UREP0 + i, true);  // repair units (a6)
         sh.q_total = pos;
         __threadfence_block();
         sh.q_final = 1;
+        if (tl) tl[9] = gtime();
         MARK(112);
       }
       __syncwarp();
@@ -918,7 +1017,6 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
       if (warp < GAW)
         for (int i = tid; i < nrows; i += GAW * 32) tslice[i] = s0 + i < nb ? __ldg(a.table + (size_t)b * a.MB + s0 + i) : 0;
       const bool own_ob = a.app && ob >= s0 && ob < s1;  // this CTA appends the new token
-      const int page_ob = own_ob ? __ldg(a.table + (size_t)b * a.MB + ob) : 0;
       double qs[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) qs[j] = 0.0;
@@ -961,33 +1059,12 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         if (tl && lane == 0 && c == 1 && warp >= 4) tl[12] = gtime();
         uint4* st = reinterpret_cast<uint4*>(ring + (size_t)bi * T::BYTES);
         if (own_ob && ob >= g0r + w_lo && ob < g0r + min(rows_c, w_lo + RPW)) {
-          // a0: the warp that scores the block the new token falls in appends it: cache slot, running
-          // sum and mean-key summary (exact fp64 sum, one division, one RNE to bf16, Q2) -- and patches
-          // the summary row it has staged, so the score below is the score after the append.
-          if (sub == 0) {
-            const int pos_t = len - 1, slot = pos_t - ob * a.bs;
-            const size_t ch = ((size_t)b * a.Hkv + h) * D + l * 8;
-            const uint4 kn = __ldg(reinterpret_cast<const uint4*>(a.k_new + ch));
-            const uint4 vn = __ldg(reinterpret_cast<const uint4*>(a.v_new + ch));
-            const size_t dst = (((size_t)page_ob * a.Hkv + h) * a.bs + slot) * (size_t)D + l * 8;
-            *reinterpret_cast<uint4*>(a.kp_w + dst) = kn;
-            *reinterpret_cast<uint4*>(a.vp_w + dst) = vn;
-            const uint32_t w[4] = {kn.x, kn.y, kn.z, kn.w};
-            uint32_t o[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const double x0 = (double)bf16_lo(w[j]), x1 = (double)bf16_hi(w[j]);
-              const double a0 = slot == 0 ? x0 : __dadd_rn(a.open_sum[ch + 2 * j], x0);
-              const double a1 = slot == 0 ? x1 : __dadd_rn(a.open_sum[ch + 2 * j + 1], x1);
-              a.open_sum[ch + 2 * j] = a0;
-              a.open_sum[ch + 2 * j + 1] = a1;
-              o[j] = (uint32_t)f64_to_bf16_rne(__ddiv_rn(a0, (double)(slot + 1))) |
-                     ((uint32_t)f64_to_bf16_rne(__ddiv_rn(a1, (double)(slot + 1))) << 16);
-            }
-            const uint4 rowv = make_uint4(o[0], o[1], o[2], o[3]);
-            st[(ob - g0r) * LPR + l] = rowv;
-            a.summ_w[(rowoff + ob) * LPR + l] = rowv;
-          }
+          // a0: the block the new token falls in is scored after the append: its summary row was computed
+          // by a tile warp while the chunk was in flight (below); patch the staged row
+          if (lane == 0) wait_flag(&sh.patch_ready, err, 15);
+          __syncwarp();
+          __threadfence_block();
+          if (sub == 0) st[(ob - g0r) * LPR + l] = *reinterpret_cast<const uint4*>(&sh.patch_row[l * 4]);
           __syncwarp();
         }
         // Exact dot products (Q1): every partial sum is exact in fp64, so the order is free.  Lane group
@@ -1065,63 +1142,61 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
       }
       if (tl && lane == 0) tl[1] = gtime();
       MARK(300);
-      // a8 (Eq. 3) and the prediction for the next step (Eq. 2), OFF the critical path: the slice's scores are
-      // in shared memory; warps 4 and 5 take four consecutive blocks per thread (one st.async of prediction keys)
-      if (warp >= GE0 && warp < GE0 + GEW) {
-        asm volatile("bar.sync 3, %0;\n" ::"n"(SCW * 32) : "memory");
-        const uint32_t pkeys_a = smem_u32(pkeys), bp_a = smem_u32(&sh.bar_pred);
-#pragma unroll 1
-        for (int r4 = (tid - GE0 * 32) * 4; r4 < nrows; r4 += GEW * 32 * 4) {
-          double el[4], ev[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int i = s0 + r4 + e;
-            const bool has = i < min(nb, n_old);
-            el[e] = has ? Lg[i] : 0.0;
-            ev[e] = has ? Vg[i] : 0.0;
-          }
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int i = s0 + r4 + e;
-            pk[e] = 0u;
-            if (i < nb) {
-              const double xd = (double)scs[r4 + e];
-              double ln = xd, vn = 0.0;
-              if (i < n_old) {  // non-contracted fp64, both lines use l^{t-1} (Q5)
-                vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, el[e])), __dmul_rn(omb, ev[e]));
-                ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, el[e]));
-              }
-              Lg[i] = ln;
-              Vg[i] = vn;
-              pk[e] = score_key(f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn))));
-            }
-          }
-          if (a.Bud > 0) st_async_v4(mapa(pkeys_a + (uint32_t)(s0 + r4) * 4u, ema_rank), pk[0], pk[1], pk[2], pk[3], mapa(bp_a, ema_rank));
-        }
-      } else {
-        asm volatile("bar.arrive 3, %0;\n" ::"n"(SCW * 32) : "memory");
-      }
       }  // scoring warps
       if (!waited) { cluster_wait(); waited = true; }
-      // ---- a2: the true top-K by ALL EIGHT scoring warps (keys in registers, no histogram) when the row fits
+      // ---- a2: the true top-K (keys in registers, no histogram) when the row fits the fast path
       const int kA = min(a.K, nb);
       const bool fastA = nb <= 256 * 18 && kA <= 256;
       if (warp < SCW && fastA) {
-        const Grp g8{tid, SCW * 32, warp, SCW, 1};
-        const SelMem m8{hist, red, cand, offs};
+        const Grp g4{tid, SCW * 32, warp, SCW, 1};
+        const SelMem m4{hist, red, cand, offs};
         MARK(700);
         wait_bar(&sh.bar_keys, ipar, err, 9);  // every CTA's keys have landed
         MARK(701);
         if (tl && lane == 0) tl[7] = gtime();
-        if (nb <= 256 * 9) grp_select_v3<256, 9>(keys, nb, kA, g8, m8, amask, tl);
-        else grp_select_v3<256, 18>(keys, nb, kA, g8, m8, amask, tl);
-        g8.sync();
+        if (nb <= 256 * 9) grp_select_v3<256, 9>(keys, nb, kA, g4, m4, amask, tl);
+        else grp_select_v3<256, 18>(keys, nb, kA, g4, m4, amask, tl);
+        g4.sync();
         if (tl && lane == 0) tl[8] = gtime();
       }
 
       // =======================================================================================
+      if (warp == 10 && a.app && ob >= s0 && ob < s1) {
+        // a0 by an idle tile warp, off the scoring warps' critical path: cache slot, running sum and mean-key
+        // summary of the open block (exact fp64 sum, one division, one RNE to bf16, Q2), D / 32 channels per lane
+        constexpr int CPL = D / 32;  // 2 or 4 channels = 1 or 2 words per lane
+        const int pos_t = len - 1, slot = pos_t - ob * a.bs;
+        const size_t ch = ((size_t)b * a.Hkv + h) * D + lane * CPL;
+        const size_t page = (size_t)__ldg(a.table + (size_t)b * a.MB + ob);
+        const size_t dst = ((page * a.Hkv + h) * a.bs + slot) * (size_t)D + lane * CPL;
+        uint32_t kw[CPL / 2], vw[CPL / 2], o[CPL / 2];
+#pragma unroll
+        for (int j = 0; j < CPL / 2; ++j) {
+          kw[j] = __ldg(reinterpret_cast<const uint32_t*>(a.k_new + ch) + j);
+          vw[j] = __ldg(reinterpret_cast<const uint32_t*>(a.v_new + ch) + j);
+        }
+        double s_old[CPL];
+#pragma unroll
+        for (int j = 0; j < CPL; ++j) s_old[j] = slot == 0 ? 0.0 : a.open_sum[ch + j];
+#pragma unroll
+        for (int j = 0; j < CPL / 2; ++j) {
+          reinterpret_cast<uint32_t*>(a.kp_w + dst)[j] = kw[j];
+          reinterpret_cast<uint32_t*>(a.vp_w + dst)[j] = vw[j];
+          const double x0 = (double)bf16_lo(kw[j]), x1 = (double)bf16_hi(kw[j]);
+          const double a0 = slot == 0 ? x0 : __dadd_rn(s_old[2 * j], x0);
+          const double a1 = slot == 0 ? x1 : __dadd_rn(s_old[2 * j + 1], x1);
+          a.open_sum[ch + 2 * j] = a0;
+          a.open_sum[ch + 2 * j + 1] = a1;
+          o[j] = (uint32_t)f64_to_bf16_rne(__ddiv_rn(a0, (double)(slot + 1))) |
+                 ((uint32_t)f64_to_bf16_rne(__ddiv_rn(a1, (double)(slot + 1))) << 16);
+          sh.patch_row[lane * (CPL / 2) + j] = o[j];
+          reinterpret_cast<uint32_t*>(a.summ_w + (rowoff + ob) * LPR)[lane * (CPL / 2) + j] = o[j];
+        }
+        __syncwarp();
+        if (lane == 0) { __threadfence_block(); sh.patch_ready = 1; }
+      }
       if (warp >= TW0) {
+        {
         // ---- tile warps: a4 + a6.  Ring positions are claimed in order; a speculative partial whose
         // fate is unknown is parked in a slot, everything else is folded into this warp's running state.
         float* wst = slots + (size_t)(a.NSLOT + warp - TW0) * SLOTF;
@@ -1141,6 +1216,13 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           qps = ps;
         };
         load_q(0);
+        // running state of the first eight query heads in REGISTERS (Eq. 6-8, unnormalised, m in log2 units);
+        // further heads (G > 8, second pass) fold into the shared-memory image
+        float orun[D / 16][4], mrun[2] = {-CUDART_INF_F, -CUDART_INF_F}, lrun[2] = {0.f, 0.f};
+#pragma unroll
+        for (int dt = 0; dt < D / 16; ++dt)
+#pragma unroll
+          for (int e = 0; e < 4; ++e) orun[dt][e] = 0.f;
 #pragma unroll 1
         for (;;) {
           int p = 0;
@@ -1186,6 +1268,8 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             return __shfl_sync(FULL, f, 0);
           };
           MARK(500 + (p & 63));
+          const unsigned long long tc0 = tl ? gtime() : 0ull;
+          if (tl && lane == 0) { tl[13] += 1; if (rep && tl[10] == 0) tl[10] = tc0; }
           int f = fate();
           if (f == 0) {  // already known to be over-predicted: let the tile land, free the buffer
             wait_bar(&sh.fullK[bi], par, err, 6);
@@ -1197,11 +1281,15 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           float* dst = wst;
           bool fold = true;
           int slot = -1;
+          unsigned long long tcw = 0ull;
+          if (tl) { wait_bar(&sh.fullK[bi], par, err, 6); tcw = gtime(); }
 #pragma unroll 1
           for (int ps = 0; ps < NG; ++ps) {  // (one copy of the tile code: the instruction cache is small)
             if (ps != qps) load_q(ps);
             float o[D / 16][4], mt[2], lt[2];
-            tile_partial<D, ST>(Ks, &sh.fullK[bi], &sh.fullV[bi], par, qb, valid, sl2, pk, pv, ps == 0, o, mt, lt, err);
+            const unsigned long long tp0 = tl ? gtime() : 0ull;
+            tile_partial<D, ST>(Ks, &sh.fullK[bi], &sh.fullV[bi], par, qb, valid, sl2, pk, pv, ps == 0, o, mt, lt, err, warp >= 8 ? tl : nullptr);
+            if (tl && lane == 0 && warp >= 8) { tl[6] += tl[1] - tp0; tl[3] = gtime(); }
             if (ps == NG - 1) {  // every lane is done with the tile: the buffer may be refilled
               __syncwarp();
               if (lane == 0) mbar_arrive(&sh.empty[bi]);
@@ -1222,13 +1310,41 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
                 }
               }
             }
-            if (f != 0) state_put<D>(dst, a.G, ps, o, mt, lt, fold);
+            if (f != 0) {
+              if (fold && ps == 0) {
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                  const float mn = fmaxf(mrun[j], mt[j]);
+                  const float al = mrun[j] == -CUDART_INF_F ? 0.f : ex2(mrun[j] - mn), be = ex2(mt[j] - mn);
+                  lrun[j] = al * lrun[j] + be * lt[j];
+                  mrun[j] = mn;
+#pragma unroll
+                  for (int dt = 0; dt < D / 16; ++dt) {
+                    orun[dt][j] = al * orun[dt][j] + be * o[dt][j];
+                    orun[dt][2 + j] = al * orun[dt][2 + j] + be * o[dt][2 + j];
+                  }
+                }
+              } else {
+                state_put<D>(dst, a.G, ps, o, mt, lt, fold);
+              }
+            }
+            if (tl && lane == 0 && warp >= 8) tl[7] += gtime() - tl[3];
+          }
+          if (tl && lane == 0) {
+            const unsigned long long tc1 = gtime();
+            if (rep && tl[12] == 0) tl[12] = tc1;
+            tl[14] += tc1 - tc0;                      // total time in tiles (wait for the data + compute)
+            tl[8] += tcw - tc0;                       // ... of which waiting for K
+            if (tl[11] == 0) tl[11] = tc1 - tc0;      // first tile
+            tl[9] = tc1 - tc0;                        // last tile
           }
         }
+        state_put<D>(wst, a.G, 0, orun, mrun, lrun, false);  // the running state, for the merge
         __syncwarp();
         if (lane == 0) mbar_arrive(&sh.bar_tw);
         MARK(600);
         if (tl && lane == 0) tl[4] = gtime();
+        }
       } else if (warp < GA0 + GAW) {
         // ---- group A: true top-K (a2), diff (a5), repair units, lists, merge (a7) ----------------------
         const Grp g{tid - GA0 * 32, GAW * 32, warp - GA0, GAW, 2};
@@ -1261,6 +1377,44 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           sh.sel_done = 1;
         }
         if (tl && lane == 0) tl[2] = gtime();
+        // a8 (Eq. 3) and the prediction for the next step (Eq. 2), off the critical path: the slice's scores are
+        // in shared memory; four consecutive blocks per thread (one st.async of prediction keys)
+        {
+          const uint32_t pkeys_a = smem_u32(pkeys), bp_a = smem_u32(&sh.bar_pred);
+          const double alpha = th0, beta = th1, gamma = th2;
+          const double oma = __dsub_rn(1.0, alpha), omb = __dsub_rn(1.0, beta);
+          double* Lg = a.ema_l + rowoff;
+          double* Vg = a.ema_v + rowoff;
+#pragma unroll 1
+          for (int r4 = g.tid * 4; r4 < nrows; r4 += g.nt * 4) {
+            double el[4], ev[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int i = s0 + r4 + e;
+              const bool has = i < min(nb, n_old);
+              el[e] = has ? Lg[i] : 0.0;
+              ev[e] = has ? Vg[i] : 0.0;
+            }
+            uint32_t pk[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int i = s0 + r4 + e;
+              pk[e] = 0u;
+              if (i < nb) {
+                const double xd = (double)scs[r4 + e];
+                double ln = xd, vn = 0.0;
+                if (i < n_old) {  // non-contracted fp64, both lines use l^{t-1} (Q5)
+                  vn = __dadd_rn(__dmul_rn(beta, __dsub_rn(xd, el[e])), __dmul_rn(omb, ev[e]));
+                  ln = __dadd_rn(__dmul_rn(alpha, xd), __dmul_rn(oma, el[e]));
+                }
+                Lg[i] = ln;
+                Vg[i] = vn;
+                pk[e] = score_key(f64_to_score(__dadd_rn(ln, __dmul_rn(gamma, vn))));
+              }
+            }
+            if (a.Bud > 0) st_async_v4(mapa(pkeys_a + (uint32_t)(s0 + r4) * 4u, ema_rank), pk[0], pk[1], pk[2], pk[3], mapa(bp_a, ema_rank));
+          }
+        }
         if (rank == 0) {  // the row's lists as the API reports them, off the critical path
           const uint32_t tot = grp_emit(amask, pmask, nb, g, m, a.setA + (size_t)row * a.K, a.K,
                                         a.setM + (size_t)row * a.K, a.K);
@@ -1281,8 +1435,8 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           }
         }
         if ((int)rank == ema_rank && a.Bud > 0) {
-          // ---- P of the next step = top-min(Bud, #stateful) of the Eq. 2 predictions (a3): the same group,
-          // the same code (one copy in the instruction cache), while this CTA's repair tiles are in flight
+          // ---- P of the next step = top-min(Bud, #stateful) of the Eq. 2 predictions (a3), on one CTA of the
+          // cluster, by the same group with the same code, while the repair tiles are in flight
           uint32_t* emask = offs + 2 * a.MBw;  // [MBw]
           MARK(800);
           wait_bar(&sh.bar_pred, ipar, err, 13);
@@ -1464,7 +1618,10 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
   a.UCAP = (a.Bud + CS - 1) / CS + a.K;
   a.SLMAX = ((((a.MB + 3) & ~3) + CS - 1) / CS + 3 + 4) & ~3;
   const int SW = D + 4, SLOTF = a.G * SW;
-  a.NSLOT = 8;
+  // a slot per speculative unit of a CTA if they fit (a unit whose fate is unknown and that finds no slot
+  // holds its warp until A is known); then the deepest ring; a ring of at least four tenants comes first
+  a.NSLOT = std::max(1, std::min(16, ((a.Bud + CS - 1) / CS) * ((a.bs + ST - 1) / ST)));
+  const int min_ring = 4;
   const int budget = c->row_dyn[key];
   int NBUF = NBMAX;
   for (;;) {
@@ -1476,19 +1633,20 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
     a.o_plist = take(std::max(1, a.Bud) * 4);
     a.o_pmask = take(a.MBw * 4);
     a.o_amask = take(a.MBw * 4);
-    a.o_offs = take(std::max(3 * a.MBw, CANDX) * 4);  // emission offsets (2 groups) + the prediction bitmask; also the 256 partial ranks of a selection
+    a.o_offs = take(3 * a.MBw * 4);  // emission offsets (2 groups) + the prediction bitmask
     a.o_tslice = take(a.SLMAX * 4);
-    a.o_sc = take((a.SLMAX + T::CHR) * 4);
+    a.o_sc = take(a.SLMAX * 4);
     a.o_units = take(a.UCAP * 8);
-    a.o_cand = take(2 * CAND * 8);
+    a.o_cand = take((CANDX + 64) * 8);
     a.o_red = take(2 * 32 * 4);
     a.o_slots = take((a.NSLOT + NTW) * SLOTF * 4);
     a.o_slotblk = take(a.NSLOT * 4);
     a.o_recv = take(CS * a.HL * SW * 4);
     a.o_end = o;
     if (o <= budget) break;
-    if (NBUF > 2) { --NBUF; continue; }
-    if (a.NSLOT > 1) { a.NSLOT /= 2; NBUF = NBMAX; continue; }
+    if (NBUF > min_ring) { --NBUF; continue; }
+    if (a.NSLOT > 1) { --a.NSLOT; continue; }
+    if (NBUF > 1) { --NBUF; continue; }
     return cudaErrorInvalidConfiguration;
   }
   a.NBUF = NBUF;
@@ -1556,7 +1714,7 @@ static int page_map(prr_ctx* c, const void* base, int box_rows, CUtensorMap* out
 int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
                 int spec, cudaStream_t s, const void* k_new, const void* v_new) {
   const size_t r = (size_t)kv->layer * c->maxB * c->Hkv;
-  const int ST = std::min(c->bs, 64);
+  const int ST = std::min(c->bs, c->sub_tile);
   RowArgs a{};
   if (int e = page_map(c, kv->k_pages, ST, &a.mapK)) return e;
   if (int e = page_map(c, kv->v_pages, ST, &a.mapV)) return e;

@@ -663,6 +663,7 @@ extern "C" int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value) {
     case PRR_OPT_PDL: if (value != 0 && value != 1) break; ctx->pdl = value; return PRR_OK;
     case PRR_OPT_CLUSTER: if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break; ctx->force_cs = value; return PRR_OK;
     case PRR_OPT_CUT: if (value != 0 && value != 1) break; ctx->cut = value; return PRR_OK;
+    case PRR_OPT_SUBTILE: if (value != 16 && value != 32 && value != 64) break; ctx->sub_tile = value; ctx->tmaps.clear(); return PRR_OK;
     default: break;
   }
   PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_option: unknown option %d or bad value %d", option, value);
@@ -674,6 +675,7 @@ extern "C" int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* v
     case PRR_OPT_PDL: *value_out = ctx->pdl; return PRR_OK;
     case PRR_OPT_CLUSTER: *value_out = ctx->force_cs; return PRR_OK;
     case PRR_OPT_CUT: *value_out = ctx->cut; return PRR_OK;
+    case PRR_OPT_SUBTILE: *value_out = ctx->sub_tile; return PRR_OK;
     case PRR_OPT_LAST_CLUSTER: *value_out = ctx->last_cs; return PRR_OK;
     case PRR_OPT_LAST_RING: *value_out = ctx->last_nbuf; return PRR_OK;
     case PRR_OPT_LAST_GRID: *value_out = ctx->last_grid; return PRR_OK;

@@ -50,7 +50,7 @@ struct prr_ctx {
   int n_sm = 0, smem_optin = 0, fused = 1;
   // fused step (k_row.cu): per kernel instantiation, attribute set + co-resident clusters of 1, 2, 4, 8 CTAs
   int row_attr[6] = {0, 0, 0, 0, 0, 0}; int row_maxcl[6][4] = {}; int row_dyn[6] = {};
-  int force_cs = 0, pdl = 1, cut = 1;          // tuning: cluster size override, programmatic dependent launch, early cut
+  int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;          // tuning: cluster size override, programmatic dependent launch, early cut
   int last_cs = 0, last_nbuf = 0, last_grid = 0; // launch shape of the last fused step (introspection)
   std::unordered_map<const void*, std::array<uint64_t, 16>> tmaps; // encoded CUtensorMap per K/V page pool
   // ---- calibration scratch (allocated on first prr_calibrate) ----

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libprr.so")
 
 OK, E_INVALID, E_UNSUPPORTED, E_STATE, E_CUDA, E_NOMEM = range(6)
 DROP, RETAIN = 0, 1
-OPT_PDL, OPT_CLUSTER, OPT_CUT, OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID = 0, 1, 2, 16, 17, 18
+OPT_PDL, OPT_CLUSTER, OPT_CUT, OPT_SUBTILE, OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID = 0, 1, 2, 3, 16, 17, 18
 FUSED, STREAMS = 0, 1
 
 SYMBOLS = [
