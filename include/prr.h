@@ -231,10 +231,15 @@ int32_t prr_timeline_peek(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps
  * that still runs every row at once; 1/2/4/8 force a size.  PRR_OPT_CUT: 1 (default) = once A is known,
  * predicted blocks that missed and whose tile has not been requested yet are not requested (PRR_DROP
  * only; the output is attention over A either way); 0 = every block of P is fetched.  PRR_OPT_SUBTILE:
- * tokens per tile unit of the fused step, 16 / 32 / 64 (default 64; a block larger than that is several units).  Read-only:
+ * tokens per tile unit of the cluster kernel, 16 / 32 / 64 (default 64; a block larger than that is several units).
+ * PRR_OPT_KERNEL: which fused kernel runs a step: 0 (default) = the library chooses by the number of
+ * (sequence, KV head) rows, 1 = the persistent cooperative grid (k_step.cu), 2 = a cluster per row (k_row.cu).
+ * PRR_OPT_PACE: percent of the estimated HBM rate at which the persistent kernel issues its first wave of
+ * speculative tiles (default 100; 0 = unpaced).  Read-only:
  * PRR_OPT_LAST_CLUSTER / _LAST_RING / _LAST_GRID = cluster size, ring depth and grid of the last fused
- * launch.  Unknown option or bad value -> PRR_E_INVALID. */
-enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_SUBTILE = 3, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
+ * launch, PRR_OPT_LAST_KERNEL = the kernel it used (1 or 2).  Unknown option or bad value -> PRR_E_INVALID. */
+enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_SUBTILE = 3, PRR_OPT_KERNEL = 4, PRR_OPT_PACE = 5,
+       PRR_OPT_LAST_KERNEL = 19, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
        PRR_OPT_LAST_GRID = 18 };
 int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value);
 int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* value_out /* host */);

@@ -35,6 +35,7 @@
 #include "prr_internal.h"
 
 namespace prr {
+namespace cluster {  // (k_step.cu has its own tile / selection code: keep the two apart)
 
 constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr int NWARP = 12, NTHR = 32 * NWARP;
@@ -1689,7 +1690,8 @@ static EncodeTiledFn encode_fn() {
 }
 static int page_map(prr_ctx* c, const void* base, int box_rows, CUtensorMap* out) {
   static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap is 128 bytes");
-  auto it = c->tmaps.find(base);
+  const void* key = reinterpret_cast<const void*>(reinterpret_cast<uintptr_t>(base) | (uintptr_t)(box_rows / 16 - 1));  // (16-byte aligned base)
+  auto it = c->tmaps.find(key);
   if (it == c->tmaps.end()) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return (int)cudaErrorNotSupported;
@@ -1705,14 +1707,17 @@ static int page_map(prr_ctx* c, const void* base, int box_rows, CUtensorMap* out
     std::array<uint64_t, 16> blob;
     memcpy(blob.data(), &m, 128);
     if (c->tmaps.size() > 4096) c->tmaps.clear();
-    it = c->tmaps.emplace(base, blob).first;
+    it = c->tmaps.emplace(key, blob).first;
   }
   memcpy(out, it->second.data(), 128);
   return 0;
 }
 
-int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
-                int spec, cudaStream_t s, const void* k_new, const void* v_new) {
+}  // namespace cluster
+using namespace cluster;
+
+int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
+                        int spec, cudaStream_t s, const void* k_new, const void* v_new) {
   const size_t r = (size_t)kv->layer * c->maxB * c->Hkv;
   const int ST = std::min(c->bs, c->sub_tile);
   RowArgs a{};

@@ -101,10 +101,15 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
     cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    if (c->fused && (!coop || c->n_sm < 1)) {
+    c->coop = coop;
+    if (c->n_sm < 1) {
       delete c;
-      PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: PRR_FUSED needs cooperative launch support");
+      PRR_FAIL(none, PRR_E_CUDA, "prr_create: no multiprocessors reported");
     }
+    int mclk = 0, bus = 0;
+    cudaDeviceGetAttribute(&mclk, cudaDevAttrMemoryClockRate, dev);     // kHz
+    cudaDeviceGetAttribute(&bus, cudaDevAttrGlobalMemoryBusWidth, dev); // bits
+    if (mclk > 0 && bus > 0) c->hbm_gbs_est = 0.8f * 2.0f * (float)mclk * 1e3f * (float)bus / 8.0f / 1e9f;
   }
 
   const size_t rows = (size_t)c->NL * c->maxB * c->Hkv;
@@ -462,7 +467,15 @@ static void enqueue_ema(prr_ctx* c, const prr_paged_kv* kv, cudaStream_t main, b
 static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries,
                       float* out, int spec, cudaStream_t s, const char* fn, const void* k_new = nullptr,
                       const void* v_new = nullptr) {
-  const int e = launch_step(c, kv, q, summaries, out, spec, s, k_new, v_new);
+  // Which fused kernel: the persistent cooperative grid when the rows are few (its warps are spread over
+  // every SM whatever the batch), a cluster per row once the rows fill the GPU (measured: DESIGN.md section 8).
+  const int rows = kv->batch * c->Hkv;
+  int kern = c->kernel;
+  if (kern == 0) kern = rows >= 64 ? 2 : 1;
+  if (kern == 1 && !c->coop) kern = 2;
+  c->last_kernel = kern;
+  const int e = kern == 2 ? launch_step_cluster(c, kv, q, summaries, out, spec, s, k_new, v_new)
+                          : launch_step_persist(c, kv, q, summaries, out, spec, s, k_new, v_new);
   if (e) {
     cudaGetLastError();
     PRR_FAIL(c, PRR_E_CUDA, "%s: fused step launch: %s", fn, cudaGetErrorString((cudaError_t)e));
@@ -664,6 +677,8 @@ extern "C" int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value) {
     case PRR_OPT_CLUSTER: if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break; ctx->force_cs = value; return PRR_OK;
     case PRR_OPT_CUT: if (value != 0 && value != 1) break; ctx->cut = value; return PRR_OK;
     case PRR_OPT_SUBTILE: if (value != 16 && value != 32 && value != 64) break; ctx->sub_tile = value; ctx->tmaps.clear(); return PRR_OK;
+    case PRR_OPT_KERNEL: if (value < 0 || value > 2) break; ctx->kernel = value; ctx->tmaps.clear(); return PRR_OK;
+    case PRR_OPT_PACE: if (value < 0 || value > 1000) break; ctx->pace_pct = value; return PRR_OK;
     default: break;
   }
   PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_option: unknown option %d or bad value %d", option, value);
@@ -676,6 +691,9 @@ extern "C" int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* v
     case PRR_OPT_CLUSTER: *value_out = ctx->force_cs; return PRR_OK;
     case PRR_OPT_CUT: *value_out = ctx->cut; return PRR_OK;
     case PRR_OPT_SUBTILE: *value_out = ctx->sub_tile; return PRR_OK;
+    case PRR_OPT_KERNEL: *value_out = ctx->kernel; return PRR_OK;
+    case PRR_OPT_PACE: *value_out = ctx->pace_pct; return PRR_OK;
+    case PRR_OPT_LAST_KERNEL: *value_out = ctx->last_kernel; return PRR_OK;
     case PRR_OPT_LAST_CLUSTER: *value_out = ctx->last_cs; return PRR_OK;
     case PRR_OPT_LAST_RING: *value_out = ctx->last_nbuf; return PRR_OK;
     case PRR_OPT_LAST_GRID: *value_out = ctx->last_grid; return PRR_OK;

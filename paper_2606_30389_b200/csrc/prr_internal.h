@@ -47,10 +47,12 @@ struct prr_ctx {
   float* pred = nullptr;      // [maxB, Hkv, MB] Eq. 2 predictions of the row being ranked (fused step)
   uint32_t* ctl = nullptr;    // fused step: exit counter, error flag, tickets, per-row dependency counters
   unsigned long long* tl = nullptr; int tl_on = 0, tl_warps = 0; // fused step: per-warp phase stamps (debug)
-  int n_sm = 0, smem_optin = 0, fused = 1;
+  int n_sm = 0, smem_optin = 0, fused = 1, coop = 0;
   // fused step (k_row.cu): per kernel instantiation, attribute set + co-resident clusters of 1, 2, 4, 8 CTAs
   int row_attr[6] = {0, 0, 0, 0, 0, 0}; int row_maxcl[6][4] = {}; int row_dyn[6] = {};
-  int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;          // tuning: cluster size override, programmatic dependent launch, early cut
+  int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;
+  int kernel = 0;                                // fused step: 0 auto, 1 persistent cooperative grid (k_step.cu), 2 cluster per row (k_row.cu)
+  int last_kernel = 0; int pace_pct = 100; float hbm_gbs_est = 6400.f; bool coop_attr[8] = {};          // tuning: cluster size override, programmatic dependent launch, early cut
   int last_cs = 0, last_nbuf = 0, last_grid = 0; // launch shape of the last fused step (introspection)
   std::unordered_map<const void*, std::array<uint64_t, 16>> tmaps; // encoded CUtensorMap per K/V page pool
   // ---- calibration scratch (allocated on first prr_calibrate) ----
@@ -118,10 +120,14 @@ void launch_merge(prr_ctx* c, int batch, const int32_t* merge_src, const int32_t
                   const float* O_spec, const float* m_spec, const float* l_spec, int w_spec,
                   const float* O_rep, const float* m_rep, const float* l_rep, int w_rep,
                   float* out, float* m_out, float* l_out, cudaStream_t s);
-// k_step.cu: one fused launch for a whole layer-step; spec = 0 is the sequential path.  Returns 0
-// or a cudaError_t.
-int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
-                int spec, cudaStream_t s, const void* k_new = nullptr, const void* v_new = nullptr);
+// One fused launch for a whole layer-step; spec = 0 is the sequential path.  Returns 0 or a cudaError_t.
+// k_step.cu: one persistent cooperative grid, warps as workers, global-memory flags between the stages
+// (best when the rows are few: batch 1).  k_row.cu: one thread-block cluster per (sequence, KV head) row,
+// everything between the stages of a row on chip (best when the rows fill the GPU).
+int launch_step_persist(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
+                        int spec, cudaStream_t s, const void* k_new, const void* v_new);
+int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries, float* out,
+                        int spec, cudaStream_t s, const void* k_new, const void* v_new);
 // k_calib.cu
 int launch_calibrate(prr_ctx* c, int layer, int seq, const float* IS, int T, int N,
                      const int32_t* n_valid, cudaStream_t s);
