@@ -32,6 +32,7 @@ __global__ void k_append(uint16_t* __restrict__ kp, uint16_t* __restrict__ vp,
   const int b = blockIdx.x;
   const int pos = seq_lens[b];
   const int blk = pos / bs, slot = pos - blk * bs;
+  if (blk >= MB) return;  // the sequence is full: nothing is written, the length stays (the caller maps max_blocks_per_seq pages)
   const size_t page = (size_t)table[(size_t)b * MB + blk];
   for (int idx = threadIdx.x; idx < Hkv * D; idx += blockDim.x) {
     const int h = idx / D, c = idx - h * D;

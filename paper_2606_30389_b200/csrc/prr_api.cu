@@ -248,6 +248,9 @@ extern "C" int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* 
                               void* summaries, void* stream) {
   CHECK_KV("prr_append");
   CHECK_PTR(k_new, "prr_append"); CHECK_PTR(v_new, "prr_append"); CHECK_PTR(summaries, "prr_append");
+  // (PRR_STREAMS: the layer's EMA update on the side stream derives the block count from seq_lens, which
+  // this call increments: it must have finished)
+  join_layer(ctx, kv->layer, (cudaStream_t)stream);
   launch_append(ctx, kv, k_new, v_new, summaries, (cudaStream_t)stream);
   return check_launch(ctx, "prr_append");
 }

@@ -27,7 +27,7 @@ class GpuLayer:
     """One layer of a config on the GPU: owns the caller-side buffers of include/prr.h."""
 
     def __init__(self, cfg: synth.Config, inp: synth.LayerInputs, policy=prr.DROP, ctx=None, layer=0,
-                 n_layers=1, budget=None, orchestration=prr.FUSED):
+                 n_layers=1, budget=None, orchestration=prr.FUSED, kernel=None, options=()):
         self.cfg, self.inp, self.layer = cfg, inp, layer
         dev = inp.k_pages.device
         self.MB = inp.block_table.shape[1]
@@ -35,6 +35,10 @@ class GpuLayer:
         self.ctx = ctx or prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, self.Bud, max_batch=cfg.B,
                                       max_blocks_per_seq=self.MB, n_layers=n_layers, policy=policy,
                                       orchestration=orchestration)
+        if kernel is not None:
+            self.ctx.set_option(prr.OPT_KERNEL, kernel)
+        for opt, val in options:
+            self.ctx.set_option(opt, val)
         self.k_pages, self.v_pages = inp.k_pages.clone(), inp.v_pages.clone()
         self.seq_lens = inp.seq_lens.clone()
         self.kv = self.ctx.kv(self.k_pages, self.v_pages, inp.block_table, self.seq_lens, layer)

@@ -23,10 +23,14 @@ TB128 = synth.Config("TB128", B=1, L=1, Hq=16, Hkv=1, d=64, ctx_lo=2000, ctx_hi=
 SHAPES = [TINY, T128, T16, TB128]
 
 
-def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None, orchestration=prr.FUSED):
+KERNELS = [prr.KERNEL_PERSISTENT, prr.KERNEL_CLUSTER]   # the two fused kernels (k_step.cu, k_row.cu)
+KID = {prr.KERNEL_PERSISTENT: "persistent", prr.KERNEL_CLUSTER: "cluster", None: "auto"}
+
+
+def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None, orchestration=prr.FUSED, kernel=None, options=()):
     cfg = cfg if seed is None else cfg.scaled(seed=seed)
     inp = synth.make_layer(cfg, 0, device=DEV, steps=steps)
-    gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget, orchestration=orchestration)
+    gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget, orchestration=orchestration, kernel=kernel, options=options)
     ol = H.oracle_layer(cfg, inp, policy=policy, budget=budget)
     return cfg, inp, gl, ol
 
@@ -239,10 +243,14 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
 
 
 def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True,
-               fused_append=False, orchestration=prr.FUSED):
+               fused_append=False, orchestration=prr.FUSED, kernel=None, options=(), sequential=False):
+    """Whole decode steps against the oracle: scores and block sets bit-exact, outputs within tolerance, and
+    (seq_check) the library's own sequential select-then-attend path within 1e-5 of PRR.  sequential=True
+    drives prr_attend itself against the oracle."""
     steps = cfg.steps if steps is None else steps
-    cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps, orchestration=orchestration)
-    twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget) if seq_check else None
+    cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps, orchestration=orchestration,
+                            kernel=kernel, options=options)
+    twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget, kernel=kernel, options=options) if seq_check else None
     if calibrate:
         gres = gl.calibrate(inp.q_cal)
         ores = ol.calibrate(synth.bits(inp.q_cal))
@@ -256,14 +264,24 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
         if not fused_append:
             gl.append(t)
         ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
-        out = gl.step_append(t) if fused_append else gl.step(t)
+        out = gl.step_append(t, sequential=sequential) if fused_append else gl.step(t, sequential=sequential)
         torch.cuda.synchronize()
         r = ol.step(synth.bits(inp.q_dec[t]))
+        if sequential:   # select-then-attend: no speculation, the output is attention over A whatever the policy
+            qb = synth.bits(inp.q_dec[t])
+            r = dict(r, out=np.stack([O.attend(qb[b], ol.k, ol.v, ol.table[b], ol.lens[b], r["A"][b], cfg.bs)
+                                      for b in range(cfg.B)]))
         sc = gl.scores()
         for b in range(cfg.B):
             nb = ol.n_blocks()[b]
             assert np.array_equal(sc[b, :, :nb].view(np.uint32), r["scores"][b, :, :nb].view(np.uint32)), f"scores t{t}"
-        H.compare_sets(gl, r, f"t{t}")
+        if sequential:
+            A = gl.sets()[0]
+            for b in range(cfg.B):
+                for h in range(cfg.Hkv):
+                    assert np.array_equal(H.unpad(A[b, h]), r["A"][b][h]), f"t{t} A b{b} h{h}"
+        else:
+            H.compare_sets(gl, r, f"t{t}")
         e = H.check_out(out.cpu().numpy(), r["out"], f"out t{t}")
         worst = (max(worst[0], e[0]), max(worst[1], e[1]))
         if twin:   # the library's own sequential select-then-attend path
@@ -276,7 +294,9 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
             for h in range(cfg.Hkv):
                 hits += len(r["A"][b][h]) - len(r["M"][b][h]); tot += len(r["A"][b][h])
     st = gl.ctx.get_stats()
-    assert st[0] == tot and st[1] == hits and st[2] == tot - hits
+    if not sequential:
+        assert st[0] == tot and st[1] == hits and st[2] == tot - hits
+    gl.ctx.check()
     if fused_append and twin:   # the cache, the summaries and the lengths the fused append leaves behind
         assert torch.equal(gl.seq_lens, twin.seq_lens), "seq_lens after fused append"
         assert torch.equal(gl.k_pages.view(torch.int16), twin.k_pages.view(torch.int16)), "k_pages after fused append"
@@ -285,25 +305,38 @@ def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, se
     return worst, hits / max(tot, 1)
 
 
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
 @pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
 @pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
-def test_decode_steps_small_shapes(cfg, policy):
-    run_decode(cfg, policy=policy)
+def test_decode_steps_small_shapes(cfg, policy, kernel):
+    run_decode(cfg, policy=policy, kernel=kernel)
 
 
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
 @pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
 @pytest.mark.parametrize("cfg", SHAPES, ids=lambda c: c.name)
-def test_step_append_small_shapes(cfg, policy):
+def test_step_append_small_shapes(cfg, policy, kernel):
     """prr_step_append (a0 fused into the step's launch) against the oracle and against the
     separate prr_append + prr_attend calls of a twin layer, including the cache it leaves behind."""
-    run_decode(cfg, policy=policy, fused_append=True)
+    run_decode(cfg, policy=policy, fused_append=True, kernel=kernel)
 
 
-def test_step_append_block_boundary_and_full_size():
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+@pytest.mark.parametrize("policy", [prr.DROP, prr.RETAIN])
+@pytest.mark.parametrize("cfg", [TINY, T128], ids=lambda c: c.name)
+def test_sequential_path_against_oracle(cfg, policy, kernel):
+    """prr_attend, the in-library select-then-attend baseline (a10), against the oracle itself: A bit-exact,
+    output = attention over A under both policies (nothing is speculated, so nothing is retained)."""
+    run_decode(cfg, policy=policy, kernel=kernel, sequential=True, seq_check=False)
+    run_decode(cfg, policy=policy, kernel=kernel, sequential=True, seq_check=False, fused_append=True)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+def test_step_append_block_boundary_and_full_size(kernel):
     """Appends that open a new block (slot 0) and the headline config at full size."""
-    run_decode(T16.scaled(ctx_lo=16 * 5, ctx_hi=16 * 5), steps=20, fused_append=True)   # starts on a boundary
-    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=4, fused_append=True)
-    run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=2, seq_check=False, fused_append=True)
+    run_decode(T16.scaled(ctx_lo=16 * 5, ctx_hi=16 * 5), steps=20, fused_append=True, kernel=kernel)   # starts on a boundary
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=4, fused_append=True, kernel=kernel)
+    run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=2, fused_append=True, kernel=kernel)
 
 
 def test_streams_orchestration_whole_steps():
@@ -336,34 +369,89 @@ def test_decode_c0_full():
     assert hit > 0.5
 
 
-def test_decode_without_calibration_and_zero_budget():
-    run_decode(TINY, calibrate=False)                 # first step: no state -> P = {} -> repair all of A
-    run_decode(TINY, budget=0, seq_check=False)       # no speculation at all
-    run_decode(T16.scaled(K=40), steps=4)             # K > number of blocks
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+def test_decode_without_calibration_and_zero_budget(kernel):
+    run_decode(TINY, calibrate=False, kernel=kernel)                 # first step: no state -> P = {} -> repair all of A
+    run_decode(TINY, budget=0, seq_check=False, kernel=kernel)       # no speculation at all
+    run_decode(T16.scaled(K=40), steps=4, kernel=kernel)             # K > number of blocks
 
 
-def test_decode_c1_sampled_steps():
-    """BASELINE.json configs[1] at full size (32768 ctx, 512 blocks), first 12 steps."""
-    run_decode(synth.CONFIGS["C1"].scaled(T_cal=32), steps=12, seq_check=True)
+def test_decode_c1_all_steps():
+    """BASELINE.json configs[1] at full size (32768 ctx, 512 blocks): all 128 steps, every output compared,
+    PRR within 1e-5 of the library's sequential path at every step."""
+    run_decode(synth.CONFIGS["C1"].scaled(T_cal=32))
+    run_decode(synth.CONFIGS["C1"].scaled(T_cal=32), steps=12, kernel=prr.KERNEL_CLUSTER)
 
 
-def test_decode_c2_full_size_sampled_steps():
-    """configs[2], the headline 128K case, at full size: 6 steps, every output compared."""
-    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=6)
+def test_decode_c2_all_steps():
+    """configs[2], the headline 128K case, at full size: all 128 steps, every output compared."""
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16))
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=16), steps=8, kernel=prr.KERNEL_CLUSTER)
 
 
-def test_decode_c4_full_size_sampled_steps():
-    """configs[4]: batch 4, GQA 7, block 32, 4096 blocks, K=128, budget 160, rho 0.7."""
-    worst, hit = run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=3, seq_check=False)
+def test_decode_c4_all_steps():
+    """configs[4]: batch 4, GQA 7, block 32, 4096 blocks, K=128, budget 160, rho 0.7: all 64 steps."""
+    run_decode(synth.CONFIGS["C4"].scaled(T_cal=8))
+    run_decode(synth.CONFIGS["C4"].scaled(T_cal=8), steps=4, kernel=prr.KERNEL_CLUSTER)
 
 
-def test_decode_c3_shape_two_layers():
-    """configs[3] shape (batch 16, ragged lengths in [16384, 32768]) on 2 of its 32 layers."""
+def test_decode_c3_all_layers():
+    """configs[3]: batch 16, ragged lengths in [16384, 32768], a stack of 32 independently seeded layers sharing
+    ONE context, theta calibrated per (layer, sequence), 8 of the 64 decode steps.  Four layers are resident and
+    interleave like a model's forward pass at a time (the oracle's host copy of a layer is 1.6 GB); every layer's
+    scores, block sets and outputs are compared at every step, and PRR against the library's own sequential
+    path (1e-5) on a twin context."""
+    cfg = synth.CONFIGS["C3"].scaled(T_cal=8)
+    steps, L, GROUP = 8, cfg.L, 4
+    MB = (cfg.ctx_hi + steps + cfg.bs - 1) // cfg.bs + 1
+    mk = lambda: prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B, max_blocks_per_seq=MB,
+                             n_layers=L)
+    ctx, ctx2 = mk(), mk()
+    kernels = set()
+    for l0 in range(0, L, GROUP):
+        layers = []
+        for l in range(l0, min(L, l0 + GROUP)):
+            inp = synth.make_layer(cfg, l, device=DEV, steps=steps)
+            gl = H.GpuLayer(cfg, inp, ctx=ctx, layer=l, n_layers=L)
+            twin = H.GpuLayer(cfg, inp, ctx=ctx2, layer=l, n_layers=L)
+            ol = H.oracle_layer(cfg, inp)
+            gres = gl.calibrate(inp.q_cal)
+            twin.calibrate(inp.q_cal)
+            ores = ol.calibrate(synth.bits(inp.q_cal))
+            for b in range(cfg.B):
+                assert gres[b][0][0] == ores[b][0], f"theta* L{l} b{b}"
+            layers.append((inp, gl, twin, ol))
+        for t in range(steps):
+            for inp, gl, twin, ol in layers:          # layers interleave like a model's forward pass
+                gl.step_append(t)
+                twin.append(t)
+                twin.step(t, sequential=True)
+            torch.cuda.synchronize()
+            kernels.add(ctx.get_option(prr.OPT_LAST_KERNEL))
+            for inp, gl, twin, ol in layers:          # every layer keeps its own out buffer
+                ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+                r = ol.step(synth.bits(inp.q_dec[t]))
+                sc = gl.scores()
+                for b in range(cfg.B):
+                    nb = ol.n_blocks()[b]
+                    assert np.array_equal(sc[b, :, :nb].view(np.uint32), r["scores"][b, :, :nb].view(np.uint32))
+                H.compare_sets(gl, r, f"t{t} L{gl.layer}")
+                H.check_out(gl.out.cpu().numpy(), r["out"], f"C3 t{t} L{gl.layer}")
+                assert (gl.out - twin.out).abs().max().item() <= 1e-5, f"PRR vs sequential t{t} L{gl.layer}"
+        del layers
+        torch.cuda.empty_cache()
+    ctx.check(); ctx2.check()
+    assert kernels == {prr.KERNEL_CLUSTER}        # 128 rows: the library runs a cluster per row here
+
+
+def test_decode_c3_shape_persistent_kernel():
+    """The same shape on the other fused kernel: 2 layers, 3 steps."""
     cfg = synth.CONFIGS["C3"].scaled(T_cal=8)
     steps = 3
     MB = (cfg.ctx_hi + steps + cfg.bs - 1) // cfg.bs + 1
     ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B, max_blocks_per_seq=MB,
                       n_layers=2)
+    ctx.set_option(prr.OPT_KERNEL, prr.KERNEL_PERSISTENT)
     layers = []
     for l in range(2):
         inp = synth.make_layer(cfg, l, device=DEV, steps=steps)
@@ -373,15 +461,118 @@ def test_decode_c3_shape_two_layers():
         ol.theta = [(0.6, 0.2, 0.5)] * cfg.B
         layers.append((inp, gl, ol))
     for t in range(steps):
-        for inp, gl, ol in layers:          # layers interleave like a model's forward pass
+        for inp, gl, ol in layers:
             gl.append(t)
             gl.step(t)
         torch.cuda.synchronize()
-        for inp, gl, ol in layers:          # every layer keeps its own out buffer
+        for inp, gl, ol in layers:
             ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
             r = ol.step(synth.bits(inp.q_dec[t]))
             H.compare_sets(gl, r, f"t{t} L{gl.layer}")
             H.check_out(gl.out.cpu().numpy(), r["out"], f"C3 t{t} L{gl.layer}")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+@pytest.mark.parametrize("pdl", [1, 0])
+@pytest.mark.parametrize("name", ["TINY", "C1", "C2"])
+def test_graph_captured_back_to_back_steps(name, pdl, kernel):
+    """32 prr_step_append steps captured into ONE graph and replayed without a host synchronisation between
+    them (with and without programmatic dependent launch): every out, the final block sets, scores and the
+    cache must equal what an eager, step-by-step synchronised twin produces, and the last step the oracle's."""
+    cfg = TINY.scaled(steps=32) if name == "TINY" else synth.CONFIGS[name].scaled(T_cal=8)
+    n = 32
+    cfg, inp, gl, ol = make(cfg, steps=n, kernel=kernel, options=[(prr.OPT_PDL, pdl)])
+    _, _, g2, _ = make(cfg, steps=n, kernel=kernel, options=[(prr.OPT_PDL, pdl)])
+    gl.calibrate(inp.q_cal); g2.calibrate(inp.q_cal); ol.calibrate(synth.bits(inp.q_cal))
+    outs_e = []
+    for t in range(n):
+        outs_e.append(gl.step_append(t).clone())
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+    s = torch.cuda.Stream()
+    outs_g = [torch.zeros_like(g2.out) for _ in range(n)]
+    with torch.cuda.stream(s):
+        g2.ctx.graph_begin(s)
+        for t in range(n):
+            g2.ctx.step_append(g2.kv, inp.q_dec[t].contiguous(), inp.k_new[t].contiguous(), inp.v_new[t].contiguous(),
+                               g2.summ, outs_g[t], stream=s)
+        graph = g2.ctx.graph_end(s)
+        graph.launch(s)
+    s.synchronize()
+    g2.ctx.check()
+    for t in range(n):
+        assert (outs_e[t] - outs_g[t]).abs().max().item() <= 2e-6, t
+    H.compare_sets(g2, r, "last step of the graph")
+    H.check_out(outs_g[-1].cpu().numpy(), r["out"], "last step of the graph")
+    assert np.array_equal(g2.scores().view(np.uint32), gl.scores().view(np.uint32))
+    assert torch.equal(g2.seq_lens, gl.seq_lens)
+    assert torch.equal(g2.k_pages.view(torch.int16), gl.k_pages.view(torch.int16))
+    assert torch.equal(g2.summ.view(torch.int16), gl.summ.view(torch.int16))
+    graph.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+def test_fused_selection_ties(kernel):
+    """The fused kernels' own top-K on rows full of ties: keys (hence summaries and scores) of many blocks are
+    made identical, a second group is zeroed (score exactly 0), so the K-th and the budget-th rank fall inside
+    runs of equal scores and the lower-index rule decides; more than 128 equal candidates at the threshold."""
+    cfg = synth.Config("TIES", B=2, L=1, Hq=8, Hkv=2, d=64, ctx_lo=64 * 300, ctx_hi=64 * 300, bs=64, K=40, Bud=60,
+                       rho=0.9, steps=4, T_cal=8)
+    inp = synth.make_layer(cfg, 0, device=DEV, steps=cfg.steps)
+    tab = inp.block_table.long()
+    for b in range(cfg.B):
+        src = tab[b, 7]
+        for i in range(20, 220):          # 200 blocks share one page image: 200 equal scores per row
+            inp.k_pages[tab[b, i]] = inp.k_pages[src]
+        for i in range(230, 260):         # 30 blocks of zero keys: score +0
+            inp.k_pages[tab[b, i]] = 0
+    gl = H.GpuLayer(cfg, inp, kernel=kernel)
+    ol = H.oracle_layer(cfg, inp)
+    gl.ctx.set_ema_params(0, -1, 0.8, 0.1, 0.25)
+    ol.theta = [(0.8, 0.1, 0.25)] * cfg.B
+    for t in range(cfg.steps):
+        out = gl.step_append(t)
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+        H.compare_sets(gl, r, f"ties t{t}")
+        H.check_out(out.cpu().numpy(), r["out"], f"ties t{t}")
+    gl.ctx.check()
+
+
+def test_streams_orchestration_full_size_and_graph():
+    """PRR_STREAMS (the paper's literal two-stream, event-ordered orchestration) at configs[1] size, and captured
+    into a graph: several steps without a host synchronisation, starting one token before a block boundary so
+    the append of the next step crosses it while the EMA update of the previous one may still be running."""
+    run_decode(synth.CONFIGS["C1"].scaled(T_cal=8), steps=4, orchestration=prr.STREAMS)
+    cfg = T16.scaled(ctx_lo=16 * 6 - 1, ctx_hi=16 * 6 - 1, steps=12)
+    cfg, inp, gl, ol = make(cfg, orchestration=prr.STREAMS)
+    _, _, g2, _ = make(cfg, orchestration=prr.STREAMS)
+    for g in (gl, g2):
+        g.ctx.set_ema_params(0, -1, 0.6, 0.2, 0.5)
+    ol.theta = [(0.6, 0.2, 0.5)] * cfg.B
+    n = cfg.steps
+    for t in range(n):                                  # no host synchronisation between the steps
+        gl.append(t); gl.step(t)
+    torch.cuda.synchronize()
+    for t in range(n):
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+    H.compare_sets(gl, r, "streams, unsynchronised steps")
+    H.check_out(gl.out.cpu().numpy(), r["out"], "streams, unsynchronised steps")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g2.ctx.graph_begin(s)
+        for t in range(n):
+            g2.ctx.append(g2.kv, inp.k_new[t].contiguous(), inp.v_new[t].contiguous(), g2.summ, stream=s)
+            g2.ctx.decode_step(g2.kv, inp.q_dec[t].contiguous(), g2.summ, g2.out, stream=s)
+        graph = g2.ctx.graph_end(s)
+        graph.launch(s)
+    s.synchronize()
+    H.compare_sets(g2, r, "streams in a graph")
+    H.check_out(g2.out.cpu().numpy(), r["out"], "streams in a graph")
+    graph.destroy()
 
 
 def test_graph_replay_matches_eager():
