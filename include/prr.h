@@ -133,6 +133,36 @@ int32_t prr_predict(prr_ctx* ctx, int32_t layer, int32_t batch, int32_t* P_out,
 int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, const float* scores,
                        const int32_t* n_blocks, void* stream);
 
+/* --- profiling-guided speculation budget (PAPER.md:204-208 section 4.4, :229, :424 A.6) --------- */
+
+/* The budget of prr_create is the WIDTH of a prediction row and the largest budget; the budget in force
+ * (blocks of P predicted for the next step, delta * K of Eq. 1) is a per-layer run-time value, initially
+ * that maximum.  prr_set_budget changes it (layer = -1: every layer) and re-predicts the layer's next P
+ * under it, so the next decode step already speculates on the new budget.  0 = no speculation: the step
+ * degenerates to select-then-attend through the repair path. */
+int32_t prr_set_budget(prr_ctx* ctx, int32_t layer, int32_t budget, void* stream);
+int32_t prr_get_budget(const prr_ctx* ctx, int32_t layer, int32_t* budget_out /* host */);
+/* The paper's offline sweep, in the library: for every candidate budget (host int32 [n_budgets]) run the T
+ * decode steps of a query trajectory q_traj (dev bf16 [T, batch, n_q_heads, head_dim], e.g. the prefill
+ * trajectory used for prr_calibrate) on the layer's cache WITHOUT appending, each step timed by CUDA events
+ * on `stream` (cold_l2 != 0: a 256 MB write between steps, outside the timed interval), and the same for
+ * the sequential select-then-attend path.  The paper compares the speculative-attention time with the
+ * selection window; timing the whole critical path per budget measures what that comparison stands for,
+ * including the repair work a smaller budget causes.  us_out (host float [n_budgets]) = mean us per step
+ * (the first step is a warm-up), us_sequential_out (host float) likewise, best_budget_out (host) = the
+ * candidate with the smallest time, or 0 if the sequential path beats them all ("largest safe delta" here
+ * is the fastest one).  The layer's predictor state, prediction buffers, counters and budget are saved
+ * before and restored after.  Synchronises `stream`; not allowed inside a stream capture. */
+int32_t prr_profile_budget(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_traj, int32_t T,
+                           const void* summaries, const int32_t* budgets, int32_t n_budgets, int32_t cold_l2,
+                           float* us_out, float* us_sequential_out, int32_t* best_budget_out, void* stream);
+/* Lookup by context length: a least-squares polynomial (degree <= 3) through the profiled
+ * (context length, best budget) points, evaluated and clamped to [0, budget of prr_create] by
+ * prr_budget_for.  Before any fit prr_budget_for returns the budget of prr_create. */
+int32_t prr_budget_fit(prr_ctx* ctx, int32_t n, const int32_t* ctx_lens /* host */, const int32_t* budgets /* host */,
+                       int32_t degree);
+int32_t prr_budget_for(const prr_ctx* ctx, int32_t ctx_len, int32_t* budget_out /* host */);
+
 /* --- selection (a1, a2) ---------------------------------------------------------------------- */
 
 /* Block importance (PAPER.md:66 compressed attention; group aggregated as in A.1 PAPER.md:372):

@@ -65,7 +65,7 @@ struct RowArgs {
   int32_t* setA; int32_t* setM; int32_t* counts;
   uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, retain, spec, cut;
-  int CS, NBUF, NSLOT, UCAP, HL, SLMAX, NBH;
+  int CS, NBUF, NSLOT, UCAP, HL, SLMAX, NBH, BudSel;  // BudSel <= Bud: the run-time budget of the NEXT prediction
   // dynamic shared memory offsets (bytes)
   int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
       o_slots, o_slotblk, o_recv, o_end;
@@ -1442,8 +1442,10 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           MARK(800);
           wait_bar(&sh.bar_pred, ipar, err, 13);
           MARK(801);
-          const int kp = min(a.Bud, nb);
-          if (nb <= 128 * 18 && kp <= 128) {
+          const int kp = min(a.BudSel, nb);
+          if (kp == 0) {
+            for (int w = g.tid; w < a.MBw; w += g.nt) emask[w] = 0u;
+          } else if (nb <= 128 * 18 && kp <= 128) {
             grp_select_v3<128, 18>(pkeys, nb, kp, g, m, emask, nullptr);
           } else if (nb <= 128 * 36 && kp <= 128) {
             grp_select_v3<128, 36>(pkeys, nb, kp, g, m, emask, nullptr);
@@ -1738,7 +1740,7 @@ int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const
   a.ctl = c->ctl; a.stats = c->stats;
   a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32 + 1;
-  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.NBH = c->MB;
+  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.NBH = c->MB; a.BudSel = c->bud_eff[kv->layer];
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.cut = c->cut;

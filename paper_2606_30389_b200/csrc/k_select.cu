@@ -145,7 +145,7 @@ struct EmaKArgs {
   double* ema_l; double* ema_v; int32_t* n_state; const double* theta;  // already offset to (layer, seq0)
   const float* scores; const int32_t* seq_lens; const int32_t* n_blocks;
   int32_t* P_out; int32_t* P_count; int32_t* P_save;
-  int Hkv, MB, Bud, bs;
+  int Hkv, MB, Bud, BudSel, bs;  // Bud: width of a P row; BudSel <= Bud: blocks predicted (the run-time budget)
 };
 
 __global__ void __launch_bounds__(SEL_NT) k_ema(EmaKArgs a) {
@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(SEL_NT) k_ema(EmaKArgs a) {
     for (int j = tid; j < a.Bud; j += SEL_NT) a.P_save[(size_t)row * a.Bud + j] = P_row[j];
   __syncthreads();
   if (a.scores && tid == 0) a.n_state[row] = n_new;
-  const int k = min(a.Bud, n_new);
+  const int k = min(a.BudSel, n_new);
   int cnt = 0;
   if (k > 0) {
     uint32_t T;
@@ -236,6 +236,7 @@ void launch_ema(prr_ctx* c, const EmaArgs& e, cudaStream_t s) {
   a.Hkv = c->Hkv;
   a.MB = c->MB;
   a.Bud = c->Bud;
+  a.BudSel = c->bud_eff[e.layer];
   a.bs = c->bs;
   const size_t smem = sel_smem_bytes(c->MB);
   ensure_smem((const void*)k_ema, smem);

@@ -424,7 +424,7 @@ struct StepArgs {
   unsigned long long* mt_spec; unsigned long long* mt_rep;
   uint32_t* ctl; uint32_t* sel; unsigned long long* sel2; uint32_t* ufs; uint32_t* ufr; uint32_t* sfl;  // header, then the flag arrays
   unsigned long long* stats; unsigned long long* tl;
-  int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;
+  int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, BudSel, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;  // BudSel <= Bud: the run-time budget of the NEXT prediction
   int msw;  // channels per merge item (16 .. D): the narrowest slice that still gives every merge warp at most one item
   float scale; float pace_ns; double score_c;
 };
@@ -1107,7 +1107,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
     if (a.Bud <= 0) return;
   }
   // ---- exact selection (one call site) ----
-  const int k = min(is_sel ? a.K : a.Bud, n);
+  const int k = min(is_sel ? a.K : a.BudSel, n);
   Keys ks{in_sm ? smem_u32(m.keys) : 0u, is_sel ? sc : pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
@@ -1119,7 +1119,7 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
       kreg[e] = i < n ? m.keys[i] : 0u;
     }
   }
-  if (k < n) {
+  if (k > 0 && k < n) {
     if (fast) {
       if (tl && tm.tid == 0) tl[9] = gtime();
       t = fast_kth(kreg, ks, n, k, tm, m, tl);
@@ -1749,7 +1749,7 @@ static int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const 
     a.sel = c->ctl + CTL_HDR; a.sel2 = (unsigned long long*)(a.sel + rme); a.ufs = a.sel + rme + 2 * rm; a.ufr = a.ufs + rm * c->Bud; a.sfl = a.ufr + rm * c->K;
   } a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
-  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.Rmax = c->maxB * c->Hkv;
+  a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.BudSel = c->bud_eff[kv->layer]; a.Rmax = c->maxB * c->Hkv;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.scale = c->sm_scale; a.score_c = c->score_c;

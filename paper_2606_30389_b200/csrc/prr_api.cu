@@ -2,6 +2,7 @@
 // two-stream, event-ordered orchestration of one PRR layer-step (Fig. 1, :38-42).
 #include <cmath>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 
 #include "prr_internal.h"
@@ -180,6 +181,7 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
   c->ev_upd.assign(c->NL, nullptr);
   c->upd_pending.assign(c->NL, 0);
+  c->bud_eff.assign(c->NL, c->Bud);
   for (int l = 0; l < c->NL; ++l) A(cudaEventCreateWithFlags(&c->ev_upd[l], cudaEventDisableTiming));
   if (e != cudaSuccess) {
     g_create_err = std::string("prr_create: ") + cudaGetErrorString(e);
@@ -388,6 +390,162 @@ extern "C" int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, co
   launch_ema(ctx, e, s);
   sync_pred(ctx, layer, 0, batch, s);
   return check_launch(ctx, "prr_ema_update");
+}
+
+// ---------------------------------------------------------------------------------------------
+// Profiling-guided speculation budget (PAPER.md:204-208 section 4.4, :229, :424 A.6)
+// ---------------------------------------------------------------------------------------------
+static void repredict(prr_ctx* c, int layer, cudaStream_t s) {  // P of the next step under the layer's current budget
+  if (c->Bud <= 0) return;
+  join_layer(c, layer, s);
+  EmaArgs e{};
+  e.layer = layer; e.batch = c->maxB; e.seq0 = 0;
+  e.P_out = c->P_next + layer_rows(c, layer) * c->Bud;
+  launch_ema(c, e, s);
+  sync_pred(c, layer, 0, c->maxB, s);
+}
+
+extern "C" int32_t prr_set_budget(prr_ctx* ctx, int32_t layer, int32_t budget, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < -1 || layer >= ctx->NL || budget < 0 || budget > ctx->Bud)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_budget: need -1 <= layer < n_layers and 0 <= budget <= the budget of prr_create");
+  for (int l = layer < 0 ? 0 : layer; l < (layer < 0 ? ctx->NL : layer + 1); ++l) {
+    ctx->bud_eff[l] = budget;
+    repredict(ctx, l, (cudaStream_t)stream);
+  }
+  return check_launch(ctx, "prr_set_budget");
+}
+
+extern "C" int32_t prr_get_budget(const prr_ctx* ctx, int32_t layer, int32_t* budget_out) {
+  if (!ctx || !budget_out || layer < 0 || layer >= ctx->NL) return PRR_E_INVALID;
+  *budget_out = ctx->bud_eff[layer];
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_profile_budget(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_traj, int32_t T,
+                                      const void* summaries, const int32_t* budgets, int32_t n_budgets,
+                                      int32_t cold_l2, float* us_out, float* us_sequential_out,
+                                      int32_t* best_budget_out, void* stream) {
+  CHECK_KV("prr_profile_budget");
+  CHECK_PTR(q_traj, "prr_profile_budget"); CHECK_PTR(summaries, "prr_profile_budget");
+  if (T < 2 || n_budgets < 1 || !budgets) PRR_FAIL(ctx, PRR_E_INVALID, "prr_profile_budget: need T >= 2 and at least one budget");
+  for (int i = 0; i < n_budgets; ++i)
+    if (budgets[i] < 0 || budgets[i] > ctx->Bud) PRR_FAIL(ctx, PRR_E_INVALID, "prr_profile_budget: budget out of range");
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(s, &cap);
+  if (cap != cudaStreamCaptureStatusNone) PRR_FAIL(ctx, PRR_E_STATE, "prr_profile_budget: cannot run inside a stream capture");
+  join_updates(ctx, s);
+  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  const int layer = kv->layer;
+  const size_t r = layer_rows(ctx, layer), nr = (size_t)ctx->maxB * ctx->Hkv;
+  // the layer's predictor state is saved and put back: profiling leaves no trace
+  struct Save { void* dev; void* copy; size_t bytes; };
+  std::vector<Save> saves = {
+      {ctx->ema_l + r * ctx->MB, nullptr, nr * ctx->MB * sizeof(double)}, {ctx->ema_v + r * ctx->MB, nullptr, nr * ctx->MB * sizeof(double)},
+      {ctx->n_state + r, nullptr, nr * sizeof(int32_t)}, {ctx->parity + layer, nullptr, sizeof(int32_t)},
+      {ctx->Pbuf[0] + r * ctx->Bud, nullptr, nr * ctx->Bud * sizeof(int32_t)}, {ctx->Pbuf[1] + r * ctx->Bud, nullptr, nr * ctx->Bud * sizeof(int32_t)},
+      {ctx->P_next + r * ctx->Bud, nullptr, nr * ctx->Bud * sizeof(int32_t)}, {ctx->P_used + r * ctx->Bud, nullptr, nr * ctx->Bud * sizeof(int32_t)},
+      {ctx->stats, nullptr, 4 * sizeof(unsigned long long)}};
+  cudaError_t e = cudaSuccess;
+  for (auto& v : saves) {
+    if (!v.bytes) continue;
+    if (e == cudaSuccess) e = cudaMalloc(&v.copy, v.bytes);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(v.copy, v.dev, v.bytes, cudaMemcpyDeviceToDevice, s);
+  }
+  void* flush = nullptr;
+  const size_t flush_bytes = (size_t)256 << 20;  // larger than L2
+  if (cold_l2 && e == cudaSuccess) e = cudaMalloc(&flush, flush_bytes);
+  std::vector<cudaEvent_t> ev(2 * (size_t)T, nullptr);
+  for (auto& x : ev) if (e == cudaSuccess) e = cudaEventCreate(&x);
+  const int saved_budget = ctx->bud_eff[layer];
+  const size_t qstep = (size_t)kv->batch * ctx->Hq * ctx->D;  // bf16 elements per step
+  int rc = PRR_OK;
+  auto restore = [&]() { for (auto& v : saves) if (v.copy) cudaMemcpyAsync(v.dev, v.copy, v.bytes, cudaMemcpyDeviceToDevice, s); };
+  auto run = [&](int budget, bool sequential, float* us) {  // mean over the steps after the first (warm-up of clocks and code)
+    restore();
+    ctx->bud_eff[layer] = budget;
+    repredict(ctx, layer, s);
+    for (int t = 0; t < T && rc == PRR_OK; ++t) {
+      if (flush) cudaMemsetAsync(flush, t, flush_bytes, s);
+      cudaEventRecord(ev[2 * t], s);
+      const void* q = (const uint16_t*)q_traj + (size_t)t * qstep;
+      rc = sequential ? prr_attend(ctx, kv, q, summaries, ctx->st_out, stream) : prr_decode_step(ctx, kv, q, summaries, ctx->st_out, stream);
+      join_layer(ctx, layer, s);
+      cudaEventRecord(ev[2 * t + 1], s);
+    }
+    if (rc != PRR_OK) return;
+    if (cudaStreamSynchronize(s) != cudaSuccess) { rc = PRR_E_CUDA; return; }
+    double tot = 0.0;
+    for (int t = 1; t < T; ++t) { float ms = 0.f; cudaEventElapsedTime(&ms, ev[2 * t], ev[2 * t + 1]); tot += ms; }
+    *us = (float)(tot * 1e3 / (T - 1));
+  };
+  float best_us = 0.f, seq_us = 0.f;
+  int best = 0;
+  if (e == cudaSuccess) {
+    run(0, true, &seq_us);
+    best_us = seq_us; best = 0;  // no speculation at all is the fallback PRR must beat
+    for (int i = 0; i < n_budgets && rc == PRR_OK; ++i) {
+      float us = 0.f;
+      run(budgets[i], false, &us);
+      if (us_out) us_out[i] = us;
+      if (rc == PRR_OK && us < best_us) { best_us = us; best = budgets[i]; }
+    }
+    restore();
+    ctx->bud_eff[layer] = saved_budget;
+    repredict(ctx, layer, s);
+    cudaStreamSynchronize(s);
+  }
+  for (auto& x : ev) if (x) cudaEventDestroy(x);
+  for (auto& v : saves) if (v.copy) cudaFree(v.copy);
+  if (flush) cudaFree(flush);
+  if (e != cudaSuccess) { cudaGetLastError(); PRR_FAIL(ctx, e == cudaErrorMemoryAllocation ? PRR_E_NOMEM : PRR_E_CUDA, "prr_profile_budget: %s", cudaGetErrorString(e)); }
+  if (rc != PRR_OK) return rc;
+  if (us_sequential_out) *us_sequential_out = seq_us;
+  if (best_budget_out) *best_budget_out = best;
+  return check_launch(ctx, "prr_profile_budget");
+}
+
+// Least-squares polynomial budget(context length) through the profiled points ("polynomial
+// regression" for lengths off the grid).  Normal equations in x = len / max(len), Gaussian elimination.
+extern "C" int32_t prr_budget_fit(prr_ctx* ctx, int32_t n, const int32_t* ctx_lens, const int32_t* budgets, int32_t degree) {
+  if (!ctx) return PRR_E_INVALID;
+  if (n < 1 || !ctx_lens || !budgets || degree < 0 || degree > 3) PRR_FAIL(ctx, PRR_E_INVALID, "prr_budget_fit: need n >= 1 points and 0 <= degree <= 3");
+  const int m = std::min(degree, n - 1) + 1;  // coefficients
+  double xs = 1.0;
+  for (int i = 0; i < n; ++i) { if (ctx_lens[i] < 1) PRR_FAIL(ctx, PRR_E_INVALID, "prr_budget_fit: context lengths must be >= 1"); xs = std::max(xs, (double)ctx_lens[i]); }
+  double A[4][5] = {};
+  for (int i = 0; i < n; ++i) {
+    const double x = ctx_lens[i] / xs;
+    double p[7] = {1, x, x * x, x * x * x, x * x * x * x, x * x * x * x * x, x * x * x * x * x * x};
+    for (int a = 0; a < m; ++a) { for (int b = 0; b < m; ++b) A[a][b] += p[a + b]; A[a][m] += p[a] * budgets[i]; }
+  }
+  for (int c0 = 0; c0 < m; ++c0) {
+    int piv = c0;
+    for (int rr = c0 + 1; rr < m; ++rr) if (std::fabs(A[rr][c0]) > std::fabs(A[piv][c0])) piv = rr;
+    if (std::fabs(A[piv][c0]) < 1e-12) PRR_FAIL(ctx, PRR_E_INVALID, "prr_budget_fit: the points do not determine a polynomial of this degree");
+    for (int b = 0; b <= m; ++b) std::swap(A[c0][b], A[piv][b]);
+    for (int rr = 0; rr < m; ++rr) {
+      if (rr == c0) continue;
+      const double f = A[rr][c0] / A[c0][c0];
+      for (int b = c0; b <= m; ++b) A[rr][b] -= f * A[c0][b];
+    }
+  }
+  ctx->bud_poly.assign(m, 0.0);
+  for (int a = 0; a < m; ++a) ctx->bud_poly[a] = A[a][m] / A[a][a];
+  ctx->bud_xscale = xs;
+  return PRR_OK;
+}
+
+extern "C" int32_t prr_budget_for(const prr_ctx* ctx, int32_t ctx_len, int32_t* budget_out) {
+  if (!ctx || !budget_out || ctx_len < 0) return PRR_E_INVALID;
+  if (ctx->bud_poly.empty()) { *budget_out = ctx->Bud; return PRR_OK; }  // nothing fitted: the budget of prr_create
+  const double x = ctx_len / ctx->bud_xscale;
+  double y = 0.0;
+  for (size_t a = ctx->bud_poly.size(); a-- > 0;) y = y * x + ctx->bud_poly[a];
+  const long v = std::lround(y);
+  *budget_out = (int32_t)std::min<long>(ctx->Bud, std::max<long>(0, v));
+  return PRR_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

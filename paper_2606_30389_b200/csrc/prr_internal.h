@@ -68,6 +68,9 @@ struct prr_ctx {
   cudaEvent_t ev_fork = nullptr, ev_spec = nullptr, ev_sel = nullptr;
   std::vector<cudaEvent_t> ev_upd; // per layer: EMA update of the last step of that layer done
   std::vector<char> upd_pending;
+  std::vector<int> bud_eff;        // per layer: blocks predicted for the next step, 0 .. Bud (prr_set_budget)
+  std::vector<double> bud_poly;    // fitted budget(context length): coefficients in x = ctx_len / bud_xscale (prr_budget_fit)
+  double bud_xscale = 1.0;
   std::vector<void*> allocs;
   int64_t launches = 0;
   std::string err;

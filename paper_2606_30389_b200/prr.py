@@ -23,6 +23,7 @@ FUSED, STREAMS = 0, 1
 SYMBOLS = [
     "prr_create", "prr_destroy", "prr_last_error", "prr_version", "prr_build_summaries", "prr_append",
     "prr_set_ema_params", "prr_reset_ema", "prr_calibrate", "prr_predict", "prr_ema_update", "prr_score",
+    "prr_set_budget", "prr_get_budget", "prr_profile_budget", "prr_budget_fit", "prr_budget_for",
     "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_step_append",
     "prr_decode_step_host",
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
@@ -246,6 +247,37 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().prr_launch_count(self._h))
+
+    # -- profiling-guided budget ------------------------------------------------------------
+    def set_budget(self, layer: int, budget: int, stream=None):
+        self._chk(lib().prr_set_budget(self._h, int(layer), int(budget), C.c_void_p(_stream(stream))))
+
+    def get_budget(self, layer: int) -> int:
+        v = C.c_int32(0)
+        self._chk(lib().prr_get_budget(self._h, int(layer), C.byref(v)))
+        return int(v.value)
+
+    def profile_budget(self, kv, q_traj, summaries, budgets, cold_l2=True, stream=None):
+        """-> (us per step for each budget, us per step of the sequential path, best budget)."""
+        n = len(budgets)
+        b = (C.c_int32 * n)(*[int(x) for x in budgets])
+        us = (C.c_float * n)()
+        seq = C.c_float(0.0)
+        best = C.c_int32(0)
+        self._chk(lib().prr_profile_budget(self._h, C.byref(kv), C.c_void_p(_p(q_traj)), int(q_traj.shape[0]),
+                                           C.c_void_p(_p(summaries)), b, n, int(bool(cold_l2)), us, C.byref(seq),
+                                           C.byref(best), C.c_void_p(_stream(stream))))
+        return list(us), float(seq.value), int(best.value)
+
+    def budget_fit(self, ctx_lens, budgets, degree=2):
+        n = len(ctx_lens)
+        self._chk(lib().prr_budget_fit(self._h, n, (C.c_int32 * n)(*[int(x) for x in ctx_lens]),
+                                       (C.c_int32 * n)(*[int(x) for x in budgets]), int(degree)))
+
+    def budget_for(self, ctx_len: int) -> int:
+        v = C.c_int32(0)
+        self._chk(lib().prr_budget_for(self._h, int(ctx_len), C.byref(v)))
+        return int(v.value)
 
     def set_option(self, option: int, value: int):
         self._chk(lib().prr_set_option(self._h, int(option), int(value)))

@@ -575,6 +575,64 @@ def test_streams_orchestration_full_size_and_graph():
     graph.destroy()
 
 
+@pytest.mark.parametrize("kernel", KERNELS, ids=KID.get)
+@pytest.mark.parametrize("cfg", [TINY, T128], ids=lambda c: c.name)
+def test_runtime_budget_varies_per_step(cfg, kernel):
+    """prr_set_budget (delta is a run-time choice): the budget changes between steps, down to
+    0 (no speculation) and back to the maximum; A, P, M stay bit-exact against the oracle run with the same
+    per-step budget, outputs in tolerance, PRR within 1e-5 of the sequential path."""
+    cfg, inp, gl, ol = make(cfg, kernel=kernel, steps=8)
+    twin = H.GpuLayer(cfg, inp, kernel=kernel)
+    gl.calibrate(inp.q_cal); twin.calibrate(inp.q_cal); ol.calibrate(synth.bits(inp.q_cal))
+    plan = [cfg.Bud, cfg.K, 3, 0, 0, cfg.Bud, 1, cfg.K // 2]
+    for t in range(8):
+        gl.ctx.set_budget(0, plan[t]); ol.budget = plan[t]
+        assert gl.ctx.get_budget(0) == plan[t]
+        out = gl.step_append(t)
+        twin.append(t); o2 = twin.step(t, sequential=True)
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+        for b in range(cfg.B):
+            for h in range(cfg.Hkv):
+                assert len(r["P"][b][h]) <= plan[t]
+        H.compare_sets(gl, r, f"budget {plan[t]} t{t}")
+        H.check_out(out.cpu().numpy(), r["out"], f"budget {plan[t]} t{t}")
+        assert (out - o2).abs().max().item() <= 1e-5
+    with pytest.raises(prr.PrrError):
+        gl.ctx.set_budget(0, cfg.Bud + 1)
+
+
+def test_profile_budget_leaves_no_trace_and_fit():
+    """prr_profile_budget sweeps candidate budgets on the layer's cache (section 4.4 in the library) and
+    restores the predictor state: the decode steps after it still match the oracle bit-exactly.  prr_budget_fit /
+    prr_budget_for: a polynomial through profiled points, pinned on exactly representable data."""
+    cfg, inp, gl, ol = make(TINY, steps=6)
+    gl.calibrate(inp.q_cal); ol.calibrate(synth.bits(inp.q_cal))
+    for t in range(2):
+        gl.step_append(t); ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t])); r = ol.step(synth.bits(inp.q_dec[t]))
+    cands = [0, 4, cfg.K, cfg.Bud]
+    us, seq_us, best = gl.ctx.profile_budget(gl.kv, inp.q_cal.contiguous(), gl.summ, cands, cold_l2=False)
+    assert len(us) == 4 and all(0.5 < u < 5000 for u in us) and 0.5 < seq_us < 5000
+    assert best in cands
+    assert gl.ctx.get_budget(0) == cfg.Bud
+    for t in range(2, 6):
+        out = gl.step_append(t)
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t])); r = ol.step(synth.bits(inp.q_dec[t]))
+        H.compare_sets(gl, r, f"after profiling t{t}")
+        H.check_out(out.cpu().numpy(), r["out"], f"after profiling t{t}")
+    c = gl.ctx
+    assert c.budget_for(12345) == cfg.Bud                          # nothing fitted yet: the budget of prr_create
+    c.budget_fit([4096, 8192, 16384, 32768], [12, 10, 6, 2], degree=3)   # 4 points, degree 3: interpolation
+    assert [c.budget_for(x) for x in (4096, 8192, 16384, 32768)] == [12, 10, 6, 2]
+    c.budget_fit([1000, 2000, 3000], [3, 5, 7], degree=1)                # exactly linear data
+    assert [c.budget_for(x) for x in (1000, 1500, 2000, 2500, 3000)] == [3, 4, 5, 6, 7]
+    assert c.budget_for(0) == 1 and c.budget_for(10 ** 6) == cfg.Bud     # clamped to [0, budget of prr_create]
+    c.budget_fit([5000], [9], degree=2)                                  # one point: a constant
+    assert c.budget_for(1) == 9 and c.budget_for(99999) == 9
+
+
 def test_graph_replay_matches_eager():
     cfg, inp, gl, ol = make(TINY)
     _, _, g2, _ = make(TINY)
