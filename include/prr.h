@@ -52,6 +52,12 @@ enum { PRR_DROP = 0, PRR_RETAIN = 1 };
  * speculative attention, repair and merge are ordered by device-scope counters.
  * PRR_STREAMS: the paper's orchestration, one kernel per stage on two event-ordered streams. */
 enum { PRR_FUSED = 0, PRR_STREAMS = 1 };
+/* The paper's ablation ladder (Table 2).  S3 (default): the EMA predictor with its budget and
+ * incremental repair.  S2: the prediction is the last step's true top-K (theta = (1, 1, 0), budget = K) with
+ * incremental repair.  S1: the same prediction, but ANY miss in a row discards the speculative result and
+ * attention is recomputed over all of A (the fallback PRR avoids).  The output is attention over
+ * A in every mode; the modes differ in the work on the critical path. */
+enum { PRR_MODE_S3 = 0, PRR_MODE_S2 = 1, PRR_MODE_S1 = 2 };
 
 typedef struct prr_ctx prr_ctx; /* opaque, library-owned */
 
@@ -77,7 +83,8 @@ typedef struct {
 } prr_paged_kv;
 
 /* Problem statement (PAPER.md:109 Eq. 1, :135): block size, top-K of the DSA, speculation budget
- * |P| <= budget = delta*K.  block_size in {16,32,64,128}; 1 <= K <= 512; 0 <= budget <= 1024. */
+ * |P| <= budget = delta*K.  block_size in {16,32,64,128,256}; 1 <= K <= 512; 0 <= budget <= 1024.  Blocks of 256
+ * tokens run on the fused cluster kernel only (the stage calls and PRR_STREAMS return PRR_E_UNSUPPORTED). */
 int32_t prr_create(const prr_layout* layout, int32_t block_size, int32_t K, int32_t budget,
                    prr_ctx** out);
 int32_t prr_destroy(prr_ctx* ctx);
@@ -162,6 +169,11 @@ int32_t prr_profile_budget(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_t
 int32_t prr_budget_fit(prr_ctx* ctx, int32_t n, const int32_t* ctx_lens /* host */, const int32_t* budgets /* host */,
                        int32_t degree);
 int32_t prr_budget_for(const prr_ctx* ctx, int32_t ctx_len, int32_t* budget_out /* host */);
+
+/* Ablation modes (see PRR_MODE_*).  S2 / S1 set theta = (1, 1, 0) for every (layer, sequence) and the budget
+ * to min(K, budget of prr_create); S3 leaves theta and the budget as they are (calibrate / set them).  S1
+ * needs PRR_DROP and PRR_FUSED and runs on the cluster kernel. */
+int32_t prr_set_mode(prr_ctx* ctx, int32_t mode, void* stream);
 
 /* --- selection (a1, a2) ---------------------------------------------------------------------- */
 

@@ -65,6 +65,7 @@ struct RowArgs {
   int32_t* setA; int32_t* setM; int32_t* counts;
   uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, retain, spec, cut;
+  int recompute;  // ablation S1: any miss in the row -> the speculative result is discarded, all of A is fetched
   int CS, NBUF, NSLOT, UCAP, HL, SLMAX, NBH, BudSel;  // BudSel <= Bud: the run-time budget of the NEXT prediction
   // dynamic shared memory offsets (bytes)
   int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
@@ -709,6 +710,8 @@ struct Sh {  // static shared memory
   int chunk_cnt[NBMAX];
   volatile int pos_unit[NBMAX];
   volatile int patch_ready;  // the open block's new summary row is in patch_row
+  volatile int no_hits;      // S1: the row had a miss, nothing speculative is used
+  int miss_cnt;
   alignas(16) uint32_t patch_row[64];
 };
 
@@ -761,7 +764,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
   auto row_init = [&]() {
     if (tid == 0) {
       sh.q_total = 0; sh.q_final = 0; sh.sel_done = 0; sh.spec_ready = 0; sh.n_rep = 0;
-      sh.t_next = 0; sh.n_slots = 0; sh.rep_cnt = 0; sh.patch_ready = 0;
+      sh.t_next = 0; sh.n_slots = 0; sh.rep_cnt = 0; sh.patch_ready = 0; sh.no_hits = 0; sh.miss_cnt = 0;
     }
     for (int i = tid; i < NTW * SLOTF; i += NTHR) slots[(size_t)a.NSLOT * SLOTF + i] = (i % SW) == 0 ? -CUDART_INF_F : 0.f;
     for (int i = tid; i < a.MBw; i += NTHR) { pmask[i] = 0u; amask[i] = 0u; }
@@ -955,7 +958,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             while (u_spec < n_spec) {  // next speculative unit worth a request
               const int blk = units[u_spec].x;
               bool skip = blk < 0;
-              if (!skip && nrep >= 0 && a.cut && !a.retain) skip = !((amask[blk >> 5] >> (blk & 31)) & 1u);
+              if (!skip && nrep >= 0 && !a.retain) skip = sh.no_hits || (a.cut && !((amask[blk >> 5] >> (blk & 31)) & 1u));
               if (!skip) break;
               ++u_spec; sub_spec = 0;
             }
@@ -1264,7 +1267,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             int f = -1;
             if (lane == 0 && sh.sel_done) {
               __threadfence_block();
-              f = (int)((amask[blk >> 5] >> (blk & 31)) & 1u);
+              f = sh.no_hits ? 0 : (int)((amask[blk >> 5] >> (blk & 31)) & 1u);
             }
             return __shfl_sync(FULL, f, 0);
           };
@@ -1364,9 +1367,18 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         if (g.tid == 0) wait_flag(&sh.spec_ready, err, 10);
         g.sync();
         // repair units: the missed blocks of this CTA's slice (all of A's in the sequential path)
+        bool all_rep = false;
+        if (a.recompute && !a.retain) {  // S1: does the row have a miss at all?  (every CTA holds the whole bitmasks)
+          int mc = 0;
+          for (int w = g.tid; w < (nb + 31) >> 5; w += g.nt) mc += __popc(amask[w] & ~pmask[w]);
+          mc = __reduce_add_sync(FULL, mc);
+          if (lane == 0 && mc) atomicAdd(&sh.miss_cnt, mc);
+          g.sync();
+          all_rep = sh.miss_cnt > 0;
+        }
         for (int i = s0 + g.tid; i < min(s1, nb); i += g.nt) {
           const uint32_t bit = 1u << (i & 31);
-          if ((amask[i >> 5] & bit) && !(pmask[i >> 5] & bit)) {
+          if ((amask[i >> 5] & bit) && (all_rep || !(pmask[i >> 5] & bit))) {
             const int pos = atomicAdd(&sh.rep_cnt, 1);
             units[UREP0 + pos] = make_int2(i, tslice[i - s0]);
           }
@@ -1374,6 +1386,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
         g.sync();
         if (g.tid == 0) {
           sh.n_rep = sh.rep_cnt;
+          sh.no_hits = all_rep ? 1 : 0;
           __threadfence_block();
           sh.sel_done = 1;
         }
@@ -1479,7 +1492,7 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           for (int e = 0; e < nsl + NTW; ++e) {
             if (e < nsl) {
               const int blk = slotblk[e] & 0xfffff;
-              if (!a.retain && !((amask[blk >> 5] >> (blk & 31)) & 1u)) continue;
+              if (!a.retain && (sh.no_hits || !((amask[blk >> 5] >> (blk & 31)) & 1u))) continue;
             }
             const float* st = slots + (size_t)(e < nsl ? e : a.NSLOT + (e - nsl)) * SLOTF + gq * SW;
             const float me = st[0], le = st[1];
@@ -1618,7 +1631,7 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
   if (CS > 1 && ncl < R) return cudaErrorInvalidConfiguration;
   a.CS = CS;
   a.HL = (a.G + CS - 1) / CS;
-  a.UCAP = (a.Bud + CS - 1) / CS + a.K;
+  a.UCAP = (a.Bud + CS - 1) / CS + a.K;  // (S1 makes every block of A in the slice a repair unit: <= K)
   a.SLMAX = ((((a.MB + 3) & ~3) + CS - 1) / CS + 3 + 4) & ~3;
   const int SW = D + 4, SLOTF = a.G * SW;
   // a slot per speculative unit of a CTA if they fit (a unit whose fate is unknown and that finds no slot
@@ -1744,6 +1757,7 @@ int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.cut = c->cut;
+  a.recompute = c->mode == PRR_MODE_S1 ? 1 : 0;
   a.scale = c->sm_scale; a.score_c = c->score_c;
   cudaError_t e = cudaErrorInvalidValue;
 #define PRR_CASE(DD, SS) if (c->D == DD && ST == SS) e = plan_and_launch<DD, SS>(c, a, s);

@@ -76,8 +76,10 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   const int G = lay->n_q_heads / lay->n_kv_heads;
   if (lay->head_dim != 64 && lay->head_dim != 128)
     PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: head_dim must be 64 or 128");
-  if (block_size != 16 && block_size != 32 && block_size != 64 && block_size != 128)
-    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: block_size must be 16, 32, 64 or 128");
+  if (block_size != 16 && block_size != 32 && block_size != 64 && block_size != 128 && block_size != 256)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: block_size must be 16, 32, 64, 128 or 256");
+  if (block_size == 256 && lay->orchestration != PRR_FUSED)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: block_size 256 needs PRR_FUSED");
   if (G > 16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: GQA group > 16 unsupported");
   if (lay->kv_dtype != PRR_BF16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: kv_dtype must be PRR_BF16");
   if (lay->max_blocks_per_seq > 32768 || K > 512 || budget > 1024)
@@ -405,6 +407,24 @@ static void repredict(prr_ctx* c, int layer, cudaStream_t s) {  // P of the next
   sync_pred(c, layer, 0, c->maxB, s);
 }
 
+extern "C" int32_t prr_set_mode(prr_ctx* ctx, int32_t mode, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (mode != PRR_MODE_S3 && mode != PRR_MODE_S2 && mode != PRR_MODE_S1) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_mode: unknown mode");
+  if (mode == PRR_MODE_S1 && (ctx->lay.overpredict_policy != PRR_DROP || !ctx->fused))
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_mode: S1 (recompute on any miss) needs PRR_DROP and PRR_FUSED");
+  ctx->mode = mode;
+  if (mode == PRR_MODE_S3) return PRR_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  for (int l = 0; l < ctx->NL; ++l) {  // "reuse the last step's top-K": alpha = beta = 1, gamma = 0, |P| = K
+    join_layer(ctx, l, s);
+    k_set_theta<<<(ctx->maxB + 63) / 64, 64, 0, s>>>(ctx->theta + (size_t)l * ctx->maxB * 3, ctx->maxB, 1.0, 1.0, 0.0);
+    ctx->launches++;
+    ctx->bud_eff[l] = std::min(ctx->K, ctx->Bud);
+    repredict(ctx, l, s);
+  }
+  return check_launch(ctx, "prr_set_mode");
+}
+
 extern "C" int32_t prr_set_budget(prr_ctx* ctx, int32_t layer, int32_t budget, void* stream) {
   if (!ctx) return PRR_E_INVALID;
   if (layer < -1 || layer >= ctx->NL || budget < 0 || budget > ctx->Bud)
@@ -574,6 +594,7 @@ extern "C" int32_t prr_topk(prr_ctx* ctx, const float* scores, const int32_t* n_
 extern "C" int32_t prr_speculate(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* P,
                                  float* O_part, float* m_part, float* l_part, void* stream) {
   CHECK_KV("prr_speculate");
+  if (ctx->bs > 128) PRR_FAIL(ctx, PRR_E_UNSUPPORTED, "prr_speculate: blocks of 256 tokens run on the fused step only");
   CHECK_PTR(q, "prr_speculate");
   if (!P || !O_part || !m_part || !l_part) PRR_FAIL(ctx, PRR_E_INVALID, "prr_speculate: null argument");
   if (ctx->Bud < 1) PRR_FAIL(ctx, PRR_E_STATE, "prr_speculate: ctx was created with budget 0");
@@ -585,6 +606,7 @@ extern "C" int32_t prr_repair(prr_ctx* ctx, const prr_paged_kv* kv, const void* 
                               const int32_t* P, const float* O_part, const float* m_part,
                               const float* l_part, float* out, float* m_out, float* l_out, void* stream) {
   CHECK_KV("prr_repair");
+  if (ctx->bs > 128) PRR_FAIL(ctx, PRR_E_UNSUPPORTED, "prr_repair: blocks of 256 tokens run on the fused step only");
   CHECK_PTR(q, "prr_repair");
   if (!A || !out) PRR_FAIL(ctx, PRR_E_INVALID, "prr_repair: null argument");
   if (P && (!O_part || !m_part || !l_part)) PRR_FAIL(ctx, PRR_E_INVALID, "prr_repair: P given without its partial states");
@@ -633,6 +655,7 @@ static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const v
   const int rows = kv->batch * c->Hkv;
   int kern = c->kernel;
   if (kern == 0) kern = rows >= 64 ? 2 : 1;
+  if (c->bs > 128 || c->mode == PRR_MODE_S1) kern = 2;  // (only the cluster kernel cuts a block into sub-tiles / recomputes on a miss)
   if (kern == 1 && !c->coop) kern = 2;
   c->last_kernel = kern;
   const int e = kern == 2 ? launch_step_cluster(c, kv, q, summaries, out, spec, s, k_new, v_new)

@@ -51,6 +51,7 @@ struct prr_ctx {
   // fused step (k_row.cu): per kernel instantiation, attribute set + co-resident clusters of 1, 2, 4, 8 CTAs
   int row_attr[6] = {0, 0, 0, 0, 0, 0}; int row_maxcl[6][4] = {}; int row_dyn[6] = {};
   int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;
+  int mode = 0;                                  // PRR_MODE_S3 (EMA + repair) | _S2 (reuse + repair) | _S1 (reuse + recompute on any miss)
   int kernel = 0;                                // fused step: 0 auto, 1 persistent cooperative grid (k_step.cu), 2 cluster per row (k_row.cu)
   int last_kernel = 0; int pace_pct = 100; float hbm_gbs_est = 6400.f; bool coop_attr[8] = {};          // tuning: cluster size override, programmatic dependent launch, early cut
   int last_cs = 0, last_nbuf = 0, last_grid = 0; // launch shape of the last fused step (introspection)

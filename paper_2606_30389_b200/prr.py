@@ -18,12 +18,13 @@ DROP, RETAIN = 0, 1
 OPT_PDL, OPT_CLUSTER, OPT_CUT, OPT_SUBTILE, OPT_KERNEL, OPT_PACE = 0, 1, 2, 3, 4, 5
 OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID, OPT_LAST_KERNEL = 16, 17, 18, 19
 KERNEL_AUTO, KERNEL_PERSISTENT, KERNEL_CLUSTER = 0, 1, 2
+MODE_S3, MODE_S2, MODE_S1 = 0, 1, 2
 FUSED, STREAMS = 0, 1
 
 SYMBOLS = [
     "prr_create", "prr_destroy", "prr_last_error", "prr_version", "prr_build_summaries", "prr_append",
     "prr_set_ema_params", "prr_reset_ema", "prr_calibrate", "prr_predict", "prr_ema_update", "prr_score",
-    "prr_set_budget", "prr_get_budget", "prr_profile_budget", "prr_budget_fit", "prr_budget_for",
+    "prr_set_mode", "prr_set_budget", "prr_get_budget", "prr_profile_budget", "prr_budget_fit", "prr_budget_for",
     "prr_topk", "prr_speculate", "prr_repair", "prr_attend", "prr_decode_step", "prr_step_append",
     "prr_decode_step_host",
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
@@ -247,6 +248,9 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().prr_launch_count(self._h))
+
+    def set_mode(self, mode: int, stream=None):
+        self._chk(lib().prr_set_mode(self._h, int(mode), C.c_void_p(_stream(stream))))
 
     # -- profiling-guided budget ------------------------------------------------------------
     def set_budget(self, layer: int, budget: int, stream=None):

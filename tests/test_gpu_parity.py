@@ -633,6 +633,48 @@ def test_profile_budget_leaves_no_trace_and_fit():
     assert c.budget_for(1) == 9 and c.budget_for(99999) == 9
 
 
+@pytest.mark.parametrize("mode,kernel", [(prr.MODE_S2, prr.KERNEL_PERSISTENT), (prr.MODE_S2, prr.KERNEL_CLUSTER),
+                                         (prr.MODE_S1, None), (prr.MODE_S3, None)], ids=["S2-persistent", "S2-cluster", "S1", "S3"])
+@pytest.mark.parametrize("cfg", [TINY, T128], ids=lambda c: c.name)
+def test_ablation_modes(cfg, mode, kernel):
+    """S1 = reuse the last top-K and recompute on any miss, S2 = reuse + repair, S3 = EMA + repair.
+    S1 / S2 predict P_t = A_{t-1} (the oracle with theta = (1, 1, 0), budget K: pinned in test_oracle_pins); the
+    output is attention over A in every mode, the modes differ in the work done."""
+    cfg, inp, gl, ol = make(cfg, kernel=kernel)
+    if mode == prr.MODE_S3:
+        gl.calibrate(inp.q_cal); ol.calibrate(synth.bits(inp.q_cal))
+    gl.ctx.set_mode(mode)
+    if mode != prr.MODE_S3:
+        ol.theta = [(1.0, 1.0, 0.0)] * cfg.B
+        ol.budget = min(cfg.K, cfg.Bud)
+    prevA = None
+    for t in range(cfg.steps):
+        out = gl.step_append(t)
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+        A, P, M = H.compare_sets(gl, r, f"mode {mode} t{t}")
+        if mode != prr.MODE_S3 and prevA is not None:
+            assert np.array_equal(P[..., :cfg.K], prevA)               # the prediction IS the last true set
+        prevA = A
+        H.check_out(out.cpu().numpy(), r["out"], f"mode {mode} t{t}")
+    if mode == prr.MODE_S1:
+        assert gl.ctx.get_option(prr.OPT_LAST_KERNEL) == prr.KERNEL_CLUSTER
+    gl.ctx.check()
+
+
+def test_block_size_256():
+    """Table 3 of the paper sweeps block sizes 16 .. 256: a 256-token block is four sub-tiles of the
+    cluster kernel; whole steps against the oracle, open block ragged."""
+    cfg = synth.Config("T256", B=2, L=1, Hq=8, Hkv=2, d=128, ctx_lo=256 * 9 + 5, ctx_hi=256 * 12 + 201, bs=256, K=3, Bud=5,
+                       rho=0.9, steps=6, T_cal=8)
+    run_decode(cfg, fused_append=True)
+    run_decode(cfg, policy=prr.RETAIN)
+    with pytest.raises(prr.PrrError) as e:
+        prr.Context(8, 2, 128, 256, 3, 5, orchestration=prr.STREAMS)
+    assert e.value.code == prr.E_UNSUPPORTED
+
+
 def test_graph_replay_matches_eager():
     cfg, inp, gl, ol = make(TINY)
     _, _, g2, _ = make(TINY)
