@@ -2,6 +2,7 @@
 """bench.py — per-layer DSA decode critical path of PRR on B200 (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--layers R] [--impl reference]
+                    [--budget profiled|config] [--kernel auto|persistent|cluster] [--sweep]
 
 A "step" is ONE LAYER-STEP: one pass of the whole hot path (append + summary refresh, score, top-K,
 diff, EMA predict/update, speculative attention over P, repair of A\\P, merge: ONE fused launch)
@@ -32,8 +33,19 @@ import torch
 
 from paper_2606_30389_b200 import synth
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_step launch (ncu --set full, profiles/r1_k_step_C2.md)
-NCU_TRAFFIC = {"C2": 32_050_000}
+
+def ncu_traffic(cfg_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one fused-step launch, from the tracked ncu summary of
+    this round (profiles/r2_traffic_<config>.md, a line `traffic_bytes_per_launch: N`); None if absent."""
+    p = os.path.join(ROOT, "profiles", f"r2_traffic_{cfg_name}.md")
+    try:
+        for line in open(p):
+            if line.startswith("traffic_bytes_per_launch:"):
+                return int(float(line.split(":")[1].split()[0]))
+    except OSError:
+        pass
+    return None
+
 
 METRIC = "per_layer_dsa_decode_critical_path"
 UNIT = "us"
@@ -138,6 +150,39 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
+# ---- N > 1: one process per GPU, no data-path collective (rows are independent: DESIGN.md section 6).  The
+# process group only carries the barrier around the timed region and the max-over-ranks of the device
+# time; tests/test_dist_host.py runs these helpers with the gloo backend, world size 2, on CPU.
+def rank_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")),
+            int(os.environ.get("WORLD_SIZE", "1")))
+
+
+def dist_init(world, local, use_cuda=True):
+    if world <= 1:
+        return None
+    import torch.distributed as dist
+    if use_cuda:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    else:
+        dist.init_process_group("gloo")
+    return dist
+
+
+def max_over_ranks(x, dist, device="cpu"):
+    """Whole-job time = the slowest rank's device time."""
+    if dist is None:
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def rank_seed_offset(rank):
+    """Weak scaling: every rank draws its own sequences (seed + rank)."""
+    return rank
+
+
 def workload_name(cfg, R):
     return (f"{cfg.name}: batch {cfg.B}, {cfg.Hq}q/{cfg.Hkv}kv heads, d={cfg.d}, ctx {cfg.ctx_lo}"
             + (f"-{cfg.ctx_hi}" if cfg.ctx_hi != cfg.ctx_lo else "") +
@@ -149,7 +194,7 @@ def workload_name(cfg, R):
 class Stack:
     """R layers of the workload resident in HBM + the library context."""
 
-    def __init__(self, cfg, R, tokens, dev, seed_off=0):
+    def __init__(self, cfg, R, tokens, dev, seed_off=0, kernel=0):
         from paper_2606_30389_b200 import prr
         self.prr, self.cfg, self.R, self.dev = prr, cfg, R, dev
         self.inps = [synth.make_layer(cfg.scaled(seed=cfg.seed + seed_off), l, device=dev, steps=tokens,
@@ -157,6 +202,7 @@ class Stack:
         self.MB = self.inps[0].block_table.shape[1]
         self.ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B,
                                max_blocks_per_seq=self.MB, n_layers=R)
+        self.ctx.set_option(prr.OPT_KERNEL, kernel)
         self.kvs, self.summ = [], []
         for l, inp in enumerate(self.inps):
             kv = self.ctx.kv(inp.k_pages, inp.v_pages, inp.block_table, inp.seq_lens, l)
@@ -182,6 +228,14 @@ class Stack:
                 self.ctx.calibrate(l, b, trajs[b].contiguous(), want_host=False)
         torch.cuda.synchronize()
         return time.perf_counter() - t0
+
+    def profile_budget(self, candidates):
+        """prr_profile_budget on layer 0 with its prefill query trajectory (section 4.4): (us per budget,
+        us of the sequential path, best budget).  The budget is then set for every layer."""
+        inp = self.inps[0]
+        us, seq_us, best = self.ctx.profile_budget(self.kvs[0], inp.q_cal.contiguous(), self.summ[0], candidates,
+                                                   cold_l2=True)
+        return us, seq_us, best
 
     def enqueue(self, n, stream, sequential=False):
         """Enqueue the next n layer-steps (append + PRR step) on `stream`."""
@@ -216,6 +270,52 @@ def timed_launch(graphs, stream):
     return e0.elapsed_time(e1)            # ms
 
 
+def sweep(args):
+    """Table-3-shaped sweep: block size {16 .. 256} x token budget {1K .. 8K} at 128K context,
+    32 q / 8 kv heads, d = 128, batch 1: the sparse-attention work of a step (the sequential fused step: score,
+    top-K, attention over the selected blocks, merge) in us and as a fraction of the HBM roofline of that cell
+    (summaries + selected KV).  One line per cell, then one JSON line."""
+    from paper_2606_30389_b200 import prr
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(0)
+    peak, peak_src = peaks()
+    stream = torch.cuda.Stream(device=dev)
+    cells = []
+    for bs in (16, 32, 64, 128, 256):
+        for tokens in (1024, 2048, 4096, 6144, 8192):
+            K = tokens // bs
+            if K > 512:
+                cells.append({"block": bs, "tokens": tokens, "skipped": "K > 512 blocks"})
+                continue
+            cfg = synth.Config(f"S{bs}_{tokens}", B=1, L=1, Hq=32, Hkv=8, d=128, ctx_lo=131072, ctx_hi=131072, bs=bs, K=K,
+                               Bud=min(1024, K + K // 2), rho=0.95, steps=8, T_cal=8)
+            R, n = 8, 256
+            st = Stack(cfg, R, n // R + 8, dev, kernel={"auto": 0, "persistent": 1, "cluster": 2}[args.kernel])
+            for l in range(R):
+                st.ctx.set_ema_params(l, -1, 0.6, 0.2, 0.5)
+            res = {}
+            for seq in (True, False):
+                with torch.cuda.stream(stream):
+                    st.enqueue(16, stream, sequential=seq)
+                torch.cuda.synchronize()
+                g = st.capture(n, stream, sequential=seq)
+                torch.cuda.synchronize()
+                res[seq] = timed_launch(g, stream) * 1e3 / n
+                for x in g:
+                    x.destroy()
+            st.ctx.check()
+            ab = algorithmic_bytes(cfg, 131072 + 20)
+            cell = {"block": bs, "tokens": tokens, "K": K, "sequential_us": round(res[True], 2), "prr_us": round(res[False], 2),
+                    "bytes": int(ab), "frac_sequential": round(ab / (res[True] * 1e-6) / 1e9 / peak, 3),
+                    "kernel": st.ctx.get_option(prr.OPT_LAST_KERNEL)}
+            cells.append(cell)
+            print(json.dumps(cell), file=sys.stderr, flush=True)
+            del st
+            torch.cuda.empty_cache()
+    print(json.dumps({"sweep": "block size x token budget, 128K context, 32q/8kv, d=128, batch 1 (PAPER.md Table 3 shape)",
+                      "peak_gbs": peak, "peak_source": peak_src, "cells": cells}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -227,10 +327,15 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=512)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-seq", action="store_true", help="skip the sequential select-then-attend leg")
+    ap.add_argument("--budget", default="profiled", choices=["profiled", "config"],
+                    help="speculation budget: chosen by prr_profile_budget among candidates <= the config's (PAPER.md "
+                         "section 4.4), or the config's fixed one")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "persistent", "cluster"])
+    ap.add_argument("--sweep", action="store_true", help="Table-3-shaped sweep: block size x token budget at 128K, 32q/8kv")
     args = ap.parse_args()
 
-    rank = int(os.environ.get("RANK", "0"))
-    if int(os.environ.get("LOCAL_RANK", "0")) == 0 and args.impl != "reference":
+    rank, local, world = rank_env()
+    if local == 0 and args.impl != "reference":
         from paper_2606_30389_b200 import build as _b       # incremental: a no-op when libprr.so is up to date
         _b.build()
     elif args.impl != "reference":                          # the other ranks wait for rank 0's build
@@ -239,9 +344,9 @@ def main():
             if os.path.exists(_b.LIB) and not os.path.exists(_b.LIB + ".lock"):
                 break
             time.sleep(0.5)
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     cfg = synth.CONFIGS[args.config]
+    if args.sweep:
+        return sweep(args)
     if args.impl == "reference":
         if args.steps == 16384:
             args.steps, args.warmup = 12, 3
@@ -249,20 +354,31 @@ def main():
         return
     args.warmup = max(args.warmup, 3)
 
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dist = dist_init(world, local)
     torch.cuda.set_device(local)
     dev = torch.device(f"cuda:{local}")
     R = args.layers
     K, W = args.steps, args.warmup
     E = args.e2e_steps
     seq_steps = 0 if args.no_seq else min(K, 4096)
-    total = 3 * W + K + seq_steps + E
+    total = 4 * W + K + seq_steps + E + min(K, 2048)
     tokens = (total + R - 1) // R + 2
-    st = Stack(cfg, R, tokens, dev, seed_off=rank)          # weak scaling: every rank its own sequences
+    kern = {"auto": 0, "persistent": 1, "cluster": 2}[args.kernel]
+    st = Stack(cfg, R, tokens, dev, seed_off=rank_seed_offset(rank), kernel=kern)
     cal_s = st.calibrate()
     stream = torch.cuda.Stream(device=dev)
+    # ---- speculation budget: the library's profiling-guided choice (PAPER.md 204-208), capped by the config's
+    budget_info = {"mode": args.budget, "config_budget": cfg.Bud, "budget": cfg.Bud}
+    if args.budget == "profiled" and cfg.Bud > 0:
+        cands = sorted({0, cfg.K // 4, cfg.K // 2, (3 * cfg.K) // 4, cfg.K, (cfg.K + cfg.Bud) // 2, cfg.Bud})
+        us_b, seq_b, best = st.profile_budget(cands)
+        if world > 1:                                       # one choice for the job: rank 0's
+            tb = torch.tensor([best], device=dev)
+            dist.broadcast(tb, 0)
+            best = int(tb.item())
+        st.ctx.set_budget(-1, best)
+        budget_info.update(budget=best, delta=best / cfg.K, candidates=cands, us_per_candidate=[round(u, 2) for u in us_b],
+                           us_sequential_profiled=round(seq_b, 2))
 
     def barrier():
         torch.cuda.synchronize()
@@ -288,11 +404,25 @@ def main():
     for g in graphs:
         g.destroy()
     stats = st.ctx.get_stats(reset=True)
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, dev)
     us_step = ms * 1e3 / K
+
+    # ---- PRR at the config's fixed budget, same protocol (what the profiled budget is compared with) --
+    fixed_us = None
+    if budget_info["budget"] != cfg.Bud and not args.no_seq:
+        st.ctx.set_budget(-1, cfg.Bud)
+        with torch.cuda.stream(stream):
+            st.enqueue(W, stream)
+        torch.cuda.synchronize()
+        n_f = min(K, 2048)
+        g3 = st.capture(n_f, stream)
+        barrier()
+        fixed_us = timed_launch(g3, stream) * 1e3 / n_f
+        for g in g3:
+            g.destroy()
+        st.ctx.set_budget(-1, budget_info["budget"])
+        st.ctx.get_stats(reset=True)
+    budget_info["us_at_config_budget"] = fixed_us
 
     # ---- in-library sequential select-then-attend, same protocol --------------------------------
     seq_us = None
@@ -326,14 +456,12 @@ def main():
             st.ctx.decode_step_host(st.kvs[l], qh[l][t], kh[l][t], vh[l][t], st.summ[l], oh, stream=stream)
             st.pos += 1
         e_us = (time.perf_counter() - w0) / E * 1e6
-        if world > 1:
-            t = torch.tensor([e_us], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_us = float(t.item())
+        e_us = max_over_ranks(e_us, dist, dev)
         e2e = {"value": e_us, "unit": UNIT,
                "h2d_bytes_per_step": int(cfg.B * (cfg.Hq + 2 * cfg.Hkv) * cfg.d * 2),
                "d2h_bytes_per_step": int(cfg.B * cfg.Hq * cfg.d * 4)}
 
+    st.ctx.check()                                          # no fused step ever gave up on a dependency
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -356,11 +484,15 @@ def main():
                           "frac_of_nominal_8TBs": abytes / (us_step * 1e-6) / 1e9 / 8000.0, "peak_source": peak_src},
         "sequential_us": seq_us, "speedup_vs_sequential": (seq_us / us_step) if seq_us else None,
         "hit_rate": stats[1] / max(stats[0], 1), "mean_missed_per_row": stats[2] * K and stats[2] / (K * cfg.B * cfg.Hkv),
-        "roofline": {"kernel": "k_step (fused persistent layer-step: append, score, top-K, EMA, speculative "
-                               "units, repair, merge in one cooperative launch)",
+        "budget": budget_info,
+        "fused_kernel": {1: "k_step (persistent cooperative grid, warps as workers)",
+                         2: "k_row (one thread-block cluster per (sequence, KV head) row)"}.get(
+                             st.ctx.get_option(st.prr.OPT_LAST_KERNEL), "?"),
+        "roofline": {"kernel": "the fused layer-step (append, score, top-K, EMA, speculative units, repair, merge in ONE "
+                               "launch): " + {1: "k_step", 2: "k_row"}.get(st.ctx.get_option(st.prr.OPT_LAST_KERNEL), "?"),
                      "bound": "hbm", "achieved": abytes / (us_step * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": abytes / (us_step * 1e-6) / 1e9 / peak,
-                     "traffic": NCU_TRAFFIC.get(cfg.name), "us_per_launch": us_step, "launches_per_step": 1,
+                     "traffic": ncu_traffic(cfg.name), "us_per_launch": us_step, "launches_per_step": 1,
                      "units_per_launch": 1, "bytes_per_unit": int(abytes), "peak_source": peak_src,
                      "how": "algorithmic bytes of one layer-step (summaries + selected KV, SURVEY.md 8(d)) / "
                             "(timed region / K launches); the step is latency-bound, not bandwidth-bound: see "
