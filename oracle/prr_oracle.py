@@ -14,6 +14,10 @@ What each part is, and what pins it (tests/test_oracle_pins.py; readings Q1..Q15
                  pins: identical keys -> that key; brute force; power-of-two counts exact
   score          group-aggregated scaled logit against the summary (A.1 PAPER.md:372)
                  pins: exact big-integer dot product; G=1 plain matmul; linearity; x2 scaling bit-exact
+  summarize_quest / score_quest   Quest's channel-wise min / max page metadata and its upper-bound score
+                 with the GQA mean query, s = sum_i max(Qbar_i m_i, Qbar_i M_i) (A.1)
+                 pins: per-channel python loops; G = 1 = Quest's MHA form; m == M -> the mean-summary score
+                 bit for bit; s >= the mean query's logit with EVERY token of the block; x2 scaling
   topk           K highest scores, ties -> lower index (BASELINE.json north_star)
                  pins: brute-force python sort incl. duplicates, K>=n, all-equal, permutation invariant
   ema_*          Eq. 2 / Eq. 3, init l=IS, v=0
@@ -132,6 +136,51 @@ def score(q_bits, summ_bits, n_blocks) -> np.ndarray:
             s = np.zeros(nb, dtype=np.float64)
             for g in range(G):
                 s = s + kbar @ q[b, h * G + g]
+            out[b, h, :nb] = f64_to_f32(s * c)
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# 2b. Quest scoring extended to GQA — A.1: "we first compute a representative query
+#     Qbar = (1/G) sum_g Q_g ... maintain the corresponding channel-wise minimum and maximum key
+#     metadata (m_p, M_p) ... the importance score of page p is
+#     s_p = sum_i max(Qbar_i m_{p,i}, Qbar_i M_{p,i})".  Scaled like `score` (x 1/sqrt d), so that a
+#     block whose min equals its max scores exactly what the mean summary gives.
+# ----------------------------------------------------------------------------------------------
+def summarize_quest(k_pages, block_table, seq_lens, bs: int, max_blocks: int | None = None) -> np.ndarray:
+    """mm[b,h,i,0,:] = channel-wise minimum, mm[b,h,i,1,:] = maximum over the valid tokens of block i, as
+    bf16 bit patterns uint16 [B,Hkv,max_blocks,2,d] (min / max of bf16 values are bf16 values: no rounding)."""
+    B = block_table.shape[0]
+    Hkv, d = k_pages.shape[1], k_pages.shape[3]
+    mb = block_table.shape[1] if max_blocks is None else max_blocks
+    out = np.zeros((B, Hkv, mb, 2, d), dtype=np.uint16)
+    for b in range(B):
+        for i in range(n_blocks_of(seq_lens[b], bs)):
+            for h in range(Hkv):
+                n_i = min(bs, int(seq_lens[b]) - i * bs)
+                bits = k_pages[int(block_table[b][i]), h, :n_i, :]          # [n_i, d] uint16
+                val = bf16_to_f64(bits)
+                out[b, h, i, 0] = bits[np.argmin(val, axis=0), np.arange(d)]
+                out[b, h, i, 1] = bits[np.argmax(val, axis=0), np.arange(d)]
+    return out
+
+
+def score_quest(q_bits, mm_bits, n_blocks) -> np.ndarray:
+    """s[b,h,p] = fp32( ( sum_i max(qs_i m_{p,i}, qs_i M_{p,i}) ) * c ), qs = sum_{g in group(h)} q_g = G Qbar,
+    c = 1/(G sqrt d).  float32 [B,Hkv,max_blocks]; entries at p >= n_blocks[b] are 0."""
+    B, Hq, d = q_bits.shape
+    Hkv, mb = mm_bits.shape[1], mm_bits.shape[2]
+    G = Hq // Hkv
+    c = score_scale(G, d)
+    q = bf16_to_f64(q_bits)
+    out = np.zeros((B, Hkv, mb), dtype=np.float32)
+    for b in range(B):
+        nb = int(n_blocks[b])
+        for h in range(Hkv):
+            qs = q[b, h * G:(h + 1) * G].sum(axis=0)                       # [d], exact
+            lo = bf16_to_f64(mm_bits[b, h, :nb, 0])                        # [nb, d]
+            hi = bf16_to_f64(mm_bits[b, h, :nb, 1])
+            s = np.maximum(qs * lo, qs * hi).sum(axis=1)
             out[b, h, :nb] = f64_to_f32(s * c)
     return out
 
@@ -332,7 +381,7 @@ class OracleLayer:
     Order inside a step (Q10): append, then score/top-K/predict/attend with seq_len including
     the new token, then the EMA update."""
 
-    def __init__(self, k_pages, v_pages, block_table, seq_lens, bs, K, budget, Hq, policy=DROP):
+    def __init__(self, k_pages, v_pages, block_table, seq_lens, bs, K, budget, Hq, policy=DROP, summary="mean"):
         self.k = np.array(k_pages, dtype=np.uint16, copy=True)
         self.v = np.array(v_pages, dtype=np.uint16, copy=True)
         self.table = np.asarray(block_table)
@@ -341,7 +390,8 @@ class OracleLayer:
         self.B = self.table.shape[0]
         self.Hkv, self.d = self.k.shape[1], self.k.shape[3]
         self.mb = self.table.shape[1]
-        self.summ = summarize(self.k, self.table, self.lens, bs)
+        self.summary = summary                       # "mean" | "quest" (A.1)
+        self.summ = (summarize if summary == "mean" else summarize_quest)(self.k, self.table, self.lens, bs)
         self.ema = [[EmaState(self.mb) for _ in range(self.Hkv)] for _ in range(self.B)]
         self.theta = [(1.0, 1.0, 0.0)] * self.B
 
@@ -349,7 +399,7 @@ class OracleLayer:
         return np.array([n_blocks_of(n, self.bs) for n in self.lens], dtype=np.int64)
 
     def scores(self, q_bits):
-        return score(q_bits, self.summ, self.n_blocks())
+        return (score if self.summary == "mean" else score_quest)(q_bits, self.summ, self.n_blocks())
 
     def calibrate(self, q_cal_bits, n_valid=None):
         """Synthetic prefill trajectory (DESIGN.md input recipe): T_cal query rows scored against
@@ -358,7 +408,8 @@ class OracleLayer:
         nb = self.n_blocks()
         res = []
         for b in range(self.B):
-            IS = np.stack([score(q_cal_bits[t, b:b + 1], self.summ[b:b + 1], nb[b:b + 1])[0, :, :nb[b]]
+            sfn = score if self.summary == "mean" else score_quest
+            IS = np.stack([sfn(q_cal_bits[t, b:b + 1], self.summ[b:b + 1], nb[b:b + 1])[0, :, :nb[b]]
                            for t in range(T)], axis=1)             # [Hkv, T, N]
             theta, H, states, H_all = calibrate(IS, self.K, self.budget, n_valid)
             self.theta[b] = theta
@@ -381,8 +432,13 @@ class OracleLayer:
             self.lens[b] = pos + 1
             i = pos // self.bs
             for h in range(self.Hkv):
-                kk = block_tokens(self.k, self.table[b], self.lens[b], h, i, self.bs)
-                self.summ[b, h, i] = f64_to_bf16(kk.sum(axis=0) / float(kk.shape[0]))
+                if self.summary == "mean":
+                    kk = block_tokens(self.k, self.table[b], self.lens[b], h, i, self.bs)
+                    self.summ[b, h, i] = f64_to_bf16(kk.sum(axis=0) / float(kk.shape[0]))
+                else:
+                    kk = block_tokens(self.k, self.table[b], self.lens[b], h, i, self.bs)
+                    self.summ[b, h, i, 0] = f64_to_bf16(kk.min(axis=0))          # exact: a min of bf16 values
+                    self.summ[b, h, i, 1] = f64_to_bf16(kk.max(axis=0))
 
     def step(self, q_bits, update=True):
         """q_bits uint16 [B,Hq,d] -> dict(out [B,Hq,d] f64, scores, A, P, M, N per (b,h))."""

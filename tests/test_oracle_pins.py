@@ -498,3 +498,104 @@ def test_synth_is_seeded_and_shaped():
     pg = a.block_table[0]
     assert torch.isfinite(a.k_pages[pg[:64].long()].float()).all()
     assert torch.isnan(a.k_pages[pg[64:].long()].float()).all()
+
+
+# ----------------------------------------------------------------------------------------------
+# Quest min / max summaries with the GQA mean query (A.1)
+# ----------------------------------------------------------------------------------------------
+def _quest_cache(rng, B=2, Hkv=2, d=8, bs=4, lens=(9, 14)):
+    nb = max((n + bs - 1) // bs for n in lens)
+    n_pages = B * nb
+    k = O.f64_to_bf16(rng.standard_normal((n_pages, Hkv, bs, d)))
+    table = rng.permutation(n_pages).reshape(B, nb).astype(np.int32)
+    return k, table, np.array(lens, dtype=np.int64), bs
+
+
+def test_quest_summary_is_channelwise_min_max_by_python_loops():
+    rng = np.random.default_rng(11)
+    k, table, lens, bs = _quest_cache(rng)
+    mm = O.summarize_quest(k, table, lens, bs)
+    kv = O.bf16_to_f64(k)
+    for b in range(2):
+        for i in range((lens[b] + bs - 1) // bs):
+            n_i = min(bs, lens[b] - i * bs)
+            for h in range(2):
+                for c in range(8):
+                    col = [kv[table[b, i], h, t, c] for t in range(n_i)]
+                    assert O.bf16_to_f64(mm[b, h, i, 0, c]) == min(col)
+                    assert O.bf16_to_f64(mm[b, h, i, 1, c]) == max(col)
+
+
+def test_quest_score_by_python_loops_and_mha_form():
+    """The formula of A.1 term by term with exact rationals; G = 1 is Quest's own MHA score."""
+    from fractions import Fraction
+    rng = np.random.default_rng(12)
+    k, table, lens, bs = _quest_cache(rng)
+    mm = O.summarize_quest(k, table, lens, bs)
+    nb = (lens + bs - 1) // bs
+    for G in (1, 3):
+        q = O.f64_to_bf16(rng.standard_normal((2, 2 * G, 8)))
+        got = O.score_quest(q, mm, nb)
+        qv, lo, hi = O.bf16_to_f64(q), O.bf16_to_f64(mm[..., 0, :]), O.bf16_to_f64(mm[..., 1, :])
+        for b in range(2):
+            for h in range(2):
+                for p in range(nb[b]):
+                    tot = Fraction(0)
+                    for i in range(8):
+                        qs = sum(Fraction(float(qv[b, h * G + g, i])) for g in range(G))
+                        tot += max(qs * Fraction(float(lo[b, h, p, i])), qs * Fraction(float(hi[b, h, p, i])))
+                    want = np.float32(float(tot) / (G * np.sqrt(8.0)))
+                    assert abs(float(got[b, h, p]) - float(tot) / (G * np.sqrt(8.0))) <= 1e-7 * max(1.0, abs(float(tot)))
+                    assert got[b, h, p] == want or abs(float(got[b, h, p]) - float(want)) <= np.spacing(want)
+
+
+def test_quest_score_reduces_to_mean_score_when_min_equals_max():
+    """A block of identical keys (or of one token) has m == M == the mean key: both scores, bit for bit."""
+    rng = np.random.default_rng(13)
+    k, table, lens, bs = _quest_cache(rng, lens=(8, 13))           # sequence 1: its last block holds one token
+    for pg in range(k.shape[0]):
+        k[pg, :, :, :] = k[pg, :, :1, :]                           # every block: identical tokens
+    q = O.f64_to_bf16(rng.standard_normal((2, 4, 8)))
+    nb = (lens + bs - 1) // bs
+    s_mean = O.score(q, O.summarize(k, table, lens, bs), nb)
+    s_quest = O.score_quest(q, O.summarize_quest(k, table, lens, bs), nb)
+    assert np.array_equal(s_mean.view(np.uint32), s_quest.view(np.uint32))
+
+
+def test_quest_score_is_an_upper_bound_and_scales():
+    """Quest's guarantee: s_p >= Qbar . k_t / sqrt d for EVERY token t of the block; doubling q doubles s exactly;
+    a wrong sign, a swapped min / max or a dropped channel breaks one of these."""
+    rng = np.random.default_rng(14)
+    k, table, lens, bs = _quest_cache(rng, d=8, lens=(9, 16))
+    mm = O.summarize_quest(k, table, lens, bs)
+    nb = (lens + bs - 1) // bs
+    G = 2
+    q = O.f64_to_bf16(rng.standard_normal((2, 2 * G, 8)))
+    s = O.score_quest(q, mm, nb).astype(np.float64)
+    qv, kvv = O.bf16_to_f64(q), O.bf16_to_f64(k)
+    tight = 0
+    for b in range(2):
+        for h in range(2):
+            qbar = qv[b, h * G:(h + 1) * G].mean(axis=0)
+            for p in range(nb[b]):
+                n_i = min(bs, lens[b] - p * bs)
+                logits = kvv[table[b, p], h, :n_i] @ qbar / np.sqrt(8.0)
+                assert s[b, h, p] >= logits.max() - 1e-6
+                tight += s[b, h, p] <= logits.max() + 1e-6
+    assert tight >= 1                                              # one-token block: the bound is attained
+    q2 = O.f64_to_bf16(2.0 * O.bf16_to_f64(q))
+    assert np.array_equal((2.0 * O.score_quest(q, mm, nb)).view(np.uint32), O.score_quest(q2, mm, nb).view(np.uint32))
+    swapped = mm[:, :, :, ::-1, :]
+    assert np.array_equal(O.score_quest(q, swapped, nb).view(np.uint32), O.score_quest(q, mm, nb).view(np.uint32))  # max() is symmetric
+
+
+def test_oracle_layer_quest_append_keeps_min_max():
+    rng = np.random.default_rng(15)
+    k, table, lens, bs = _quest_cache(rng, lens=(7, 12))
+    table = np.concatenate([table, np.arange(table.size, table.size + 2, dtype=np.int32).reshape(2, 1)], axis=1)
+    k = np.concatenate([k, np.zeros((2,) + k.shape[1:], dtype=np.uint16)], axis=0)
+    lay = O.OracleLayer(k, k.copy(), table, lens, bs, 2, 2, 4, summary="quest")
+    for _ in range(4):
+        kn = O.f64_to_bf16(rng.standard_normal((2, 2, 8)))
+        lay.append(kn, kn)
+    assert np.array_equal(lay.summ, O.summarize_quest(lay.k, lay.table, lay.lens, bs))
