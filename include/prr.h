@@ -58,6 +58,7 @@ enum { PRR_FUSED = 0, PRR_STREAMS = 1 };
  * attention is recomputed over all of A (the fallback PRR avoids).  The output is attention over
  * A in every mode; the modes differ in the work on the critical path. */
 enum { PRR_MODE_S3 = 0, PRR_MODE_S2 = 1, PRR_MODE_S1 = 2 };
+enum { PRR_SUMMARY_MEAN = 0, PRR_SUMMARY_QUEST = 1 };
 
 typedef struct prr_ctx prr_ctx; /* opaque, library-owned */
 
@@ -278,9 +279,16 @@ int32_t prr_timeline_peek(prr_ctx* ctx, uint64_t* stamps_host, int32_t max_warps
  * (sequence, KV head) rows, 1 = the persistent cooperative grid (k_step.cu), 2 = a cluster per row (k_row.cu).
  * PRR_OPT_PACE: percent of the estimated HBM rate at which the persistent kernel issues its first wave of
  * speculative tiles (default 100; 0 = unpaced).  Read-only:
+ * PRR_OPT_SUMMARY: what a block's summary row holds.  PRR_SUMMARY_MEAN (default): the mean key, d bf16.
+ * PRR_SUMMARY_QUEST: Quest's channel-wise minimum and maximum key, 2 d bf16 per row (min then max: the summaries
+ * buffer is [batch, n_kv_heads, max_blocks_per_seq, 2, head_dim]), scored with the GQA mean query as
+ * s_p = sum_i max(Qbar_i m_{p,i}, Qbar_i M_{p,i}) / sqrt d (A.1).  prr_build_summaries, prr_append and
+ * prr_score follow the option; decode steps with Quest summaries run under PRR_STREAMS only (PRR_FUSED contexts
+ * refuse the option with PRR_E_INVALID).  Set it before the summaries are built.
  * PRR_OPT_LAST_CLUSTER / _LAST_RING / _LAST_GRID = cluster size, ring depth and grid of the last fused
  * launch, PRR_OPT_LAST_KERNEL = the kernel it used (1 or 2).  Unknown option or bad value -> PRR_E_INVALID. */
 enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_SUBTILE = 3, PRR_OPT_KERNEL = 4, PRR_OPT_PACE = 5,
+       PRR_OPT_SUMMARY = 6,
        PRR_OPT_LAST_KERNEL = 19, PRR_OPT_LAST_CLUSTER = 16, PRR_OPT_LAST_RING = 17,
        PRR_OPT_LAST_GRID = 18 };
 int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value);

@@ -23,12 +23,35 @@ __global__ void k_build_summaries(const uint16_t* __restrict__ kp, const int32_t
   if (i == nb - 1) open_sum[((size_t)b * Hkv + h) * D + c] = s;
 }
 
+// Quest's page metadata (A.1): channel-wise minimum and maximum key of the block's valid tokens,
+// row layout [2][D] (min then max).  A min / max of bf16 values is one of them: no rounding anywhere.
+__global__ void k_build_minmax(const uint16_t* __restrict__ kp, const int32_t* __restrict__ table,
+                               const int32_t* __restrict__ seq_lens, uint16_t* __restrict__ summ, int Hkv, int bs,
+                               int D, int MB) {
+  const int i = blockIdx.x, h = blockIdx.y, b = blockIdx.z, c = threadIdx.x;
+  const int len = seq_lens[b];
+  const int nb = (len + bs - 1) / bs;
+  if (i >= nb) return;
+  const int n_i = min(bs, len - i * bs);
+  const size_t page = (size_t)table[(size_t)b * MB + i];
+  const uint16_t* src = kp + ((page * Hkv + h) * bs) * (size_t)D + c;
+  uint16_t lo = src[0], hi = lo;
+  for (int t = 1; t < n_i; ++t) {
+    const uint16_t x = src[(size_t)t * D];
+    if (bf16_to_f64(x) < bf16_to_f64(lo)) lo = x;
+    if (bf16_to_f64(x) > bf16_to_f64(hi)) hi = x;
+  }
+  uint16_t* dst = summ + (((size_t)b * Hkv + h) * MB + i) * 2 * D;
+  dst[c] = lo;
+  dst[D + c] = hi;
+}
+
 // One CTA per sequence.  Token position = seq_lens[b] (before the append).
 __global__ void k_append(uint16_t* __restrict__ kp, uint16_t* __restrict__ vp,
                          const int32_t* __restrict__ table, int32_t* __restrict__ seq_lens,
                          const uint16_t* __restrict__ k_new, const uint16_t* __restrict__ v_new,
                          uint16_t* __restrict__ summ, double* __restrict__ open_sum, int Hkv, int bs,
-                         int D, int MB) {
+                         int D, int MB, int quest) {
   const int b = blockIdx.x;
   const int pos = seq_lens[b];
   const int blk = pos / bs, slot = pos - blk * bs;
@@ -40,6 +63,12 @@ __global__ void k_append(uint16_t* __restrict__ kp, uint16_t* __restrict__ vp,
     const size_t dst = ((page * Hkv + h) * bs + slot) * (size_t)D + c;
     kp[dst] = kk;
     vp[dst] = v_new[(size_t)b * Hkv * D + idx];
+    if (quest) {  // the open block's min / max absorb the token; a block's first token starts both
+      uint16_t* mm = summ + (((size_t)b * Hkv + h) * MB + blk) * 2 * D;
+      if (slot == 0 || bf16_to_f64(kk) < bf16_to_f64(mm[c])) mm[c] = kk;
+      if (slot == 0 || bf16_to_f64(kk) > bf16_to_f64(mm[D + c])) mm[D + c] = kk;
+      continue;
+    }
     const size_t so = ((size_t)b * Hkv + h) * D + c;
     const double x = bf16_to_f64(kk);
     const double s = slot == 0 ? x : __dadd_rn(open_sum[so], x);
@@ -59,6 +88,12 @@ __global__ void k_nblocks(const int32_t* __restrict__ seq_lens, int32_t* __restr
 
 void launch_build_summaries(prr_ctx* c, const prr_paged_kv* kv, void* summaries, cudaStream_t s) {
   dim3 grid(c->MB, c->Hkv, kv->batch);
+  if (c->summary_kind == PRR_SUMMARY_QUEST) {
+    k_build_minmax<<<grid, c->D, 0, s>>>((const uint16_t*)kv->k_pages, kv->block_table, kv->seq_lens,
+                                         (uint16_t*)summaries, c->Hkv, c->bs, c->D, c->MB);
+    c->launches++;
+    return;
+  }
   double* os = c->open_sum + (size_t)kv->layer * c->maxB * c->Hkv * c->D;
   k_build_summaries<<<grid, c->D, 0, s>>>((const uint16_t*)kv->k_pages, kv->block_table,
                                           kv->seq_lens, (uint16_t*)summaries, os, c->Hkv, c->bs,
@@ -72,7 +107,7 @@ void launch_append(prr_ctx* c, const prr_paged_kv* kv, const void* k_new, const 
   k_append<<<kv->batch, 256, 0, s>>>((uint16_t*)kv->k_pages, (uint16_t*)kv->v_pages,
                                      kv->block_table, kv->seq_lens, (const uint16_t*)k_new,
                                      (const uint16_t*)v_new, (uint16_t*)summaries, os, c->Hkv,
-                                     c->bs, c->D, c->MB);
+                                     c->bs, c->D, c->MB, c->summary_kind == PRR_SUMMARY_QUEST);
   c->launches++;
 }
 

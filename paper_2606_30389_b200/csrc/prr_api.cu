@@ -863,6 +863,12 @@ extern "C" int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value) {
     case PRR_OPT_SUBTILE: if (value != 16 && value != 32 && value != 64) break; ctx->sub_tile = value; ctx->tmaps.clear(); return PRR_OK;
     case PRR_OPT_KERNEL: if (value < 0 || value > 2) break; ctx->kernel = value; ctx->tmaps.clear(); return PRR_OK;
     case PRR_OPT_PACE: if (value < 0 || value > 1000) break; ctx->pace_pct = value; return PRR_OK;
+    case PRR_OPT_SUMMARY:
+      if (value != PRR_SUMMARY_MEAN && value != PRR_SUMMARY_QUEST) break;
+      if (value == PRR_SUMMARY_QUEST && ctx->fused)
+        PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_option: the fused kernels score mean summaries only; create the context with "
+                 "orchestration PRR_STREAMS to use Quest min/max summaries");
+      ctx->summary_kind = value; return PRR_OK;
     default: break;
   }
   PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_option: unknown option %d or bad value %d", option, value);
@@ -877,6 +883,7 @@ extern "C" int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* v
     case PRR_OPT_SUBTILE: *value_out = ctx->sub_tile; return PRR_OK;
     case PRR_OPT_KERNEL: *value_out = ctx->kernel; return PRR_OK;
     case PRR_OPT_PACE: *value_out = ctx->pace_pct; return PRR_OK;
+    case PRR_OPT_SUMMARY: *value_out = ctx->summary_kind; return PRR_OK;
     case PRR_OPT_LAST_KERNEL: *value_out = ctx->last_kernel; return PRR_OK;
     case PRR_OPT_LAST_CLUSTER: *value_out = ctx->last_cs; return PRR_OK;
     case PRR_OPT_LAST_RING: *value_out = ctx->last_nbuf; return PRR_OK;

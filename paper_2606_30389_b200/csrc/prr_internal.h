@@ -53,6 +53,7 @@ struct prr_ctx {
   int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;
   int mode = 0;                                  // PRR_MODE_S3 (EMA + repair) | _S2 (reuse + repair) | _S1 (reuse + recompute on any miss)
   int kernel = 0;                                // fused step: 0 auto, 1 persistent cooperative grid (k_step.cu), 2 cluster per row (k_row.cu)
+  int summary_kind = 0;  // PRR_SUMMARY_MEAN | PRR_SUMMARY_QUEST (prr_set_option)
   int last_kernel = 0; int pace_pct = 100; float hbm_gbs_est = 6400.f; bool coop_attr[8] = {};          // tuning: cluster size override, programmatic dependent launch, early cut
   int last_cs = 0, last_nbuf = 0, last_grid = 0; // launch shape of the last fused step (introspection)
   std::unordered_map<const void*, std::array<uint64_t, 16>> tmaps; // encoded CUtensorMap per K/V page pool

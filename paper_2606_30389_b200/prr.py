@@ -16,6 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libprr.so")
 OK, E_INVALID, E_UNSUPPORTED, E_STATE, E_CUDA, E_NOMEM = range(6)
 DROP, RETAIN = 0, 1
 OPT_PDL, OPT_CLUSTER, OPT_CUT, OPT_SUBTILE, OPT_KERNEL, OPT_PACE = 0, 1, 2, 3, 4, 5
+OPT_SUMMARY = 6
+SUMMARY_MEAN, SUMMARY_QUEST = 0, 1
 OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID, OPT_LAST_KERNEL = 16, 17, 18, 19
 KERNEL_AUTO, KERNEL_PERSISTENT, KERNEL_CLUSTER = 0, 1, 2
 MODE_S3, MODE_S2, MODE_S1 = 0, 1, 2

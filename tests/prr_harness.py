@@ -42,7 +42,8 @@ class GpuLayer:
         self.k_pages, self.v_pages = inp.k_pages.clone(), inp.v_pages.clone()
         self.seq_lens = inp.seq_lens.clone()
         self.kv = self.ctx.kv(self.k_pages, self.v_pages, inp.block_table, self.seq_lens, layer)
-        self.summ = torch.zeros(cfg.B, cfg.Hkv, self.MB, cfg.d, dtype=torch.bfloat16, device=dev)
+        quest = self.ctx.get_option(prr.OPT_SUMMARY) == prr.SUMMARY_QUEST      # rows hold min then max: 2 d
+        self.summ = torch.zeros((cfg.B, cfg.Hkv, self.MB) + ((2, cfg.d) if quest else (cfg.d,)), dtype=torch.bfloat16, device=dev)
         self.out = torch.zeros(cfg.B, cfg.Hq, cfg.d, dtype=torch.float32, device=dev)
         self.ctx.build_summaries(self.kv, self.summ)
 
@@ -100,10 +101,10 @@ class GpuLayer:
         return sc.cpu().numpy()
 
 
-def oracle_layer(cfg, inp, policy=O.DROP, budget=None) -> O.OracleLayer:
+def oracle_layer(cfg, inp, policy=O.DROP, budget=None, summary="mean") -> O.OracleLayer:
     return O.OracleLayer(synth.bits(inp.k_pages), synth.bits(inp.v_pages), inp.block_table.cpu().numpy(),
                          inp.seq_lens.cpu().numpy(), cfg.bs, cfg.K, cfg.Bud if budget is None else budget,
-                         cfg.Hq, policy)
+                         cfg.Hq, policy, summary)
 
 
 def unpad(row):

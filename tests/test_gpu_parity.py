@@ -27,11 +27,12 @@ KERNELS = [prr.KERNEL_PERSISTENT, prr.KERNEL_CLUSTER]   # the two fused kernels 
 KID = {prr.KERNEL_PERSISTENT: "persistent", prr.KERNEL_CLUSTER: "cluster", None: "auto"}
 
 
-def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None, orchestration=prr.FUSED, kernel=None, options=()):
+def make(cfg, policy=prr.DROP, seed=None, budget=None, steps=None, orchestration=prr.FUSED, kernel=None, options=(),
+         summary="mean"):
     cfg = cfg if seed is None else cfg.scaled(seed=seed)
     inp = synth.make_layer(cfg, 0, device=DEV, steps=steps)
     gl = H.GpuLayer(cfg, inp, policy=policy, budget=budget, orchestration=orchestration, kernel=kernel, options=options)
-    ol = H.oracle_layer(cfg, inp, policy=policy, budget=budget)
+    ol = H.oracle_layer(cfg, inp, policy=policy, budget=budget, summary=summary)
     return cfg, inp, gl, ol
 
 
@@ -243,14 +244,14 @@ def test_repair_stage_matches_attention_over_true_set(cfg, policy):
 
 
 def run_decode(cfg, policy=prr.DROP, steps=None, calibrate=True, budget=None, seed=None, seq_check=True,
-               fused_append=False, orchestration=prr.FUSED, kernel=None, options=(), sequential=False):
+               fused_append=False, orchestration=prr.FUSED, kernel=None, options=(), sequential=False, summary="mean"):
     """Whole decode steps against the oracle: scores and block sets bit-exact, outputs within tolerance, and
     (seq_check) the library's own sequential select-then-attend path within 1e-5 of PRR.  sequential=True
     drives prr_attend itself against the oracle."""
     steps = cfg.steps if steps is None else steps
     cfg, inp, gl, ol = make(cfg, policy=policy, budget=budget, seed=seed, steps=steps, orchestration=orchestration,
-                            kernel=kernel, options=options)
-    twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget, kernel=kernel, options=options) if seq_check else None
+                            kernel=kernel, options=options, summary=summary)
+    twin = H.GpuLayer(cfg, inp, policy=policy, budget=budget, kernel=kernel, options=options, orchestration=orchestration) if seq_check else None
     if calibrate:
         gres = gl.calibrate(inp.q_cal)
         ores = ol.calibrate(synth.bits(inp.q_cal))
@@ -726,3 +727,28 @@ def test_errors_are_reported_not_raised_in_c():
     bad = gl.ctx.kv(gl.k_pages, gl.v_pages, inp.block_table, gl.seq_lens, layer=3)
     with pytest.raises(prr.PrrError):
         gl.ctx.decode_step(bad, inp.q_dec[0].contiguous(), gl.summ, gl.out)
+
+
+def test_quest_minmax_summaries():
+    """§8(f)-2: Quest's channel-wise min / max block metadata scored with the GQA mean query (A.1).
+    Summaries (bulk and after appends) and scores bit-exact against the oracle; whole decode steps (both policies,
+    PRR and select-then-attend) run on them under PRR_STREAMS; a PRR_FUSED context refuses the option."""
+    q_opt = ((prr.OPT_SUMMARY, prr.SUMMARY_QUEST),)
+    for cfg in (TINY, T16, synth.CONFIGS["C1"].scaled(T_cal=8, steps=3)):
+        cfg, inp, gl, ol = make(cfg, orchestration=prr.STREAMS, options=q_opt, summary="quest")
+        torch.cuda.synchronize()
+        assert gl.summ.shape[-2:] == (2, cfg.d)
+        assert np.array_equal(synth.bits(gl.summ), ol.summ), "bulk min / max"
+        for t in range(cfg.steps):
+            gl.append(t)
+            ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        torch.cuda.synchronize()
+        assert np.array_equal(synth.bits(gl.summ), ol.summ), "min / max after appends"
+        assert np.array_equal(gl.seq_lens.cpu().numpy(), ol.lens)
+    run_decode(TINY, orchestration=prr.STREAMS, options=q_opt, summary="quest")
+    run_decode(T128, policy=prr.RETAIN, orchestration=prr.STREAMS, options=q_opt, summary="quest", fused_append=True)
+    run_decode(T16, orchestration=prr.STREAMS, options=q_opt, summary="quest", sequential=True, seq_check=False)
+    run_decode(synth.CONFIGS["C2"].scaled(T_cal=8), steps=3, orchestration=prr.STREAMS, options=q_opt, summary="quest")
+    ctx = prr.Context(8, 2, 64, 16, 4, 4, max_batch=1, max_blocks_per_seq=32)
+    with pytest.raises(prr.PrrError):
+        ctx.set_option(prr.OPT_SUMMARY, prr.SUMMARY_QUEST)
