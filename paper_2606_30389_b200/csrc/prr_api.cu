@@ -7,6 +7,9 @@
 
 #include "prr_internal.h"
 
+static constexpr size_t HOST_OUT_DIRECT = 64 << 10;  // results up to this size are stored into host memory by the kernel
+
+
 using namespace prr;
 
 static thread_local std::string g_create_err;
@@ -166,6 +169,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->st_out, qrows * c->D));
   c->st_q = sq; c->st_k = sq ? sq + qrows * c->D : nullptr; c->st_v = sq ? sq + (qrows + srows) * c->D : nullptr;
   if (e == cudaSuccess) e = cudaHostAlloc(&c->st_pin, st_elems * sizeof(uint16_t), cudaHostAllocDefault);
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->st_out_h, std::min(qrows * c->D * sizeof(float), (size_t)HOST_OUT_DIRECT), cudaHostAllocMapped);
+  if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->st_out_hd, c->st_out_h, 0);
   if (e == cudaSuccess) {
     // P lists start empty (-1); theta defaults to (1, 1, 0): "reuse the last step's top-K" (S1)
     e = cudaMemset(c->P_next, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
@@ -201,6 +206,7 @@ extern "C" int32_t prr_destroy(prr_ctx* c) {
   cudaDeviceSynchronize();
   for (void* p : c->allocs) cudaFree(p);
   if (c->st_pin) cudaFreeHost(c->st_pin);
+  if (c->st_out_h) cudaFreeHost(c->st_out_h);
   if (c->tl) cudaFreeHost(c->tl);
   if (c->cal_state) cudaFree(c->cal_state);
   if (c->cal_mask) cudaFree(c->cal_mask);
@@ -775,10 +781,28 @@ extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, co
     PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_k, pin + qfull, kb * 2, cudaMemcpyHostToDevice, s));
     PRR_CUDA(ctx, cudaMemcpyAsync(ctx->st_v, pin + qfull + kfull, kb * 2, cudaMemcpyHostToDevice, s));
   }
-  const int r = prr_step_append(ctx, kv, ctx->st_q, ctx->st_k, ctx->st_v, summaries, ctx->st_out, 0, stream);
+  // Result: a device->host copy command after the kernel costs ~17 us of queueing for 16 KB (measured, DESIGN.md
+  // section 9), so a small result is stored by the kernel itself straight into host memory: the caller's buffer when it
+  // is pinned and mapped (cudaHostAlloc / torch pin_memory), else a mapped staging buffer copied out after the sync.
+  // A large result (batch serving) keeps the copy engine: its stores would hold the reducer warps on PCIe.
+  float* out_d = ctx->st_out;
+  bool direct = false, staged = false;
+  if (qb * sizeof(float) <= HOST_OUT_DIRECT) {
+    if (out_host != ctx->out_seen) {
+      cudaPointerAttributes pa{};
+      ctx->out_seen = out_host; ctx->out_seen_d = nullptr;
+      if (cudaPointerGetAttributes(&pa, out_host) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer)
+        ctx->out_seen_d = (float*)pa.devicePointer;
+      cudaGetLastError();
+    }
+    if (ctx->out_seen_d) { out_d = ctx->out_seen_d; direct = true; }
+    else { out_d = ctx->st_out_hd; staged = true; }
+  }
+  const int r = prr_step_append(ctx, kv, ctx->st_q, ctx->st_k, ctx->st_v, summaries, out_d, 0, stream);
   if (r) return r;
-  PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));
+  if (!direct && !staged) PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));
   PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  if (staged) memcpy(out_host, ctx->st_out_h, qb * sizeof(float));
   return PRR_OK;
 }
 

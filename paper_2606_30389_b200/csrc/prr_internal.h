@@ -64,6 +64,8 @@ struct prr_ctx {
   double* cal_acc = nullptr;  // [80, Hkv] + counts [80, Hkv] + H [80] + best[1]
   // ---- host staging for prr_decode_step_host ----
   void *st_q = nullptr, *st_k = nullptr, *st_v = nullptr; float* st_out = nullptr;
+  float* st_out_h = nullptr; float* st_out_hd = nullptr;  // small results: the kernel stores them into mapped host memory (no D2H copy)
+  const void* out_seen = nullptr; float* out_seen_d = nullptr;  // last caller buffer and its device alias (null: not mapped)
   void* st_pin = nullptr;  // pinned host image of [q | k_new | v_new] for one copy across PCIe
 
   cudaStream_t side_spec = nullptr, side_ema = nullptr;
