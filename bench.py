@@ -327,10 +327,12 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=512)
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-seq", action="store_true", help="skip the sequential select-then-attend leg")
-    ap.add_argument("--budget", default="profiled", choices=["profiled", "config"],
-                    help="speculation budget: chosen by prr_profile_budget among candidates <= the config's (PAPER.md "
-                         "section 4.4), or the config's fixed one")
+    ap.add_argument("--budget", default="profiled",
+                    help="speculation budget: 'profiled' = chosen by prr_profile_budget among candidates <= the config's "
+                         "(PAPER.md section 4.4), 'config' = the config's fixed one, or a number of blocks (what an earlier "
+                         "profiled run chose: the ncu captures use it to skip the sweep)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "persistent", "cluster"])
+    ap.add_argument("--cluster", type=int, default=0, help="force the cluster size of k_row (0 = the library's choice)")
     ap.add_argument("--sweep", action="store_true", help="Table-3-shaped sweep: block size x token budget at 128K, 32q/8kv")
     args = ap.parse_args()
 
@@ -353,22 +355,30 @@ def main():
         run_reference(args, cfg, rank, world)
         return
     args.warmup = max(args.warmup, 3)
+    # every one of the R layer caches is visited at least twice before the clock starts (a layer's first visits
+    # pay for its TLB entries and tensor maps): the warm-up that is RUN is max(W, 2R) steps, reported as warmup_run
+    warm_run = max(args.warmup, 2 * args.layers)
 
     dist = dist_init(world, local)
     torch.cuda.set_device(local)
     dev = torch.device(f"cuda:{local}")
     R = args.layers
-    K, W = args.steps, args.warmup
+    K, W = args.steps, warm_run
     E = args.e2e_steps
     seq_steps = 0 if args.no_seq else min(K, 4096)
     total = 4 * W + K + seq_steps + E + min(K, 2048)
     tokens = (total + R - 1) // R + 2
     kern = {"auto": 0, "persistent": 1, "cluster": 2}[args.kernel]
     st = Stack(cfg, R, tokens, dev, seed_off=rank_seed_offset(rank), kernel=kern)
+    if args.cluster:
+        st.ctx.set_option(st.prr.OPT_CLUSTER, args.cluster)
     cal_s = st.calibrate()
     stream = torch.cuda.Stream(device=dev)
     # ---- speculation budget: the library's profiling-guided choice (PAPER.md 204-208), capped by the config's
     budget_info = {"mode": args.budget, "config_budget": cfg.Bud, "budget": cfg.Bud}
+    if args.budget not in ("profiled", "config"):
+        budget_info.update(mode="given", budget=max(0, min(cfg.Bud, int(args.budget))))
+        st.ctx.set_budget(-1, budget_info["budget"])
     if args.budget == "profiled" and cfg.Bud > 0:
         cands = sorted({0, cfg.K // 4, cfg.K // 2, (3 * cfg.K) // 4, cfg.K, (cfg.K + cfg.Bud) // 2, cfg.Bud})
         us_b, seq_b, best = st.profile_budget(cands)
@@ -474,8 +484,8 @@ def main():
     abytes = algorithmic_bytes(cfg, mean_len)
     cpu_us, cores, n_cpu = oracle_run(cfg, 64, 2, budget_s=args.cpu_seconds)
     line = {
-        "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": us_step, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "warmup_run": W, "ms_per_step": us_step / 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16 KV / fp32 softmax+accumulate (mma.sync bf16), fp64 exact scoring + EMA", "data": "synthetic",
         "config": {"workload": workload_name(cfg, R), "l2": "inputs larger than L2 (round-robin over "
                    f"{R} layer caches, ~{R * abytes * 1.4 / 1e6:.0f} MB touched between reuses)",

@@ -284,11 +284,8 @@ template <int D, int BS>
 static void launch_partial_t(prr_ctx* c, const prr_paged_kv* kv, const void* q, const int32_t* list,
                              int width, float* O, float* m, float* l, cudaStream_t s) {
   const size_t smem = (size_t)2 * BS * (D + 8) * 2;
-  static bool attr_set = false;
-  if (!attr_set && smem > 48 * 1024) {
+  if (smem > 48 * 1024)  // (per device and cheap: not cached in a process-wide flag)
     cudaFuncSetAttribute((const void*)k_partial<D, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
   dim3 grid(width, c->Hkv, kv->batch);
   k_partial<D, BS><<<grid, 2 * BS, smem, s>>>(
       (const uint16_t*)kv->k_pages, (const uint16_t*)kv->v_pages, kv->block_table, kv->seq_lens,

@@ -1606,8 +1606,12 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
     c->row_dyn[key] = c->smem_optin - (int)fa.sharedSizeBytes;
     e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->row_dyn[key]);
     if (e != cudaSuccess) return e;
-    // clusters of 1, 2, 4, 8 CTAs that can be co-resident with the whole shared memory of an SM each
-    for (int i = 0; i < 4; ++i) {
+    // clusters of 1, 2, 4, 8, 16 CTAs that can be co-resident with the whole shared memory of an SM each
+    // (16 is past the portable size: the function opts in)
+    const bool np16 = cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+    if (!np16) cudaGetLastError();
+    for (int i = 0; i < 5; ++i) {
+      if (i == 4 && !np16) { c->row_maxcl[key][i] = 0; continue; }
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((1 << i) * 8); cfg.blockDim = dim3(NTHR);
       cfg.dynamicSmemBytes = c->row_dyn[key];
@@ -1623,7 +1627,7 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
   }
   // the largest cluster that still gives every row its own cluster in one wave
   int CS = 1;
-  for (int i = 3; i >= 0; --i)
+  for (int i = 4; i >= 0; --i)
     if (c->row_maxcl[key][i] >= R) { CS = 1 << i; break; }
   if (c->force_cs > 0) CS = c->force_cs;
   int li = 0; while ((1 << li) < CS) ++li;

@@ -659,6 +659,8 @@ static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const v
   // Which fused kernel: the persistent cooperative grid when the rows are few (its warps are spread over
   // every SM whatever the batch), a cluster per row once the rows fill the GPU (measured: DESIGN.md section 8).
   const int rows = kv->batch * c->Hkv;
+  // a run-time budget of 0 (prr_set_budget re-predicted: P is empty) IS the sequential path: take it outright
+  if (spec && c->bud_eff[kv->layer] == 0) spec = 0;
   int kern = c->kernel;
   if (kern == 0) kern = rows >= 64 ? 2 : 1;
   if (c->bs > 128 || c->mode == PRR_MODE_S1) kern = 2;  // (only the cluster kernel cuts a block into sub-tiles / recomputes on a miss)
@@ -882,7 +884,7 @@ extern "C" int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value) {
   if (!ctx) return PRR_E_INVALID;
   switch (option) {
     case PRR_OPT_PDL: if (value != 0 && value != 1) break; ctx->pdl = value; return PRR_OK;
-    case PRR_OPT_CLUSTER: if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) break; ctx->force_cs = value; return PRR_OK;
+    case PRR_OPT_CLUSTER: if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16) break; ctx->force_cs = value; return PRR_OK;
     case PRR_OPT_CUT: if (value != 0 && value != 1) break; ctx->cut = value; return PRR_OK;
     case PRR_OPT_SUBTILE: if (value != 16 && value != 32 && value != 64) break; ctx->sub_tile = value; ctx->tmaps.clear(); return PRR_OK;
     case PRR_OPT_KERNEL: if (value < 0 || value > 2) break; ctx->kernel = value; ctx->tmaps.clear(); return PRR_OK;
@@ -959,6 +961,7 @@ extern "C" int32_t prr_graph_end(prr_ctx* ctx, void* stream, prr_graph** out) {
   prr_graph* g = new prr_graph();
   cudaError_t e = cudaStreamEndCapture(s, &g->graph);
   if (e == cudaSuccess) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+  if (e == cudaSuccess) e = cudaGraphUpload(g->exec, s);  // the first launch does not pay for the upload
   if (e != cudaSuccess) {
     if (g->graph) cudaGraphDestroy(g->graph);
     delete g;

@@ -49,7 +49,7 @@ struct prr_ctx {
   unsigned long long* tl = nullptr; int tl_on = 0, tl_warps = 0; // fused step: per-warp phase stamps (debug)
   int n_sm = 0, smem_optin = 0, fused = 1, coop = 0;
   // fused step (k_row.cu): per kernel instantiation, attribute set + co-resident clusters of 1, 2, 4, 8 CTAs
-  int row_attr[6] = {0, 0, 0, 0, 0, 0}; int row_maxcl[6][4] = {}; int row_dyn[6] = {};
+  int row_attr[6] = {0, 0, 0, 0, 0, 0}; int row_maxcl[6][5] = {}; int row_dyn[6] = {};
   int force_cs = 0, pdl = 1, cut = 1, sub_tile = 64;
   int mode = 0;                                  // PRR_MODE_S3 (EMA + repair) | _S2 (reuse + repair) | _S1 (reuse + recompute on any miss)
   int kernel = 0;                                // fused step: 0 auto, 1 persistent cooperative grid (k_step.cu), 2 cluster per row (k_row.cu)
