@@ -294,6 +294,26 @@ enum { PRR_OPT_PDL = 0, PRR_OPT_CLUSTER = 1, PRR_OPT_CUT = 2, PRR_OPT_SUBTILE = 
 int32_t prr_set_option(prr_ctx* ctx, int32_t option, int32_t value);
 int32_t prr_get_option(const prr_ctx* ctx, int32_t option, int32_t* value_out /* host */);
 
+/* --- no-allocation entry point ---------------------------------------------------------------- */
+
+/* Sparse attention over given block lists (a4 + a7: per-block partial states, then the Eq. 6-8 fold)
+ * for callers that may not allocate: code under stream capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  blocks: dev int32 [batch, n_kv_heads, width], -1 = hole (skipped); the listed blocks are folded in
+ * list order; out dev fp32 [batch, n_q_heads, head_dim]; m_out / l_out (dev fp32 [batch, n_q_heads], natural-log
+ * maximum and denominator of the final state) may be NULL.  Same kernels and results as prr_repair with an empty
+ * prediction, but the partial states between the two launches live in ONE static device array of
+ * PRR_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit) instead of
+ * ctx-owned buffers.  The call itself makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ * Limit: batch * n_q_heads * width * (head_dim + 2) * 4 bytes <= PRR_STATIC_SCRATCH_BYTES, 1 <= width <= 1024,
+ * block_size <= 128; beyond it -> PRR_E_UNSUPPORTED with the sizes in prr_last_error, nothing launched.
+ * Every call on a device shares the array, which keeps the last call's contents (nothing in it needs to start at
+ * zero: each call writes every slot it reads).  Calls that OVERLAP on the GPU (two streams, two host threads, two
+ * contexts on one device) race on it: order them on one stream or with events. */
+#define PRR_STATIC_SCRATCH_BYTES (8 * 1024 * 1024)
+int64_t prr_static_scratch_bytes(void);
+int32_t prr_attend_blocks_static(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const int32_t* blocks,
+                                 int32_t width, float* out, float* m_out, float* l_out, void* stream);
+
 /* --- CUDA-graph helpers (so callers need no CUDA runtime of their own) ------------------------ */
 typedef struct prr_graph prr_graph;
 int32_t prr_graph_begin(prr_ctx* ctx, void* stream);               /* start capturing `stream` */

@@ -32,6 +32,7 @@ SYMBOLS = [
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
     "prr_timeline_enable", "prr_timeline_read", "prr_timeline_peek", "prr_set_option", "prr_get_option",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
+    "prr_static_scratch_bytes", "prr_attend_blocks_static",
 ]
 
 
@@ -68,6 +69,7 @@ def lib() -> C.CDLL:
         L.prr_last_error.argtypes = [C.c_void_p]
         L.prr_version.restype = C.c_char_p
         L.prr_launch_count.restype = C.c_int64
+        L.prr_static_scratch_bytes.restype = C.c_int64
         L.prr_launch_count.argtypes = [C.c_void_p]
         L.prr_set_ema_params.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                          C.c_double, C.c_void_p]
@@ -201,6 +203,12 @@ class Context:
                                    C.c_void_p(_p(P)), C.c_void_p(_p(O_part)), C.c_void_p(_p(m_part)),
                                    C.c_void_p(_p(l_part)), C.c_void_p(_p(out)), C.c_void_p(_p(m_out)),
                                    C.c_void_p(_p(l_out)), C.c_void_p(_stream(stream))))
+
+    def attend_blocks_static(self, kv, q, blocks, width, out, m_out=None, l_out=None, stream=None):
+        """prr_attend_blocks_static: attention over given block lists; partial states in the library's static scratch."""
+        self._chk(lib().prr_attend_blocks_static(self._h, C.byref(kv), C.c_void_p(_p(q)), C.c_void_p(_p(blocks)),
+                                                 C.c_int32(int(width)), C.c_void_p(_p(out)), C.c_void_p(_p(m_out)),
+                                                 C.c_void_p(_p(l_out)), C.c_void_p(_stream(stream))))
 
     def attend(self, kv, q, summaries, out, stream=None):
         self._chk(lib().prr_attend(self._h, C.byref(kv), C.c_void_p(_p(q)), C.c_void_p(_p(summaries)),
