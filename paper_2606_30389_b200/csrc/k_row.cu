@@ -1583,7 +1583,8 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
       a.ctl[CTL_EXIT] = 0u;
       *a.parity = par_raw ^ 1;
       if (a.app)
-        for (int b = 0; b < a.B; ++b) a.seq_lens_w[b] += 1;
+        for (int b = 0; b < a.B; ++b)
+          if (a.seq_lens_w[b] / a.bs < a.MB) a.seq_lens_w[b] += 1;  // (a full sequence: nothing was written, the length stays, as in k_append)
     }
   }
 }

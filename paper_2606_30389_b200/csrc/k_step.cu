@@ -1173,9 +1173,10 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
 // a7 for one (sequence, query head, 16-channel slice of d): Eq. 6-8 over the listed partial states,
 // O unnormalised and one division at the end.  The warp is 8 groups of 4 lanes; a group owns every
 // 8th entry and its lanes one float4 of the 64-byte slice, so a pass has 80 entries in flight (the
-// whole speculative segment of a row in one round trip); the groups are folded with three shuffles.  Entry order is fixed (speculative slots
-// ascending, then repair slots ascending) and so is the reduction tree: the result is
-// deterministic; any order is the same real number (Q11).
+// whole speculative segment of a row in one round trip); the groups are folded with three shuffles.  Entries are folded speculative slots
+// ascending, then repair slots ascending; a missed block takes whichever repair slot its shared-memory
+// ticket gave it (warp-scheduling order), so the fp32 rounding of the repair segment can differ from run
+// to run by a few ulp (tests bound it by 2e-6); any order is the same real number (Q11).
 template <int D, int MSW>
 __device__ void job_merge(const StepArgs& a, int b, int hq, int dq, unsigned char* buf, uint32_t ep,
                           unsigned long long* tl) {
@@ -1611,7 +1612,8 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   last = __shfl_sync(FULL, last, 0);
   if (last) {
     if (a.app)
-      for (int b = lane; b < a.B; b += 32) a.seq_lens_w[b] += 1;
+      for (int b = lane; b < a.B; b += 32)
+        if (a.seq_lens_w[b] / a.bs < a.MB) a.seq_lens_w[b] += 1;  // (a full sequence: nothing was written, the length stays, as in k_append)
     if (lane == 0) {
       ctl[CTL_EXIT] = 0u;
       ctl[CTL_EPOCH] = ep;
