@@ -290,7 +290,7 @@ def sweep(args):
             cfg = synth.Config(f"S{bs}_{tokens}", B=1, L=1, Hq=32, Hkv=8, d=128, ctx_lo=131072, ctx_hi=131072, bs=bs, K=K,
                                Bud=min(1024, K + K // 2), rho=0.95, steps=8, T_cal=8)
             R, n = 8, 256
-            st = Stack(cfg, R, n // R + 8, dev, kernel={"auto": 0, "persistent": 1, "cluster": 2}[args.kernel])
+            st = Stack(cfg, R, 2 * (n + 16) // R + 4, dev, kernel={"auto": 0, "persistent": 1, "cluster": 2}[args.kernel])
             for l in range(R):
                 st.ctx.set_ema_params(l, -1, 0.6, 0.2, 0.5)
             res = {}

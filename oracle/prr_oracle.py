@@ -30,6 +30,10 @@ What each part is, and what pins it (tests/test_oracle_pins.py; readings Q1..Q15
                  key shift invariance; block permutation invariance
   block_state /  per-block (m, l, O) and the Eq. 6-8 fold
   fold           pins: any partition, any order == attend; identity element; M = {} is the identity
+  e4m3 codecs /  OCP e4m3 codes, power-of-two per-block scales, quantise / dequantise a paged cache (PAPER.md:319
+  quantize_kv    names fp8 as future work; format = DESIGN.md section 10).  pins: all 256 codes and random
+                 values against torch.float8_e4m3fn; midpoints tie to even; saturation; round trip; amax of a
+                 block lands on a code >= 240/448 of full scale; relative error <= 2^-4; dequantised cache exact in bf16
   prr_step       speculate over P, repair A\\P
                  pins: DROP == attend(A); RETAIN == attend(A u P); Bud = NB -> M = {}
   The paper's published ratios / hit rates (Tables 1-8): PARITY UNPINNED — they depend on models
@@ -291,6 +295,76 @@ def calibrate(IS: np.ndarray, K: int, budget: int, n_valid=None):
         finals.append(states)
     best = int(np.argmax(H_all))                                  # first maximiser (Eq. 5)
     return grid[best], float(H_all[best]), finals[best], H_all
+
+
+# ----------------------------------------------------------------------------------------------
+# 5b. fp8 (e4m3) KV blocks with per-block scales — PAPER.md:319 names fp8 as future work and fixes no format;
+#     DESIGN.md section 10 takes: OCP e4m3 ("fn": no infinities, max 448, NaN = S.1111.111), ONE power-of-two
+#     scale per (page, KV head) for K and one for V, the smallest 2^e with amax <= 448 * 2^e, codes =
+#     RNE(x / 2^e) saturated to +-448.  A power-of-two scale makes x / 2^e and code * 2^e exact, so the only
+#     rounding is the e4m3 one and the dequantised cache is again a bf16 cache: every other function of
+#     this file applies to it unchanged.
+# ----------------------------------------------------------------------------------------------
+def e4m3_to_f64(codes: np.ndarray) -> np.ndarray:
+    """uint8 e4m3 codes -> float64, exactly: (-1)^s 2^(E-7) (1 + M/8), E = 0: 2^-6 (M/8); S.1111.111 = NaN."""
+    c = np.asarray(codes, dtype=np.uint8).astype(np.int64)
+    sgn = np.where(c & 0x80, -1.0, 1.0)
+    E = (c >> 3) & 0xF
+    M = (c & 0x7).astype(np.float64)
+    val = np.where(E == 0, np.ldexp(M / 8.0, -6), np.ldexp(1.0 + M / 8.0, (E - 7).astype(np.int64)))
+    val = np.where((E == 15) & ((c & 0x7) == 7), np.nan, val)
+    return sgn * val
+
+
+def f64_to_e4m3(x: np.ndarray) -> np.ndarray:
+    """float64 -> e4m3 codes: round to nearest, ties to the even code, |x| beyond 448 saturates to +-448
+    (0x7e / 0xfe), NaN -> 0x7f.  The 127 non-negative finite codes are ascending in value, so the nearest
+    code is found by searching the table of their values; a tie takes the even code."""
+    x = np.asarray(x, dtype=np.float64)
+    table = e4m3_to_f64(np.arange(127, dtype=np.uint8))            # 0 .. 448, strictly ascending
+    ax = np.minimum(np.abs(np.nan_to_num(x, nan=0.0)), 448.0)
+    hi = np.clip(np.searchsorted(table, ax, side="left"), 0, 126)  # first code with value >= ax
+    lo = np.maximum(hi - 1, 0)
+    d_hi, d_lo = table[hi] - ax, ax - table[lo]
+    take_lo = (d_lo < d_hi) | ((d_lo == d_hi) & (lo % 2 == 0))
+    code = np.where(take_lo, lo, hi).astype(np.uint8)
+    code = np.where(np.signbit(x), code | np.uint8(0x80), code).astype(np.uint8)
+    return np.where(np.isnan(x), np.uint8(0x7F), code).astype(np.uint8)
+
+
+def pow2_scale_exp(amax: float) -> int:
+    """Smallest integer e with amax <= 448 * 2^e (0 for an all-zero block)."""
+    if not amax > 0.0:
+        return 0
+    m, x = math.frexp(float(amax))        # amax = m 2^x, 0.5 <= m < 1;  448 = 0.875 * 2^9
+    return x - 9 if m <= 0.875 else x - 8
+
+
+def quantize_kv_e4m3(pages_bits, block_table, seq_lens, bs: int):
+    """bf16 pages [n_pages, Hkv, bs, d] -> (codes uint8 of the same shape, scale float32 [n_pages, Hkv]).
+    Per (mapped page, KV head): amax over the VALID tokens of the block, scale = 2^e, codes = RNE(x / 2^e).
+    Token slots past the sequence length get code 0; pages no sequence maps keep code 0 and scale 1."""
+    n_pages, Hkv, _, d = pages_bits.shape
+    codes = np.zeros(pages_bits.shape, dtype=np.uint8)
+    scale = np.ones((n_pages, Hkv), dtype=np.float32)
+    for b in range(block_table.shape[0]):
+        for i in range(n_blocks_of(seq_lens[b], bs)):
+            pg = int(block_table[b, i])
+            for h in range(Hkv):
+                x = block_tokens(pages_bits, block_table[b], seq_lens[b], h, i, bs)
+                e = pow2_scale_exp(float(np.abs(x).max()))
+                scale[pg, h] = np.float32(math.ldexp(1.0, e))
+                codes[pg, h, :x.shape[0], :] = f64_to_e4m3(np.ldexp(x, -e))
+    return codes, scale
+
+
+def dequantize_kv_e4m3(codes, scale) -> np.ndarray:
+    """codes uint8 [n_pages, Hkv, bs, d], scale float32 [n_pages, Hkv] (powers of two) -> the dequantised
+    cache as bf16 bit patterns (exact: 4 significant bits times a power of two)."""
+    val = e4m3_to_f64(codes) * scale.astype(np.float64)[:, :, None, None]
+    bits = f64_to_bf16(val)
+    assert np.array_equal(bf16_to_f64(bits), val), "dequantised fp8 values must be exact in bf16"
+    return bits
 
 
 # ----------------------------------------------------------------------------------------------

@@ -599,3 +599,72 @@ def test_oracle_layer_quest_append_keeps_min_max():
         kn = O.f64_to_bf16(rng.standard_normal((2, 2, 8)))
         lay.append(kn, kn)
     assert np.array_equal(lay.summ, O.summarize_quest(lay.k, lay.table, lay.lens, bs))
+
+
+# ---- fp8 (e4m3) KV with per-block power-of-two scales (format: DESIGN.md section 10) ----------
+def test_e4m3_decode_all_codes_against_torch_and_closed_forms():
+    c = np.arange(256, dtype=np.uint8)
+    v = O.e4m3_to_f64(c)
+    t = torch.from_numpy(c.copy()).view(torch.float8_e4m3fn).to(torch.float32).numpy().astype(np.float64)
+    assert np.array_equal(np.isnan(v), np.isnan(t)) and np.isnan(v).sum() == 2          # 0x7f, 0xff only
+    assert np.array_equal(v[~np.isnan(v)], t[~np.isnan(t)])
+    assert v[0x7E] == 448.0 and v[0xFE] == -448.0 and v[0x01] == 2.0 ** -9 and v[0x08] == 2.0 ** -6
+    assert v[0x38] == 1.0 and v[0x3C] == 1.5 and v[0x00] == 0.0 and np.signbit(v[0x80])
+    assert np.all(np.diff(v[:127]) > 0)                                                 # what f64_to_e4m3 relies on
+
+
+def test_e4m3_encode_rne_ties_saturation_round_trip():
+    c = np.arange(256, dtype=np.uint8)
+    ok = ~np.isnan(O.e4m3_to_f64(c))
+    assert np.array_equal(O.f64_to_e4m3(O.e4m3_to_f64(c[ok])), c[ok])                   # every finite code, both zeros
+    rng = np.random.default_rng(21)
+    x = np.concatenate([rng.standard_normal(20000) * s for s in (0.01, 1.0, 60.0)]).astype(np.float32)
+    x = x[np.abs(x) <= 448.0]
+    ref = torch.from_numpy(x.copy()).to(torch.float8_e4m3fn).view(torch.uint8).numpy()  # torch rounds to nearest even
+    assert np.array_equal(O.f64_to_e4m3(x.astype(np.float64)), ref)
+    vals = O.e4m3_to_f64(np.arange(127, dtype=np.uint8))
+    mid = (vals[:-1] + vals[1:]) / 2.0                                                  # exact in fp64
+    got = O.f64_to_e4m3(mid)
+    assert np.all(got % 2 == 0) and np.all((got == np.arange(126)) | (got == np.arange(1, 127)))
+    assert np.array_equal(O.f64_to_e4m3(-mid), got | 0x80)
+    assert list(O.f64_to_e4m3(np.array([449.0, 1e30, -1e30, np.inf, np.nan, 464.0]))) == [0x7E, 0x7E, 0xFE, 0x7E, 0x7F, 0x7E]
+    brute = np.array([np.argmin(np.abs(vals - a)) for a in np.abs(x[:2000]).astype(np.float64)])
+    err = np.abs(vals[O.f64_to_e4m3(np.abs(x[:2000]).astype(np.float64))] - np.abs(x[:2000]))
+    assert np.all(err <= np.abs(vals[brute] - np.abs(x[:2000])))                        # nearest (brute force over all codes)
+
+
+def test_pow2_scale_is_the_smallest_that_fits():
+    for amax in [448.0, 448.0001, 447.9, 1.0, 0.875, 0.8751, 3.0e-5, 7.0e4, 2.0 ** -20]:
+        e = O.pow2_scale_exp(amax)
+        assert amax <= 448.0 * 2.0 ** e and amax > 448.0 * 2.0 ** (e - 1)
+    assert O.pow2_scale_exp(0.0) == 0
+
+
+def test_quantize_kv_e4m3_error_bound_and_exact_dequant():
+    rng = np.random.default_rng(22)
+    bs, Hkv, d = 16, 2, 8
+    lens = np.array([37, 64])
+    table = rng.permutation(8).astype(np.int32).reshape(2, 4)
+    k = O.f64_to_bf16(rng.standard_normal((9, Hkv, bs, d)) * rng.uniform(0.01, 30.0, size=(9, Hkv, 1, 1)))
+    k[table[0, 2], :, 5:, :] = 0x7FC0                                                   # NaN in slots past the length
+    codes, scale = O.quantize_kv_e4m3(k, table, lens, bs)
+    assert codes.dtype == np.uint8 and scale.dtype == np.float32
+    assert np.all(codes[8] == 0) and np.all(scale[8] == 1.0)                            # the unmapped page
+    assert np.all(codes[table[0, 2], :, 5:, :] == 0)                                    # slots past the length
+    assert np.all(codes[table[0, 3]] == 0)                                              # block past the length
+    deq = O.bf16_to_f64(O.dequantize_kv_e4m3(codes, scale))
+    for b in range(2):
+        for i in range(O.n_blocks_of(lens[b], bs)):
+            for h in range(Hkv):
+                x = O.block_tokens(k, table[b], lens[b], h, i, bs)
+                y = deq[table[b, i], h, :x.shape[0]]
+                s = float(scale[table[b, i], h])
+                assert math.frexp(s)[0] == 0.5                                          # a power of two
+                top = np.abs(O.e4m3_to_f64(codes[table[b, i], h, :x.shape[0]])).max()
+                assert 224.0 <= top <= 448.0                                            # amax > 224 s rounds to a code >= 224
+                assert np.all(np.abs(y - x) <= np.maximum(np.abs(x) * 2.0 ** -4, s * 2.0 ** -10))
+    # values that ARE e4m3 codes times the block's scale survive unchanged
+    k2 = O.dequantize_kv_e4m3(codes, scale)
+    c2, s2 = O.quantize_kv_e4m3(k2, table, np.array([64, 64]), bs)
+    live = [table[b, i] for b in range(2) for i in range(O.n_blocks_of(lens[b], bs))]
+    assert np.array_equal(O.dequantize_kv_e4m3(c2, s2)[live], k2[live])
