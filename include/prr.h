@@ -42,7 +42,10 @@ extern "C" {
 
 enum { PRR_OK = 0, PRR_E_INVALID = 1, PRR_E_UNSUPPORTED = 2, PRR_E_STATE = 3, PRR_E_CUDA = 4,
        PRR_E_NOMEM = 5 };
-enum { PRR_BF16 = 0 };
+/* KV page element type.  PRR_FP8_E4M3 (PAPER.md:319 names fp8 as future work; format: DESIGN.md section 10):
+ * pages hold OCP e4m3 codes, one byte per element, same [n_pages, n_kv_heads, block_size, head_dim] layout, with
+ * ONE power-of-two scale per (page, KV head) for K and one for V (prr_set_kv_scales); element = code * scale. */
+enum { PRR_BF16 = 0, PRR_FP8_E4M3 = 1 };
 /* What happens to over-predicted blocks P\A at merge (Q7).  PRR_DROP: the output is attention
  * over exactly A (BASELINE.json north_star).  PRR_RETAIN: P\A is "retained as additional
  * low-priority context", the output is attention over A u P. */
@@ -68,7 +71,7 @@ typedef struct {
   int32_t max_batch;             /* >= 1 */
   int32_t max_blocks_per_seq;    /* row stride of block_table / summaries / scores; <= 32768 */
   int32_t n_layers;              /* EMA state is kept per (layer, sequence, KV head, block) */
-  int32_t kv_dtype;              /* PRR_BF16 */
+  int32_t kv_dtype;              /* PRR_BF16 | PRR_FP8_E4M3 (needs PRR_STREAMS, block_size <= 128) */
   int32_t overpredict_policy;    /* PRR_DROP | PRR_RETAIN */
   float sm_scale;                /* softmax scale of the attention logits; 0 -> 1/sqrt(head_dim) */
   int32_t orchestration;         /* PRR_FUSED | PRR_STREAMS */
@@ -108,6 +111,25 @@ int32_t prr_build_summaries(prr_ctx* ctx, const prr_paged_kv* kv, void* summarie
  * pointers of `kv`. */
 int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* k_new, const void* v_new,
                    void* summaries, void* stream);
+
+/* --- fp8 KV (PRR_FP8_E4M3) --------------------------------------------------------------------- */
+
+/* Quantise a bf16 paged cache (kv: the bf16 pages, block table and lengths; any ctx of the same shape): per
+ * (mapped page, KV head) amax over the block's VALID tokens, scale = the smallest 2^e with amax <= 448 * 2^e,
+ * codes = round-to-nearest-even(x / 2^e) saturated to +-448; token slots past the length get code 0.
+ * k8_pages / v8_pages: dev uint8, the layout of the bf16 pages; k_scale / v_scale: dev fp32 [n_pages,
+ * n_kv_heads] (entries of unmapped pages are left untouched).  x / 2^e and code * 2^e are exact. */
+int32_t prr_quantize_kv_fp8(prr_ctx* ctx, const prr_paged_kv* kv, void* k8_pages, void* v8_pages,
+                            float* k_scale, float* v_scale, void* stream);
+/* Scales of a layer's fp8 pages (dev fp32 [n_pages, n_kv_heads], powers of two, caller-owned, read by every
+ * later call on that layer).  With a PRR_FP8_E4M3 ctx, prr_paged_kv.k_pages / v_pages point at the code pages;
+ * prr_build_summaries (mean of the dequantised keys), prr_score, prr_topk, prr_calibrate, prr_speculate,
+ * prr_repair, prr_attend and prr_decode_step (PRR_STREAMS) work as for bf16 and move half the KV bytes; the
+ * tiles are widened to bf16 on chip (exact), so every result equals the bf16 path's on the dequantised cache
+ * bit for bit.  prr_append / prr_step_append / prr_decode_step_host return PRR_E_UNSUPPORTED (a new token cannot
+ * join a block quantised with a fixed scale: re-quantise the open block with prr_quantize_kv_fp8); a call
+ * before the scales are set returns PRR_E_STATE. */
+int32_t prr_set_kv_scales(prr_ctx* ctx, int32_t layer, const float* k_scale, const float* v_scale);
 
 /* --- predictor ------------------------------------------------------------ */
 

@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libprr.so")
 OBJ = os.path.join(ROOT, "build", "prr")
-SOURCES = ["prr_api.cu", "k_cache.cu", "k_score.cu", "k_select.cu", "k_attn.cu", "k_calib.cu", "k_step.cu", "k_row.cu", "k_noalloc.cu"]
+SOURCES = ["prr_api.cu", "k_cache.cu", "k_score.cu", "k_select.cu", "k_attn.cu", "k_calib.cu", "k_step.cu", "k_row.cu", "k_noalloc.cu", "k_fp8.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 

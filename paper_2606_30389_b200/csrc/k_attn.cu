@@ -12,6 +12,7 @@
 // k_merge: one CTA per (query head, sequence): folds the listed partial states, in ascending
 // block order, with the log-sum-exp rescaling of Eq. 6-8 (written with O unnormalised and a
 // single division at the end), so P\A drops out (or is retained) by simply not being listed.
+#include <cuda_fp8.h>
 #include <math_constants.h>
 
 #include "prr_dev.cuh"
@@ -21,13 +22,41 @@ namespace prr {
 
 constexpr float LOG2E = 1.4426950408889634f;
 
-template <int D, int BS>
+// FP8: kp / vp hold e4m3 codes (one byte per element, same page layout)
+// and kscale / vscale [n_pages, Hkv] their power-of-two scales.  The codes are staged raw (half the bytes
+// from HBM), widened to bf16 in shared memory (code * 2^e is exact in bf16), and everything after that is
+// the bf16 kernel: the partial states are the bits the bf16 kernel produces on the dequantised cache.
+__device__ __forceinline__ void widen_fp8_tile(const unsigned char* raw, uint16_t* dst, float sc, int D, int LD, int BS, int NT) {
+  for (int c = threadIdx.x; c < BS * D / 16; c += NT) {  // 16 codes per chunk
+    const int row = (c * 16) / D, col = (c * 16) % D;
+    const uint4 v = *reinterpret_cast<const uint4*>(raw + (size_t)c * 16);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    uint32_t o[8];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const uint32_t c0 = (w[j] >> (16 * e)) & 0xffu, c1 = (w[j] >> (16 * e + 8)) & 0xffu;
+        const __half_raw h0 = __nv_cvt_fp8_to_halfraw((__nv_fp8_storage_t)c0, __NV_E4M3);
+        const __half_raw h1 = __nv_cvt_fp8_to_halfraw((__nv_fp8_storage_t)c1, __NV_E4M3);
+        const uint32_t b0 = __float_as_uint(__half2float(__half(h0)) * sc) >> 16;  // exact
+        const uint32_t b1 = __float_as_uint(__half2float(__half(h1)) * sc) >> 16;
+        o[2 * j + e] = b0 | (b1 << 16);
+      }
+    }
+    uint4* d = reinterpret_cast<uint4*>(dst + row * LD + col);
+    d[0] = make_uint4(o[0], o[1], o[2], o[3]);
+    d[1] = make_uint4(o[4], o[5], o[6], o[7]);
+  }
+}
+
+template <int D, int BS, bool FP8>
 __global__ void __launch_bounds__(2 * BS)
 k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
           const int32_t* __restrict__ table, const int32_t* __restrict__ seq_lens,
           const uint16_t* __restrict__ q, const int32_t* __restrict__ list, int width,
           float* __restrict__ O, float* __restrict__ Mo, float* __restrict__ Lo, int Hq, int Hkv,
-          int G, int MB, float scale) {
+          int G, int MB, float scale, const float* __restrict__ kscale, const float* __restrict__ vscale) {
   constexpr int NT = 2 * BS;   // threads
   constexpr int TW = BS / 16;  // warps, 16 tokens each
   constexpr int LD = D + 8;    // padded row stride (elements): ldmatrix conflict-free
@@ -45,7 +74,23 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
   const size_t page = (size_t)table[(size_t)b * MB + blk];
   const uint16_t* gK = kp + ((page * Hkv + h) * BS) * (size_t)D;
   const uint16_t* gV = vp + ((page * Hkv + h) * BS) * (size_t)D;
+  unsigned char* rawK = smem_raw + (size_t)2 * BS * LD * 2;  // FP8 only: [2][BS * D] codes
+  unsigned char* rawV = rawK + BS * D;
 
+  if constexpr (FP8) {
+    const unsigned char* gK8 = reinterpret_cast<const unsigned char*>(kp) + ((page * Hkv + h) * BS) * (size_t)D;
+    const unsigned char* gV8 = reinterpret_cast<const unsigned char*>(vp) + ((page * Hkv + h) * BS) * (size_t)D;
+    for (int c = tid; c < BS * D / 16; c += NT) {
+      if ((c * 16) / D < valid) cp_async16(rawK + c * 16, gK8 + c * 16);
+      else *reinterpret_cast<uint4*>(rawK + c * 16) = make_uint4(0, 0, 0, 0);
+    }
+    cp_async_commit();
+    for (int c = tid; c < BS * D / 16; c += NT) {
+      if ((c * 16) / D < valid) cp_async16(rawV + c * 16, gV8 + c * 16);
+      else *reinterpret_cast<uint4*>(rawV + c * 16) = make_uint4(0, 0, 0, 0);
+    }
+    cp_async_commit();
+  } else {
 #pragma unroll
   for (int i = 0; i < (BS * CH) / NT; ++i) {
     const int c = tid + i * NT, row = c / CH, col = c % CH;
@@ -62,6 +107,7 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
     else *reinterpret_cast<uint4*>(dst) = make_uint4(0, 0, 0, 0);
   }
   cp_async_commit();
+  }
 
   // Q fragments: A operand rows = query heads of the group (rows >= G are zero)
   const int r0 = lane >> 2, tq = lane & 3;
@@ -81,6 +127,10 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
 
   cp_async_wait<1>();
   __syncthreads();
+  if constexpr (FP8) {
+    widen_fp8_tile(rawK, Ks, kscale[page * Hkv + h], D, LD, BS, NT);
+    __syncthreads();
+  }
 
   // S = Q K^T for tokens [16*warp, 16*warp+16): two 8-token n-tiles
   const int tok0 = warp * 16;
@@ -141,6 +191,10 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
 
   cp_async_wait<0>();
   __syncthreads();
+  if constexpr (FP8) {
+    widen_fp8_tile(rawV, Vs, vscale[page * Hkv + h], D, LD, BS, NT);
+    __syncthreads();
+  }
 
   // O_w = P V over this warp's 16 tokens
   float o[D / 8][4];
@@ -283,13 +337,23 @@ k_merge(const int32_t* __restrict__ merge_src, const int32_t* __restrict__ merge
 template <int D, int BS>
 static void launch_partial_t(prr_ctx* c, const prr_paged_kv* kv, const void* q, const int32_t* list,
                              int width, float* O, float* m, float* l, cudaStream_t s) {
+  dim3 grid(width, c->Hkv, kv->batch);
+  if (c->lay.kv_dtype == PRR_FP8_E4M3) {
+    const size_t smem = (size_t)2 * BS * (D + 8) * 2 + (size_t)2 * BS * D;
+    if (smem > 48 * 1024)
+      cudaFuncSetAttribute((const void*)k_partial<D, BS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    k_partial<D, BS, true><<<grid, 2 * BS, smem, s>>>(
+        (const uint16_t*)kv->k_pages, (const uint16_t*)kv->v_pages, kv->block_table, kv->seq_lens,
+        (const uint16_t*)q, list, width, O, m, l, c->Hq, c->Hkv, c->G, c->MB, c->sm_scale,
+        c->kscale[kv->layer], c->vscale[kv->layer]);
+    return;
+  }
   const size_t smem = (size_t)2 * BS * (D + 8) * 2;
   if (smem > 48 * 1024)  // (per device and cheap: not cached in a process-wide flag)
-    cudaFuncSetAttribute((const void*)k_partial<D, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  dim3 grid(width, c->Hkv, kv->batch);
-  k_partial<D, BS><<<grid, 2 * BS, smem, s>>>(
+    cudaFuncSetAttribute((const void*)k_partial<D, BS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  k_partial<D, BS, false><<<grid, 2 * BS, smem, s>>>(
       (const uint16_t*)kv->k_pages, (const uint16_t*)kv->v_pages, kv->block_table, kv->seq_lens,
-      (const uint16_t*)q, list, width, O, m, l, c->Hq, c->Hkv, c->G, c->MB, c->sm_scale);
+      (const uint16_t*)q, list, width, O, m, l, c->Hq, c->Hkv, c->G, c->MB, c->sm_scale, nullptr, nullptr);
 }
 
 void launch_partial(prr_ctx* c, const prr_paged_kv* kv, const void* q, const int32_t* list,

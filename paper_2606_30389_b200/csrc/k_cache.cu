@@ -87,6 +87,7 @@ __global__ void k_nblocks(const int32_t* __restrict__ seq_lens, int32_t* __restr
 }
 
 void launch_build_summaries(prr_ctx* c, const prr_paged_kv* kv, void* summaries, cudaStream_t s) {
+  if (c->lay.kv_dtype == PRR_FP8_E4M3) { launch_build_summaries_fp8(c, kv, summaries, s); return; }
   dim3 grid(c->MB, c->Hkv, kv->batch);
   if (c->summary_kind == PRR_SUMMARY_QUEST) {
     k_build_minmax<<<grid, c->D, 0, s>>>((const uint16_t*)kv->k_pages, kv->block_table, kv->seq_lens,

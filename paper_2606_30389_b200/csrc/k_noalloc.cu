@@ -155,6 +155,9 @@ extern "C" int32_t prr_attend_blocks_static(prr_ctx* ctx, const prr_paged_kv* kv
   if (kv->batch < 1 || kv->batch > ctx->maxB) return fail(ctx, PRR_E_INVALID, "prr_attend_blocks_static: batch out of range");
   if (!q || !blocks || !out) return fail(ctx, PRR_E_INVALID, "prr_attend_blocks_static: null argument");
   if (width < 1 || width > 1024) return fail(ctx, PRR_E_INVALID, "prr_attend_blocks_static: width must be 1 .. 1024");
+  if (kv->layer < 0 || kv->layer >= ctx->NL) return fail(ctx, PRR_E_INVALID, "prr_attend_blocks_static: layer out of range");
+  if (ctx->lay.kv_dtype == PRR_FP8_E4M3 && (!ctx->kscale[kv->layer] || !ctx->vscale[kv->layer]))
+    return fail(ctx, PRR_E_STATE, "prr_attend_blocks_static: fp8 KV: call prr_set_kv_scales first");
   if (ctx->bs > 128) return fail(ctx, PRR_E_UNSUPPORTED, "prr_attend_blocks_static: blocks of 256 tokens run on the fused step only");
   const size_t slots = (size_t)kv->batch * ctx->Hq * (size_t)width;
   const size_t need = slots * (size_t)(ctx->D + 2) * sizeof(float);

@@ -84,7 +84,10 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   if (block_size == 256 && lay->orchestration != PRR_FUSED)
     PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: block_size 256 needs PRR_FUSED");
   if (G > 16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: GQA group > 16 unsupported");
-  if (lay->kv_dtype != PRR_BF16) PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: kv_dtype must be PRR_BF16");
+  if (lay->kv_dtype != PRR_BF16 && lay->kv_dtype != PRR_FP8_E4M3)
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: kv_dtype must be PRR_BF16 or PRR_FP8_E4M3");
+  if (lay->kv_dtype == PRR_FP8_E4M3 && (lay->orchestration != PRR_STREAMS || block_size > 128))
+    PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: PRR_FP8_E4M3 needs PRR_STREAMS and block_size <= 128");
   if (lay->max_blocks_per_seq > 32768 || K > 512 || budget > 1024)
     PRR_FAIL(none, PRR_E_UNSUPPORTED, "prr_create: max_blocks_per_seq <= 32768, K <= 512, budget <= 1024");
 
@@ -189,6 +192,7 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   c->ev_upd.assign(c->NL, nullptr);
   c->upd_pending.assign(c->NL, 0);
   c->bud_eff.assign(c->NL, c->Bud);
+  c->kscale.assign(c->NL, nullptr); c->vscale.assign(c->NL, nullptr);
   for (int l = 0; l < c->NL; ++l) A(cudaEventCreateWithFlags(&c->ev_upd[l], cudaEventDisableTiming));
   if (e != cudaSuccess) {
     g_create_err = std::string("prr_create: ") + cudaGetErrorString(e);
@@ -232,8 +236,12 @@ static int check_kv(prr_ctx* c, const prr_paged_kv* kv, const char* fn) {
     PRR_FAIL(c, PRR_E_INVALID, "%s: k_pages / v_pages must be 16-byte aligned", fn);
   if (kv->batch < 1 || kv->batch > c->maxB) PRR_FAIL(c, PRR_E_INVALID, "%s: batch out of range", fn);
   if (kv->layer < 0 || kv->layer >= c->NL) PRR_FAIL(c, PRR_E_INVALID, "%s: layer out of range", fn);
+  if (c->lay.kv_dtype == PRR_FP8_E4M3 && (!c->kscale[kv->layer] || !c->vscale[kv->layer]))
+    PRR_FAIL(c, PRR_E_STATE, "%s: fp8 KV: call prr_set_kv_scales for layer %d first", fn, kv->layer);
   return PRR_OK;
 }
+#define NO_FP8(fn) do { if (ctx && ctx->lay.kv_dtype == PRR_FP8_E4M3) \
+    PRR_FAIL(ctx, PRR_E_UNSUPPORTED, "%s: not available with PRR_FP8_E4M3 (a token cannot join a block quantised with a fixed scale)", fn); } while (0)
 #define CHECK_KV(fn) do { int _r = check_kv(ctx, kv, fn); if (_r) return _r; } while (0)
 #define CHECK_PTR(p, fn) do { if (!(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: null %s", fn, #p); \
     if (!aligned16(p)) PRR_FAIL(ctx, PRR_E_INVALID, "%s: %s must be 16-byte aligned", fn, #p); } while (0)
@@ -256,6 +264,7 @@ extern "C" int32_t prr_build_summaries(prr_ctx* ctx, const prr_paged_kv* kv, voi
 
 extern "C" int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* k_new, const void* v_new,
                               void* summaries, void* stream) {
+  NO_FP8("prr_append");
   CHECK_KV("prr_append");
   CHECK_PTR(k_new, "prr_append"); CHECK_PTR(v_new, "prr_append"); CHECK_PTR(summaries, "prr_append");
   // (PRR_STREAMS: the layer's EMA update on the side stream derives the block count from seq_lens, which
@@ -263,6 +272,27 @@ extern "C" int32_t prr_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* 
   join_layer(ctx, kv->layer, (cudaStream_t)stream);
   launch_append(ctx, kv, k_new, v_new, summaries, (cudaStream_t)stream);
   return check_launch(ctx, "prr_append");
+}
+
+extern "C" int32_t prr_quantize_kv_fp8(prr_ctx* ctx, const prr_paged_kv* kv, void* k8_pages, void* v8_pages,
+                                       float* k_scale, float* v_scale, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (!kv || !kv->k_pages || !kv->v_pages || !kv->block_table || !kv->seq_lens)
+    PRR_FAIL(ctx, PRR_E_INVALID, "prr_quantize_kv_fp8: null pointer in prr_paged_kv");
+  if (kv->batch < 1 || kv->batch > ctx->maxB) PRR_FAIL(ctx, PRR_E_INVALID, "prr_quantize_kv_fp8: batch out of range");
+  if (!k8_pages || !v8_pages || !k_scale || !v_scale) PRR_FAIL(ctx, PRR_E_INVALID, "prr_quantize_kv_fp8: null output");
+  if (!aligned16(k8_pages) || !aligned16(v8_pages)) PRR_FAIL(ctx, PRR_E_INVALID, "prr_quantize_kv_fp8: pages must be 16-byte aligned");
+  launch_quantize_fp8(ctx, kv, k8_pages, v8_pages, k_scale, v_scale, (cudaStream_t)stream);
+  return check_launch(ctx, "prr_quantize_kv_fp8");
+}
+
+extern "C" int32_t prr_set_kv_scales(prr_ctx* ctx, int32_t layer, const float* k_scale, const float* v_scale) {
+  if (!ctx) return PRR_E_INVALID;
+  if (ctx->lay.kv_dtype != PRR_FP8_E4M3) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_kv_scales: the ctx was not created with PRR_FP8_E4M3");
+  if (layer < 0 || layer >= ctx->NL) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_kv_scales: layer out of range");
+  if (!k_scale || !v_scale) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_kv_scales: null argument");
+  ctx->kscale[layer] = k_scale; ctx->vscale[layer] = v_scale;
+  return PRR_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -746,6 +776,7 @@ extern "C" int32_t prr_decode_step(prr_ctx* ctx, const prr_paged_kv* kv, const v
 extern "C" int32_t prr_step_append(prr_ctx* ctx, const prr_paged_kv* kv, const void* q, const void* k_new,
                                    const void* v_new, void* summaries, float* out, int32_t sequential,
                                    void* stream) {
+  NO_FP8("prr_step_append");
   CHECK_KV("prr_step_append");
   CHECK_PTR(q, "prr_step_append"); CHECK_PTR(k_new, "prr_step_append"); CHECK_PTR(v_new, "prr_step_append");
   CHECK_PTR(summaries, "prr_step_append");
@@ -762,6 +793,7 @@ extern "C" int32_t prr_step_append(prr_ctx* ctx, const prr_paged_kv* kv, const v
 extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_host,
                                         const void* k_new_host, const void* v_new_host, void* summaries,
                                         float* out_host, void* stream) {
+  NO_FP8("prr_decode_step_host");
   CHECK_KV("prr_decode_step_host");
   if (!q_host || !k_new_host || !v_new_host || !out_host || !summaries)
     PRR_FAIL(ctx, PRR_E_INVALID, "prr_decode_step_host: null argument");

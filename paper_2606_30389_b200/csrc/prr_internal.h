@@ -75,6 +75,7 @@ struct prr_ctx {
   std::vector<int> bud_eff;        // per layer: blocks predicted for the next step, 0 .. Bud (prr_set_budget)
   std::vector<double> bud_poly;    // fitted budget(context length): coefficients in x = ctx_len / bud_xscale (prr_budget_fit)
   double bud_xscale = 1.0;
+  std::vector<const float*> kscale, vscale;  // per layer: fp8 scales [n_pages, Hkv] (prr_set_kv_scales), caller-owned
   std::vector<void*> allocs;
   int64_t launches = 0;
   std::string err;
@@ -92,6 +93,9 @@ void launch_build_summaries(prr_ctx* c, const prr_paged_kv* kv, void* summaries,
 void launch_append(prr_ctx* c, const prr_paged_kv* kv, const void* k_new, const void* v_new,
                    void* summaries, cudaStream_t s);
 void launch_nblocks(prr_ctx* c, const int32_t* seq_lens, int batch, int32_t* nblk, cudaStream_t s);
+// k_fp8.cu (PRR_FP8_E4M3)
+void launch_quantize_fp8(prr_ctx* c, const prr_paged_kv* kv, void* k8, void* v8, float* kscale, float* vscale, cudaStream_t s);
+void launch_build_summaries_fp8(prr_ctx* c, const prr_paged_kv* kv, void* summaries, cudaStream_t s);
 // k_score.cu
 void launch_score(prr_ctx* c, const prr_paged_kv* kv, const void* q, const void* summaries,
                   float* scores, cudaStream_t s);

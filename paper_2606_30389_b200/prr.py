@@ -22,6 +22,7 @@ OPT_LAST_CLUSTER, OPT_LAST_RING, OPT_LAST_GRID, OPT_LAST_KERNEL = 16, 17, 18, 19
 KERNEL_AUTO, KERNEL_PERSISTENT, KERNEL_CLUSTER = 0, 1, 2
 MODE_S3, MODE_S2, MODE_S1 = 0, 1, 2
 FUSED, STREAMS = 0, 1
+BF16, FP8_E4M3 = 0, 1
 
 SYMBOLS = [
     "prr_create", "prr_destroy", "prr_last_error", "prr_version", "prr_build_summaries", "prr_append",
@@ -32,7 +33,7 @@ SYMBOLS = [
     "prr_get_sets", "prr_get_scores", "prr_get_ema", "prr_get_stats", "prr_check", "prr_launch_count",
     "prr_timeline_enable", "prr_timeline_read", "prr_timeline_peek", "prr_set_option", "prr_get_option",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
-    "prr_static_scratch_bytes", "prr_attend_blocks_static",
+    "prr_static_scratch_bytes", "prr_attend_blocks_static", "prr_quantize_kv_fp8", "prr_set_kv_scales",
 ]
 
 
@@ -112,9 +113,9 @@ class Context:
     """prr_ctx handle.  Methods take torch CUDA tensors with the layouts of include/prr.h."""
 
     def __init__(self, n_q_heads, n_kv_heads, head_dim, block_size, K, budget, max_batch=1,
-                 max_blocks_per_seq=1, n_layers=1, policy=DROP, sm_scale=0.0, orchestration=FUSED):
+                 max_blocks_per_seq=1, n_layers=1, policy=DROP, sm_scale=0.0, orchestration=FUSED, kv_dtype=BF16):
         self.layout = Layout(n_q_heads, n_kv_heads, head_dim, max_batch, max_blocks_per_seq, n_layers,
-                             0, policy, sm_scale, orchestration)
+                             kv_dtype, policy, sm_scale, orchestration)
         self.block_size, self.K, self.budget = block_size, K, budget
         self._h = C.c_void_p()
         r = lib().prr_create(C.byref(self.layout), block_size, K, budget, C.byref(self._h))
@@ -203,6 +204,15 @@ class Context:
                                    C.c_void_p(_p(P)), C.c_void_p(_p(O_part)), C.c_void_p(_p(m_part)),
                                    C.c_void_p(_p(l_part)), C.c_void_p(_p(out)), C.c_void_p(_p(m_out)),
                                    C.c_void_p(_p(l_out)), C.c_void_p(_stream(stream))))
+
+    def quantize_kv_fp8(self, kv, k8_pages, v8_pages, k_scale, v_scale, stream=None):
+        self._chk(lib().prr_quantize_kv_fp8(self._h, C.byref(kv), C.c_void_p(_p(k8_pages)), C.c_void_p(_p(v8_pages)),
+                                            C.c_void_p(_p(k_scale)), C.c_void_p(_p(v_scale)), C.c_void_p(_stream(stream))))
+
+    def set_kv_scales(self, layer, k_scale, v_scale):
+        self._keep_scales = getattr(self, "_keep_scales", {})
+        self._keep_scales[layer] = (k_scale, v_scale)
+        self._chk(lib().prr_set_kv_scales(self._h, C.c_int32(layer), C.c_void_p(_p(k_scale)), C.c_void_p(_p(v_scale))))
 
     def attend_blocks_static(self, kv, q, blocks, width, out, m_out=None, l_out=None, stream=None):
         """prr_attend_blocks_static: attention over given block lists; partial states in the library's static scratch."""
