@@ -71,6 +71,7 @@ struct RowArgs {
   int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
       o_slots, o_slotblk, o_recv, o_end;
   float scale; double score_c;
+  uint32_t* done_host; uint32_t done_seq;  // host-visible completion word (mapped host memory) and its value, or null
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -1579,6 +1580,10 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
   if (tid == 0) {
     __threadfence();
     const uint32_t last = atomicAdd(&a.ctl[CTL_EXIT], 1u) == gridDim.x - 1 ? 1u : 0u;
+    if (last && a.done_host) {
+      __threadfence_system();
+      *reinterpret_cast<volatile uint32_t*>(a.done_host) = a.done_seq;
+    }
     if (last) {
       a.ctl[CTL_EXIT] = 0u;
       *a.parity = par_raw ^ 1;
@@ -1749,6 +1754,7 @@ int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const
   a.kp_w = (uint16_t*)kv->k_pages; a.vp_w = (uint16_t*)kv->v_pages; a.summ_w = (uint4*)summaries;
   a.open_sum = c->open_sum + (size_t)kv->layer * c->maxB * c->Hkv * c->D; a.seq_lens_w = (int32_t*)kv->seq_lens;
   a.q = (const uint16_t*)q; a.summ = (const uint4*)summaries; a.out = out;
+  a.done_host = c->arm_seq ? c->done_d : nullptr; a.done_seq = c->arm_seq; c->arm_seq = 0;
   a.scores = c->scores + r * c->MB;
   a.ema_l = c->ema_l + r * c->MB; a.ema_v = c->ema_v + r * c->MB;
   a.n_state = c->n_state + r;

@@ -427,6 +427,7 @@ struct StepArgs {
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, BudSel, Rmax, retain, spec, buf_bytes, scr_bytes, J, CR;  // BudSel <= Bud: the run-time budget of the NEXT prediction
   int msw;  // channels per merge item (16 .. D): the narrowest slice that still gives every merge warp at most one item
   float scale; float pace_ns; double score_c;
+  uint32_t* done_host; uint32_t done_seq;  // host-visible completion word (mapped host memory) and its value, or null
 };
 
 __device__ __forceinline__ int seq_len(const StepArgs& a, int b) { return __ldcg(a.seq_lens + b) + a.app; }
@@ -1611,6 +1612,10 @@ __global__ void __launch_bounds__(32 * Tile<D, BS>::WMAX, 1) k_step(const __grid
   }
   last = __shfl_sync(FULL, last, 0);
   if (last) {
+    if (a.done_host && lane == 0) {  // every warp's results are ordered before its exit ticket (gpu scope); this fence carries them to the host
+      __threadfence_system();
+      *reinterpret_cast<volatile uint32_t*>(a.done_host) = a.done_seq;
+    }
     if (a.app)
       for (int b = lane; b < a.B; b += 32)
         if (a.seq_lens_w[b] / a.bs < a.MB) a.seq_lens_w[b] += 1;  // (a full sequence: nothing was written, the length stays, as in k_append)
@@ -1734,6 +1739,7 @@ static int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const 
   a.kp_w = (uint16_t*)kv->k_pages; a.vp_w = (uint16_t*)kv->v_pages; a.summ_w = (uint4*)summaries;
   a.open_sum = c->open_sum + (size_t)kv->layer * c->maxB * c->Hkv * c->D; a.seq_lens_w = (int32_t*)kv->seq_lens;
   a.q = (const uint16_t*)q; a.summ = (const uint4*)summaries; a.out = out;
+  a.done_host = c->arm_seq ? c->done_d : nullptr; a.done_seq = c->arm_seq; c->arm_seq = 0;
   a.scores = c->scores + r * c->MB;
   a.ema_l = c->ema_l + r * c->MB; a.ema_v = c->ema_v + r * c->MB;
   a.n_state = c->n_state + r;

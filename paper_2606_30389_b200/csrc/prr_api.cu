@@ -1,5 +1,7 @@
 // C-ABI entry points of libprr (include/prr.h): argument validation, state allocation and the
 // two-stream, event-ordered orchestration of one PRR layer-step (Fig. 1, :38-42).
+#include <atomic>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <algorithm>
@@ -174,6 +176,8 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   if (e == cudaSuccess) e = cudaHostAlloc(&c->st_pin, st_elems * sizeof(uint16_t), cudaHostAllocDefault);
   if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->st_out_h, std::min(qrows * c->D * sizeof(float), (size_t)HOST_OUT_DIRECT), cudaHostAllocMapped);
   if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->st_out_hd, c->st_out_h, 0);
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->done_h, 64, cudaHostAllocMapped);
+  if (e == cudaSuccess) { *c->done_h = 0u; e = cudaHostGetDevicePointer((void**)&c->done_d, (void*)c->done_h, 0); }
   if (e == cudaSuccess) {
     // P lists start empty (-1); theta defaults to (1, 1, 0): "reuse the last step's top-K" (S1)
     e = cudaMemset(c->P_next, 0xff, rows * (size_t)(c->Bud + 1) * sizeof(int32_t));
@@ -211,6 +215,7 @@ extern "C" int32_t prr_destroy(prr_ctx* c) {
   for (void* p : c->allocs) cudaFree(p);
   if (c->st_pin) cudaFreeHost(c->st_pin);
   if (c->st_out_h) cudaFreeHost(c->st_out_h);
+  if (c->done_h) cudaFreeHost((void*)c->done_h);
   if (c->tl) cudaFreeHost(c->tl);
   if (c->cal_state) cudaFree(c->cal_state);
   if (c->cal_mask) cudaFree(c->cal_mask);
@@ -832,10 +837,28 @@ extern "C" int32_t prr_decode_step_host(prr_ctx* ctx, const prr_paged_kv* kv, co
     if (ctx->out_seen_d) { out_d = ctx->out_seen_d; direct = true; }
     else { out_d = ctx->st_out_hd; staged = true; }
   }
+  // A result the kernel stores into host memory is announced the same way: the step's last warp stores a sequence
+  // number into a mapped host word (system-scope release after every result); polling it costs ~1 us where
+  // cudaStreamSynchronize costs the driver's wake-up.  Later work on `stream` is stream-ordered behind the kernel as usual.
+  const bool poll = (direct || staged) && ctx->fused && ctx->done_h;
+  uint32_t seq = 0;
+  if (poll) { seq = ++ctx->done_seq ? ctx->done_seq : ++ctx->done_seq; ctx->arm_seq = seq; }
   const int r = prr_step_append(ctx, kv, ctx->st_q, ctx->st_k, ctx->st_v, summaries, out_d, 0, stream);
+  ctx->arm_seq = 0;
   if (r) return r;
   if (!direct && !staged) PRR_CUDA(ctx, cudaMemcpyAsync(out_host, ctx->st_out, qb * sizeof(float), cudaMemcpyDeviceToHost, s));
-  PRR_CUDA(ctx, cudaStreamSynchronize(s));
+  bool seen = false;
+  if (poll) {
+    const auto t0 = std::chrono::steady_clock::now();
+    for (uint32_t it = 0; !(seen = *ctx->done_h == seq); ++it) {
+      if ((it & 0xfffu) == 0xfffu) {  // give up polling after 50 ms (a failed launch never stores the word): synchronise instead
+        if (std::chrono::steady_clock::now() - t0 > std::chrono::milliseconds(50)) break;
+        if (cudaStreamQuery(s) != cudaErrorNotReady) break;
+      }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+  }
+  if (!seen) PRR_CUDA(ctx, cudaStreamSynchronize(s));
   if (staged) memcpy(out_host, ctx->st_out_h, qb * sizeof(float));
   return PRR_OK;
 }

@@ -66,6 +66,9 @@ struct prr_ctx {
   void *st_q = nullptr, *st_k = nullptr, *st_v = nullptr; float* st_out = nullptr;
   float* st_out_h = nullptr; float* st_out_hd = nullptr;  // small results: the kernel stores them into mapped host memory (no D2H copy)
   const void* out_seen = nullptr; float* out_seen_d = nullptr;  // last caller buffer and its device alias (null: not mapped)
+  // completion word in mapped host memory: a fused step armed with arm_seq != 0 stores that value there (system-scope
+  // release after its last result) so that prr_decode_step_host can poll it instead of synchronising the stream
+  volatile uint32_t* done_h = nullptr; uint32_t* done_d = nullptr; uint32_t done_seq = 0, arm_seq = 0;
   void* st_pin = nullptr;  // pinned host image of [q | k_new | v_new] for one copy across PCIe
 
   cudaStream_t side_spec = nullptr, side_ema = nullptr;
