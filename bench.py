@@ -333,6 +333,7 @@ def main():
                          "profiled run chose: the ncu captures use it to skip the sweep)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "persistent", "cluster"])
     ap.add_argument("--cluster", type=int, default=0, help="force the cluster size of k_row (0 = the library's choice)")
+    ap.add_argument("--subtile", type=int, default=0, help="PRR_OPT_SUBTILE: tokens per tile unit of k_row (16 / 32 / 64)")
     ap.add_argument("--sweep", action="store_true", help="Table-3-shaped sweep: block size x token budget at 128K, 32q/8kv")
     args = ap.parse_args()
 
@@ -372,6 +373,8 @@ def main():
     st = Stack(cfg, R, tokens, dev, seed_off=rank_seed_offset(rank), kernel=kern)
     if args.cluster:
         st.ctx.set_option(st.prr.OPT_CLUSTER, args.cluster)
+    if args.subtile:
+        st.ctx.set_option(st.prr.OPT_SUBTILE, args.subtile)
     cal_s = st.calibrate()
     stream = torch.cuda.Stream(device=dev)
     # ---- speculation budget: the library's profiling-guided choice (PAPER.md 204-208), capped by the config's
@@ -500,6 +503,8 @@ def main():
         "sequential_us": seq_us, "speedup_vs_sequential": (seq_us / us_step) if seq_us else None,
         "hit_rate": stats[1] / max(stats[0], 1), "mean_missed_per_row": stats[2] * K and stats[2] / (K * cfg.B * cfg.Hkv),
         "budget": budget_info,
+        "launch_shape": {"cluster": st.ctx.get_option(st.prr.OPT_LAST_CLUSTER), "ring": st.ctx.get_option(st.prr.OPT_LAST_RING),
+                         "grid": st.ctx.get_option(st.prr.OPT_LAST_GRID)},
         "fused_kernel": {1: "k_step (persistent cooperative grid, warps as workers)",
                          2: "k_row (one thread-block cluster per (sequence, KV head) row)"}.get(
                              st.ctx.get_option(st.prr.OPT_LAST_KERNEL), "?"),

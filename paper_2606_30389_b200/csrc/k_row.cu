@@ -1646,7 +1646,8 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
   const int SW = D + 4, SLOTF = a.G * SW;
   // a slot per speculative unit of a CTA if they fit (a unit whose fate is unknown and that finds no slot
   // holds its warp until A is known); then the deepest ring; a ring of at least four tenants comes first
-  a.NSLOT = std::max(1, std::min(16, ((a.Bud + CS - 1) / CS) * ((a.bs + ST - 1) / ST)));
+  // (the sequential path parks nothing: its shared memory goes to the ring)
+  a.NSLOT = a.spec ? std::max(1, std::min(16, ((a.Bud + CS - 1) / CS) * ((a.bs + ST - 1) / ST))) : 1;
   const int min_ring = 4;
   const int budget = c->row_dyn[key];
   int NBUF = NBMAX;
