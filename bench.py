@@ -316,6 +316,62 @@ def sweep(args):
                       "peak_gbs": peak, "peak_source": peak_src, "cells": cells}), flush=True)
 
 
+def stage_fp8(args):
+    """prr_speculate (the per-block partial-state kernel, a4 / a6) over budget-many predicted blocks per row of the
+    config: bf16 pages against fp8 (e4m3) pages with per-block power-of-two scales.  Random
+    block lists, R layer caches round-robin (inputs larger than L2), CUDA events around `steps` launches."""
+    from paper_2606_30389_b200 import prr
+    cfg = synth.CONFIGS[args.config]
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(0)
+    R, n = args.layers, min(args.steps, 2048)
+    peak, peak_src = peaks()
+    res = {}
+    inps = [synth.make_layer(cfg, l, device=dev, steps=1, poison=False) for l in range(R)]
+    MB = inps[0].block_table.shape[1]
+    g = torch.Generator(device="cpu").manual_seed(7)
+    nb_min = int(min(int(i.seq_lens.min().item()) for i in inps) // cfg.bs)
+    P = torch.stack([torch.stack([torch.randperm(nb_min, generator=g)[:cfg.Bud].sort().values for _ in range(cfg.Hkv)])
+                     for _ in range(cfg.B)]).to(torch.int32).to(dev)
+    q = inps[0].q_dec[0].contiguous()
+    O_ = torch.zeros(cfg.B, cfg.Hq, cfg.Bud, cfg.d, dtype=torch.float32, device=dev)
+    m_ = torch.zeros(cfg.B, cfg.Hq, cfg.Bud, dtype=torch.float32, device=dev)
+    l_ = torch.zeros_like(m_)
+    for name, dt in (("bf16", prr.BF16), ("fp8_e4m3", prr.FP8_E4M3)):
+        ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B, max_blocks_per_seq=MB, n_layers=R,
+                          orchestration=prr.STREAMS, kv_dtype=dt)
+        kvs, keep = [], []
+        for l, inp in enumerate(inps):
+            if dt == prr.BF16:
+                kvs.append(ctx.kv(inp.k_pages, inp.v_pages, inp.block_table, inp.seq_lens, l))
+            else:
+                k8 = torch.zeros(inp.k_pages.shape, dtype=torch.uint8, device=dev); v8 = torch.zeros_like(k8)
+                ks = torch.ones(inp.k_pages.shape[0], cfg.Hkv, dtype=torch.float32, device=dev); vs = torch.ones_like(ks)
+                ctx.quantize_kv_fp8(ctx.kv(inp.k_pages, inp.v_pages, inp.block_table, inp.seq_lens, l), k8, v8, ks, vs)
+                ctx.set_kv_scales(l, ks, vs)
+                keep.append((k8, v8, ks, vs))
+                kvs.append(ctx.kv(k8, v8, inp.block_table, inp.seq_lens, l))
+        stream = torch.cuda.Stream(device=dev)
+        with torch.cuda.stream(stream):
+            for i in range(2 * R):
+                ctx.speculate(kvs[i % R], q, P, O_, m_, l_, stream=stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for i in range(n):
+                ctx.speculate(kvs[i % R], q, P, O_, m_, l_, stream=stream)
+            e1.record(stream)
+        e1.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / n
+        byts = cfg.B * cfg.Hkv * cfg.Bud * cfg.bs * cfg.d * 2 * (2 if dt == prr.BF16 else 1)
+        res[name] = {"us_per_launch": round(us, 2), "kv_bytes": byts, "GBs": round(byts / us / 1e3, 1),
+                     "frac_of_hbm_peak": round(byts / us / 1e3 / peak, 3)}
+        ctx.check()
+        ctx.destroy()
+    print(json.dumps({"stage": "prr_speculate (k_partial): per-block partial states of budget-many blocks per row", "config": cfg.name,
+                      "launches": n, "layer_caches": R, "peak_gbs": peak, "peak_source": peak_src, **res,
+                      "speedup_fp8": round(res["bf16"]["us_per_launch"] / res["fp8_e4m3"]["us_per_launch"], 3)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -334,6 +390,7 @@ def main():
     ap.add_argument("--kernel", default="auto", choices=["auto", "persistent", "cluster"])
     ap.add_argument("--cluster", type=int, default=0, help="force the cluster size of k_row (0 = the library's choice)")
     ap.add_argument("--subtile", type=int, default=0, help="PRR_OPT_SUBTILE: tokens per tile unit of k_row (16 / 32 / 64)")
+    ap.add_argument("--stage-fp8", action="store_true", help="prr_speculate on bf16 vs fp8 (e4m3) pages of the config")
     ap.add_argument("--sweep", action="store_true", help="Table-3-shaped sweep: block size x token budget at 128K, 32q/8kv")
     args = ap.parse_args()
 
@@ -350,6 +407,8 @@ def main():
     cfg = synth.CONFIGS[args.config]
     if args.sweep:
         return sweep(args)
+    if args.stage_fp8:
+        return stage_fp8(args)
     if args.impl == "reference":
         if args.steps == 16384:
             args.steps, args.warmup = 12, 3

@@ -26,25 +26,34 @@ constexpr float LOG2E = 1.4426950408889634f;
 // and kscale / vscale [n_pages, Hkv] their power-of-two scales.  The codes are staged raw (half the bytes
 // from HBM), widened to bf16 in shared memory (code * 2^e is exact in bf16), and everything after that is
 // the bf16 kernel: the partial states are the bits the bf16 kernel produces on the dequantised cache.
-__device__ __forceinline__ void widen_fp8_tile(const unsigned char* raw, uint16_t* dst, float sc, int D, int LD, int BS, int NT) {
-  for (int c = threadIdx.x; c < BS * D / 16; c += NT) {  // 16 codes per chunk
-    const int row = (c * 16) / D, col = (c * 16) % D;
-    const uint4 v = *reinterpret_cast<const uint4*>(raw + (size_t)c * 16);
-    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+
+// The raw codes of a tile land in the TAIL of the tile's own bf16 region (BS * D bytes of its BS * LD * 2) and are
+// widened in place: every thread first reads all of its chunks into registers, the block synchronises, then the
+// bf16 rows are written -- so the fp8 kernel needs no more shared memory (and runs at the occupancy) of the bf16 one.
+template <int D, int BS>
+__device__ __forceinline__ void widen_fp8_tile(uint16_t* tile, float sc) {
+  constexpr int NT = 2 * BS, LD = D + 8, NCH = (BS * D / 16) / NT;  // chunks of 16 codes per thread
+  const unsigned char* raw = reinterpret_cast<const unsigned char*>(tile) + (size_t)BS * LD * 2 - (size_t)BS * D;
+  uint4 v[NCH];
+#pragma unroll
+  for (int i = 0; i < NCH; ++i) v[i] = *reinterpret_cast<const uint4*>(raw + (size_t)(threadIdx.x + i * NT) * 16);
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < NCH; ++i) {
+    const int c = threadIdx.x + i * NT, row = (c * 16) / D, col = (c * 16) % D;
+    const uint32_t w[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
     uint32_t o[8];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const uint32_t c0 = (w[j] >> (16 * e)) & 0xffu, c1 = (w[j] >> (16 * e + 8)) & 0xffu;
-        const __half_raw h0 = __nv_cvt_fp8_to_halfraw((__nv_fp8_storage_t)c0, __NV_E4M3);
-        const __half_raw h1 = __nv_cvt_fp8_to_halfraw((__nv_fp8_storage_t)c1, __NV_E4M3);
-        const uint32_t b0 = __float_as_uint(__half2float(__half(h0)) * sc) >> 16;  // exact
-        const uint32_t b1 = __float_as_uint(__half2float(__half(h1)) * sc) >> 16;
-        o[2 * j + e] = b0 | (b1 << 16);
+      for (int e = 0; e < 2; ++e) {  // two codes per conversion instruction (cvt.rn.f16x2.e4m3x2), exact
+        const __half2_raw h2 = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)((w[j] >> (16 * e)) & 0xffffu), __NV_E4M3);
+        const float2 f = __half22float2(__half2(h2));
+        // code * 2^e is exact in fp32 and its low 16 bits are zero: the bf16 pair is the two high halves
+        o[2 * j + e] = __byte_perm(__float_as_uint(f.x * sc), __float_as_uint(f.y * sc), 0x7632);
       }
     }
-    uint4* d = reinterpret_cast<uint4*>(dst + row * LD + col);
+    uint4* d = reinterpret_cast<uint4*>(tile + row * LD + col);
     d[0] = make_uint4(o[0], o[1], o[2], o[3]);
     d[1] = make_uint4(o[4], o[5], o[6], o[7]);
   }
@@ -74,8 +83,9 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
   const size_t page = (size_t)table[(size_t)b * MB + blk];
   const uint16_t* gK = kp + ((page * Hkv + h) * BS) * (size_t)D;
   const uint16_t* gV = vp + ((page * Hkv + h) * BS) * (size_t)D;
-  unsigned char* rawK = smem_raw + (size_t)2 * BS * LD * 2;  // FP8 only: [2][BS * D] codes
-  unsigned char* rawV = rawK + BS * D;
+  // FP8 only: the raw codes land in the tail of each tile's own region (widen_fp8_tile)
+  unsigned char* rawK = reinterpret_cast<unsigned char*>(Ks) + (size_t)BS * LD * 2 - (size_t)BS * D;
+  unsigned char* rawV = reinterpret_cast<unsigned char*>(Vs) + (size_t)BS * LD * 2 - (size_t)BS * D;
 
   if constexpr (FP8) {
     const unsigned char* gK8 = reinterpret_cast<const unsigned char*>(kp) + ((page * Hkv + h) * BS) * (size_t)D;
@@ -128,7 +138,7 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
   cp_async_wait<1>();
   __syncthreads();
   if constexpr (FP8) {
-    widen_fp8_tile(rawK, Ks, kscale[page * Hkv + h], D, LD, BS, NT);
+    widen_fp8_tile<D, BS>(Ks, kscale[page * Hkv + h]);
     __syncthreads();
   }
 
@@ -192,7 +202,7 @@ k_partial(const uint16_t* __restrict__ kp, const uint16_t* __restrict__ vp,
   cp_async_wait<0>();
   __syncthreads();
   if constexpr (FP8) {
-    widen_fp8_tile(rawV, Vs, vscale[page * Hkv + h], D, LD, BS, NT);
+    widen_fp8_tile<D, BS>(Vs, vscale[page * Hkv + h]);
     __syncthreads();
   }
 
@@ -339,7 +349,7 @@ static void launch_partial_t(prr_ctx* c, const prr_paged_kv* kv, const void* q, 
                              int width, float* O, float* m, float* l, cudaStream_t s) {
   dim3 grid(width, c->Hkv, kv->batch);
   if (c->lay.kv_dtype == PRR_FP8_E4M3) {
-    const size_t smem = (size_t)2 * BS * (D + 8) * 2 + (size_t)2 * BS * D;
+    const size_t smem = (size_t)2 * BS * (D + 8) * 2;
     if (smem > 48 * 1024)
       cudaFuncSetAttribute((const void*)k_partial<D, BS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_partial<D, BS, true><<<grid, 2 * BS, smem, s>>>(
