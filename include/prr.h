@@ -180,8 +180,8 @@ int32_t prr_get_budget(const prr_ctx* ctx, int32_t layer, int32_t* budget_out /*
  * selection window; timing the whole critical path per budget measures what that comparison stands for,
  * including the repair work a smaller budget causes.  us_out (host float [n_budgets]) = median us per step
  * (the first step is a warm-up), us_sequential_out (host float) likewise, best_budget_out (host) = the
- * candidate with the smallest time if that beats the sequential path by more than 2 %, else 0 ("largest safe
- * delta" here is the fastest one that is safely faster than not speculating).  The layer's predictor state, prediction buffers, counters and budget are saved
+ * LARGEST candidate whose time is within 1 % of the fastest candidate's and beats the sequential path by more
+ * than 2 %, else 0 (the paper's "largest safe delta", with "safe" measured on the whole critical path).  The layer's predictor state, prediction buffers, counters and budget are saved
  * before and restored after.  Synchronises `stream`; not allowed inside a stream capture. */
 int32_t prr_profile_budget(prr_ctx* ctx, const prr_paged_kv* kv, const void* q_traj, int32_t T,
                            const void* summaries, const int32_t* budgets, int32_t n_budgets, int32_t cold_l2,

@@ -543,19 +543,26 @@ extern "C" int32_t prr_profile_budget(prr_ctx* ctx, const prr_paged_kv* kv, cons
     *us = v[v.size() / 2] * 1e3f;
   };
   float best_us = 0.f, seq_us = 0.f;
+  (void)best_us;
   int best = 0;
   if (e == cudaSuccess) {
     run(0, true, &seq_us);
     // No speculation at all is the fallback PRR must beat, and "safe" is read with a
     // margin: a budget is taken only if it beats the sequential path by more than 2 % (differences below that are
     // run-to-run noise of the sweep, and a wrong "yes" costs bandwidth on every step).
-    best_us = seq_us * 0.98f; best = 0;
+    // Among the budgets that are safe, the LARGEST one within 1 % of the fastest is taken ("largest safe
+    // delta": a larger prediction costs nothing while it hides behind selection, and it raises the hit rate).
+    std::vector<float> uss(n_budgets, 0.f);
+    float min_us = seq_us * 0.98f;
+    best = 0;
     for (int i = 0; i < n_budgets && rc == PRR_OK; ++i) {
-      float us = 0.f;
-      run(budgets[i], false, &us);
-      if (us_out) us_out[i] = us;
-      if (rc == PRR_OK && budgets[i] > 0 && us < best_us) { best_us = us; best = budgets[i]; }
+      run(budgets[i], false, &uss[i]);
+      if (us_out) us_out[i] = uss[i];
+      if (rc == PRR_OK && budgets[i] > 0 && uss[i] < min_us) min_us = uss[i];
     }
+    for (int i = 0; i < n_budgets && rc == PRR_OK; ++i)
+      if (budgets[i] > best && uss[i] < seq_us * 0.98f && uss[i] <= min_us * 1.01f) best = budgets[i];
+    best_us = min_us;
     restore();
     ctx->bud_eff[layer] = saved_budget;
     repredict(ctx, layer, s);
