@@ -172,6 +172,13 @@ int32_t prr_ema_update(prr_ctx* ctx, int32_t layer, int32_t batch, const float* 
  * degenerates to select-then-attend through the repair path. */
 int32_t prr_set_budget(prr_ctx* ctx, int32_t layer, int32_t budget, void* stream);
 int32_t prr_get_budget(const prr_ctx* ctx, int32_t layer, int32_t* budget_out /* host */);
+/* Batch-aware budgets (PAPER.md:319 leaves coordination across the requests of a batch as future work; DESIGN.md
+ * section 11): the sequences of a batch differ in locality, so each (layer, sequence) may carry its OWN run-time
+ * budget: 0 .. the budget of prr_create, or -1 = follow the layer's (the default).  One fused launch then serves
+ * sequences that speculate and sequences that do not (their rows go through the repair path alone).  The call
+ * re-predicts the layer's next P at once; a per-sequence budget stays until it is set to -1. */
+int32_t prr_set_budget_seq(prr_ctx* ctx, int32_t layer, int32_t seq, int32_t budget, void* stream);
+int32_t prr_get_budget_seq(const prr_ctx* ctx, int32_t layer, int32_t seq, int32_t* budget_out /* host */);
 /* The paper's offline sweep, in the library: for every candidate budget (host int32 [n_budgets]) run the T
  * decode steps of a query trajectory q_traj (dev bf16 [T, batch, n_q_heads, head_dim], e.g. the prefill
  * trajectory used for prr_calibrate) on the layer's cache WITHOUT appending, each step timed by CUDA events

@@ -472,6 +472,12 @@ class OracleLayer:
     def n_blocks(self):
         return np.array([n_blocks_of(n, self.bs) for n in self.lens], dtype=np.int64)
 
+    def budget_of(self, b: int) -> int:
+        """|P| <= delta K (Eq. 1) with delta a per-sequence input: `budget_seq[b]` if set (a list with one
+        entry per sequence, None = the layer's budget), else the layer's budget."""
+        bs_ = getattr(self, "budget_seq", None)
+        return self.budget if bs_ is None or bs_[b] is None else int(bs_[b])
+
     def scores(self, q_bits):
         return (score if self.summary == "mean" else score_quest)(q_bits, self.summ, self.n_blocks())
 
@@ -525,7 +531,7 @@ class OracleLayer:
             _, _, gamma = self.theta[b]
             for h in range(self.Hkv):
                 A = topk(IS[b, h, :nb[b]], self.K)
-                P = ema_predict_set(self.ema[b][h], gamma, self.budget)
+                P = ema_predict_set(self.ema[b][h], gamma, self.budget_of(b))
                 M, N = diff_sets(A, P)
                 A_b.append(A); P_b.append(P); M_b.append(M); N_b.append(N)
             S = A_b if self.policy == DROP else [np.union1d(a, p) for a, p in zip(A_b, P_b)]

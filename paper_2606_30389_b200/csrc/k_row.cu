@@ -72,6 +72,7 @@ struct RowArgs {
       o_slots, o_slotblk, o_recv, o_end;
   float scale; double score_c;
   uint32_t* done_host; uint32_t done_seq;  // host-visible completion word (mapped host memory) and its value, or null
+  const int32_t* bud_seq;  // per sequence of the layer: 0 = the layer's budget, v > 0 = budget v - 1 (prr_set_budget_seq)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -1456,7 +1457,8 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           MARK(800);
           wait_bar(&sh.bar_pred, ipar, err, 13);
           MARK(801);
-          const int kp = min(a.BudSel, nb);
+          const int bsel = a.bud_seq[b] > 0 ? min(a.bud_seq[b] - 1, a.Bud) : a.BudSel;
+          const int kp = min(bsel, nb);
           if (kp == 0) {
             for (int w = g.tid; w < a.MBw; w += g.nt) emask[w] = 0u;
           } else if (nb <= 128 * 18 && kp <= 128) {
@@ -1766,6 +1768,7 @@ int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const
   a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32 + 1;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.NBH = c->MB; a.BudSel = c->bud_eff[kv->layer];
+  a.bud_seq = c->bud_seq + (size_t)kv->layer * c->maxB;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.cut = c->cut;

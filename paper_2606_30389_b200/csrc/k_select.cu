@@ -146,6 +146,7 @@ struct EmaKArgs {
   const float* scores; const int32_t* seq_lens; const int32_t* n_blocks;
   int32_t* P_out; int32_t* P_count; int32_t* P_save;
   int Hkv, MB, Bud, BudSel, bs;  // Bud: width of a P row; BudSel <= Bud: blocks predicted (the run-time budget)
+  const int32_t* bud_seq;        // per sequence (already offset): 0 = the layer's budget, v > 0 = budget v - 1
 };
 
 __global__ void __launch_bounds__(SEL_NT) k_ema(EmaKArgs a) {
@@ -194,7 +195,8 @@ __global__ void __launch_bounds__(SEL_NT) k_ema(EmaKArgs a) {
     for (int j = tid; j < a.Bud; j += SEL_NT) a.P_save[(size_t)row * a.Bud + j] = P_row[j];
   __syncthreads();
   if (a.scores && tid == 0) a.n_state[row] = n_new;
-  const int k = min(a.BudSel, n_new);
+  const int bsel = a.bud_seq[bi] > 0 ? min(a.bud_seq[bi] - 1, a.Bud) : a.BudSel;  // (prr_set_budget_seq)
+  const int k = min(bsel, n_new);
   int cnt = 0;
   if (k > 0) {
     uint32_t T;
@@ -237,6 +239,7 @@ void launch_ema(prr_ctx* c, const EmaArgs& e, cudaStream_t s) {
   a.MB = c->MB;
   a.Bud = c->Bud;
   a.BudSel = c->bud_eff[e.layer];
+  a.bud_seq = c->bud_seq + (size_t)e.layer * c->maxB + e.seq0;
   a.bs = c->bs;
   const size_t smem = sel_smem_bytes(c->MB);
   ensure_smem((const void*)k_ema, smem);

@@ -428,6 +428,7 @@ struct StepArgs {
   int msw;  // channels per merge item (16 .. D): the narrowest slice that still gives every merge warp at most one item
   float scale; float pace_ns; double score_c;
   uint32_t* done_host; uint32_t done_seq;  // host-visible completion word (mapped host memory) and its value, or null
+  const int32_t* bud_seq;  // per sequence of the layer: 0 = the layer's budget, v > 0 = budget v - 1 (prr_set_budget_seq)
 };
 
 __device__ __forceinline__ int seq_len(const StepArgs& a, int b) { return __ldcg(a.seq_lens + b) + a.app; }
@@ -1108,7 +1109,8 @@ __device__ void run_job(const StepArgs& a, int jj, int R, const Team& tm, const 
     if (a.Bud <= 0) return;
   }
   // ---- exact selection (one call site) ----
-  const int k = min(is_sel ? a.K : a.BudSel, n);
+  const int bsel = a.bud_seq[b] > 0 ? min(a.bud_seq[b] - 1, a.Bud) : a.BudSel;
+  const int k = min(is_sel ? a.K : bsel, n);
   Keys ks{in_sm ? smem_u32(m.keys) : 0u, is_sel ? sc : pr};
   Thr t;
   t.key = 0u; t.idx = 0x7fffffff;  // k >= n: everything is selected
@@ -1758,6 +1760,7 @@ static int launch_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const 
   } a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.BudSel = c->bud_eff[kv->layer]; a.Rmax = c->maxB * c->Hkv;
+  a.bud_seq = c->bud_seq + (size_t)kv->layer * c->maxB;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
   a.scale = c->sm_scale; a.score_c = c->score_c;

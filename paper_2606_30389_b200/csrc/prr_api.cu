@@ -131,6 +131,7 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   A(dalloc(c, &c->ema_v, rows * c->MB));
   A(dalloc(c, &c->n_state, rows));
   A(dalloc(c, &c->theta, (size_t)c->NL * c->maxB * 3));
+  A(dalloc(c, &c->bud_seq, (size_t)c->NL * c->maxB));
   A(dalloc(c, &c->open_sum, rows * c->D));
   A(dalloc(c, &c->scores, rows * c->MB));
   A(dalloc(c, &c->setA, rows * c->K));
@@ -196,6 +197,7 @@ extern "C" int32_t prr_create(const prr_layout* lay, int32_t block_size, int32_t
   c->ev_upd.assign(c->NL, nullptr);
   c->upd_pending.assign(c->NL, 0);
   c->bud_eff.assign(c->NL, c->Bud);
+  c->bud_seq_h.assign((size_t)c->NL * c->maxB, 0);
   c->kscale.assign(c->NL, nullptr); c->vscale.assign(c->NL, nullptr);
   for (int l = 0; l < c->NL; ++l) A(cudaEventCreateWithFlags(&c->ev_upd[l], cudaEventDisableTiming));
   if (e != cudaSuccess) {
@@ -446,6 +448,30 @@ static void repredict(prr_ctx* c, int layer, cudaStream_t s) {  // P of the next
   e.P_out = c->P_next + layer_rows(c, layer) * c->Bud;
   launch_ema(c, e, s);
   sync_pred(c, layer, 0, c->maxB, s);
+}
+
+__global__ void k_set_i32(int32_t* p, int32_t v) { *p = v; }
+
+extern "C" int32_t prr_set_budget_seq(prr_ctx* ctx, int32_t layer, int32_t seq, int32_t budget, void* stream) {
+  if (!ctx) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || seq < 0 || seq >= ctx->maxB) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_budget_seq: layer / seq out of range");
+  if (budget < -1 || budget > ctx->Bud) PRR_FAIL(ctx, PRR_E_INVALID, "prr_set_budget_seq: budget must be -1 (the layer's) or 0 .. the budget of prr_create");
+  cudaStream_t s = (cudaStream_t)stream;
+  join_layer(ctx, layer, s);
+  const size_t i = (size_t)layer * ctx->maxB + seq;
+  ctx->bud_seq_h[i] = budget + 1;
+  k_set_i32<<<1, 1, 0, s>>>(ctx->bud_seq + i, budget + 1);
+  ctx->launches++;
+  repredict(ctx, layer, s);  // the next decode step already speculates on the new budget
+  return check_launch(ctx, "prr_set_budget_seq");
+}
+
+extern "C" int32_t prr_get_budget_seq(const prr_ctx* ctx, int32_t layer, int32_t seq, int32_t* budget_out) {
+  if (!ctx || !budget_out) return PRR_E_INVALID;
+  if (layer < 0 || layer >= ctx->NL || seq < 0 || seq >= ctx->maxB) return PRR_E_INVALID;
+  const int v = ctx->bud_seq_h[(size_t)layer * ctx->maxB + seq];
+  *budget_out = v > 0 ? v - 1 : ctx->bud_eff[layer];
+  return PRR_OK;
 }
 
 extern "C" int32_t prr_set_mode(prr_ctx* ctx, int32_t mode, void* stream) {
@@ -706,7 +732,11 @@ static int fused_step(prr_ctx* c, const prr_paged_kv* kv, const void* q, const v
   // every SM whatever the batch), a cluster per row once the rows fill the GPU (measured: DESIGN.md section 8).
   const int rows = kv->batch * c->Hkv;
   // a run-time budget of 0 (prr_set_budget re-predicted: P is empty) IS the sequential path: take it outright
-  if (spec && c->bud_eff[kv->layer] == 0) spec = 0;
+  if (spec && c->bud_eff[kv->layer] == 0) {
+    bool any = false;  // (a sequence with its own budget > 0 still speculates)
+    for (int b = 0; b < kv->batch; ++b) any |= c->bud_seq_h[(size_t)kv->layer * c->maxB + b] > 1;
+    if (!any) spec = 0;
+  }
   int kern = c->kernel;
   if (kern == 0) kern = rows >= 64 ? 2 : 1;
   if (c->bs > 128 || c->mode == PRR_MODE_S1) kern = 2;  // (only the cluster kernel cuts a block into sub-tiles / recomputes on a miss)

@@ -75,6 +75,8 @@ struct prr_ctx {
   cudaEvent_t ev_fork = nullptr, ev_spec = nullptr, ev_sel = nullptr;
   std::vector<cudaEvent_t> ev_upd; // per layer: EMA update of the last step of that layer done
   std::vector<char> upd_pending;
+  int32_t* bud_seq = nullptr;      // [NL, maxB] device: per-sequence budget + 1, 0 = follow the layer's (prr_set_budget_seq)
+  std::vector<int> bud_seq_h;      // host mirror of bud_seq
   std::vector<int> bud_eff;        // per layer: blocks predicted for the next step, 0 .. Bud (prr_set_budget)
   std::vector<double> bud_poly;    // fitted budget(context length): coefficients in x = ctx_len / bud_xscale (prr_budget_fit)
   double bud_xscale = 1.0;

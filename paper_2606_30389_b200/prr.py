@@ -34,6 +34,7 @@ SYMBOLS = [
     "prr_timeline_enable", "prr_timeline_read", "prr_timeline_peek", "prr_set_option", "prr_get_option",
     "prr_graph_begin", "prr_graph_end", "prr_graph_launch", "prr_graph_destroy",
     "prr_static_scratch_bytes", "prr_attend_blocks_static", "prr_quantize_kv_fp8", "prr_set_kv_scales",
+    "prr_set_budget_seq", "prr_get_budget_seq",
 ]
 
 
@@ -204,6 +205,14 @@ class Context:
                                    C.c_void_p(_p(P)), C.c_void_p(_p(O_part)), C.c_void_p(_p(m_part)),
                                    C.c_void_p(_p(l_part)), C.c_void_p(_p(out)), C.c_void_p(_p(m_out)),
                                    C.c_void_p(_p(l_out)), C.c_void_p(_stream(stream))))
+
+    def set_budget_seq(self, layer, seq, budget, stream=None):
+        self._chk(lib().prr_set_budget_seq(self._h, C.c_int32(layer), C.c_int32(seq), C.c_int32(budget), C.c_void_p(_stream(stream))))
+
+    def get_budget_seq(self, layer, seq) -> int:
+        v = C.c_int32()
+        self._chk(lib().prr_get_budget_seq(self._h, C.c_int32(layer), C.c_int32(seq), C.byref(v)))
+        return v.value
 
     def quantize_kv_fp8(self, kv, k8_pages, v8_pages, k_scale, v_scale, stream=None):
         self._chk(lib().prr_quantize_kv_fp8(self._h, C.byref(kv), C.c_void_p(_p(k8_pages)), C.c_void_p(_p(v8_pages)),

@@ -604,6 +604,42 @@ def test_runtime_budget_varies_per_step(cfg, kernel):
         gl.ctx.set_budget(0, cfg.Bud + 1)
 
 
+@pytest.mark.parametrize("mode", ["k_step", "k_row", "streams"])
+def test_per_sequence_budgets_in_one_batch(mode):
+    """prr_set_budget_seq: the sequences of ONE batch carry different run-time budgets (one of
+    them 0 = no speculation, one the layer's), changed between steps; A, P, M bit-exact against the oracle run with
+    the same per-sequence budgets, outputs in tolerance, PRR within 1e-5 of the sequential path."""
+    cfg = TINY                                                   # B = 3
+    kw = dict(kernel={"k_step": 1, "k_row": 2}.get(mode)) if mode != "streams" else dict(orchestration=prr.STREAMS)
+    cfg, inp, gl, ol = make(cfg, steps=8, **kw)
+    twin = H.GpuLayer(cfg, inp, **kw)
+    gl.calibrate(inp.q_cal); twin.calibrate(inp.q_cal); ol.calibrate(synth.bits(inp.q_cal))
+    plans = [[0, None, 5], [0, None, 5], [cfg.Bud, 0, None], [3, 0, None], [None, None, None], [0, 0, 0], [1, cfg.K, 0],
+             [None, 2, cfg.Bud]]
+    for t in range(8):
+        for b in range(cfg.B):
+            v = plans[t][b]
+            gl.ctx.set_budget_seq(0, b, -1 if v is None else v)
+            assert gl.ctx.get_budget_seq(0, b) == (cfg.Bud if v is None else v)
+        ol.budget_seq = plans[t]
+        out = gl.step_append(t) if mode != "streams" else (gl.append(t), gl.step(t))[1]
+        twin.append(t); o2 = twin.step(t, sequential=True)
+        torch.cuda.synchronize()
+        ol.append(synth.bits(inp.k_new[t]), synth.bits(inp.v_new[t]))
+        r = ol.step(synth.bits(inp.q_dec[t]))
+        for b in range(cfg.B):
+            cap = cfg.Bud if plans[t][b] is None else plans[t][b]
+            assert all(len(r["P"][b][h]) <= cap for h in range(cfg.Hkv))
+        H.compare_sets(gl, r, f"per-seq budgets {plans[t]} t{t}")
+        H.check_out(out.cpu().numpy(), r["out"], f"per-seq budgets t{t}")
+        assert (out - o2).abs().max().item() <= 1e-5
+    with pytest.raises(prr.PrrError):
+        gl.ctx.set_budget_seq(0, cfg.B, 1)                       # seq out of range
+    with pytest.raises(prr.PrrError):
+        gl.ctx.set_budget_seq(0, 0, cfg.Bud + 1)
+    gl.ctx.check()
+
+
 def test_profile_budget_leaves_no_trace_and_fit():
     """prr_profile_budget sweeps candidate budgets on the layer's cache (section 4.4 in the library) and
     restores the predictor state: the decode steps after it still match the oracle bit-exactly.  prr_budget_fit /

@@ -668,3 +668,34 @@ def test_quantize_kv_e4m3_error_bound_and_exact_dequant():
     c2, s2 = O.quantize_kv_e4m3(k2, table, np.array([64, 64]), bs)
     live = [table[b, i] for b in range(2) for i in range(O.n_blocks_of(lens[b], bs))]
     assert np.array_equal(O.dequantize_kv_e4m3(c2, s2)[live], k2[live])
+
+
+def test_oracle_layer_per_sequence_budgets():
+    """budget_seq: a sequence's P is the top-budget_seq[b] prediction; None follows the layer's
+    budget; a run with budget_seq equal to the layer's budget everywhere is the plain run; a sequence's result does
+    not depend on the other sequences' budgets (rows are independent)."""
+    rng = np.random.default_rng(31)
+    bs, Hkv, d, B = 8, 2, 8, 3
+    lens = np.array([61, 80, 47])
+    table = rng.permutation(3 * 11).astype(np.int32).reshape(3, 11)
+    k = O.f64_to_bf16(rng.standard_normal((34, Hkv, bs, d)))
+    v = O.f64_to_bf16(rng.standard_normal((34, Hkv, bs, d)))
+    qs = O.f64_to_bf16(rng.standard_normal((5, B, 4, d)))
+    def run(budget_seq):
+        lay = O.OracleLayer(k, v, table, lens, bs, 3, 5, 4)
+        lay.theta = [(0.6, 0.2, 0.5)] * B
+        lay.budget_seq = budget_seq
+        return [lay.step(qs[t]) for t in range(5)]
+    plain, same, mixed = run(None), run([5, 5, None]), run([0, 2, None])
+    for t in range(5):
+        for b in range(B):
+            for h in range(Hkv):
+                assert np.array_equal(plain[t]["P"][b][h], same[t]["P"][b][h])
+                assert np.array_equal(plain[t]["A"][b][h], mixed[t]["A"][b][h])          # A never depends on the budget
+        assert all(len(mixed[t]["P"][0][h]) == 0 for h in range(Hkv))
+        assert all(len(mixed[t]["P"][1][h]) <= 2 for h in range(Hkv))
+        assert all(np.array_equal(mixed[t]["P"][2][h], plain[t]["P"][2][h]) for h in range(Hkv))
+        if t > 0:                                                                       # P_t (budget 2) = the top 2 of P_t (budget 5)
+            for h in range(Hkv):
+                assert set(mixed[t]["P"][1][h]) <= set(plain[t]["P"][1][h]) and len(mixed[t]["P"][1][h]) == 2
+        assert np.array_equal(mixed[t]["out"], plain[t]["out"])                         # DROP: the output is attention over A
