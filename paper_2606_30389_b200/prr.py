@@ -75,6 +75,8 @@ def lib() -> C.CDLL:
         L.prr_launch_count.argtypes = [C.c_void_p]
         L.prr_set_ema_params.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double,
                                          C.c_double, C.c_void_p]
+        L.prr_decode_step_host.argtypes = [C.c_void_p, C.POINTER(PagedKV)] + [C.c_void_p] * 6  # (plain ints pass as is)
+        L.prr_decode_step_host.restype = C.c_int32
         _lib = L
     return _lib
 
@@ -244,10 +246,13 @@ class Context:
                                         C.c_int32(int(bool(sequential))), C.c_void_p(_stream(stream))))
 
     def decode_step_host(self, kv, q_host, k_new_host, v_new_host, summaries, out_host, stream=None):
-        self._chk(lib().prr_decode_step_host(self._h, C.byref(kv), C.c_void_p(_p(q_host)),
-                                             C.c_void_p(_p(k_new_host)), C.c_void_p(_p(v_new_host)),
-                                             C.c_void_p(_p(summaries)), C.c_void_p(_p(out_host)),
-                                             C.c_void_p(_stream(stream))))
+        if type(q_host) is int and type(stream) is int:  # addresses taken by the caller: marshalling only
+            r = lib().prr_decode_step_host(self._h, kv, q_host, k_new_host, v_new_host, summaries, out_host, stream)
+            if r:
+                self._chk(r)
+            return
+        self._chk(lib().prr_decode_step_host(self._h, C.byref(kv), _p(q_host), _p(k_new_host), _p(v_new_host),
+                                             _p(summaries), _p(out_host), _stream(stream)))
 
     # -- introspection -----------------------------------------------------------------------
     def get_sets(self, layer, batch, A=None, P=None, M=None, counts=None, stream=None):
