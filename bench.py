@@ -194,14 +194,14 @@ def workload_name(cfg, R):
 class Stack:
     """R layers of the workload resident in HBM + the library context."""
 
-    def __init__(self, cfg, R, tokens, dev, seed_off=0, kernel=0):
+    def __init__(self, cfg, R, tokens, dev, seed_off=0, kernel=0, policy=0):
         from paper_2606_30389_b200 import prr
         self.prr, self.cfg, self.R, self.dev = prr, cfg, R, dev
         self.inps = [synth.make_layer(cfg.scaled(seed=cfg.seed + seed_off), l, device=dev, steps=tokens,
                                       poison=False) for l in range(R)]
         self.MB = self.inps[0].block_table.shape[1]
         self.ctx = prr.Context(cfg.Hq, cfg.Hkv, cfg.d, cfg.bs, cfg.K, cfg.Bud, max_batch=cfg.B,
-                               max_blocks_per_seq=self.MB, n_layers=R)
+                               max_blocks_per_seq=self.MB, n_layers=R, policy=policy)
         self.ctx.set_option(prr.OPT_KERNEL, kernel)
         self.kvs, self.summ = [], []
         for l, inp in enumerate(self.inps):
@@ -391,6 +391,7 @@ def main():
     ap.add_argument("--cluster", type=int, default=0, help="force the cluster size of k_row (0 = the library's choice)")
     ap.add_argument("--subtile", type=int, default=0, help="PRR_OPT_SUBTILE: tokens per tile unit of k_row (16 / 32 / 64)")
     ap.add_argument("--stage-fp8", action="store_true", help="prr_speculate on bf16 vs fp8 (e4m3) pages of the config")
+    ap.add_argument("--retain", action="store_true", help="PRR_RETAIN (PAPER.md:40: over-predicted blocks stay in the output)")
     ap.add_argument("--sweep", action="store_true", help="Table-3-shaped sweep: block size x token budget at 128K, 32q/8kv")
     args = ap.parse_args()
 
@@ -429,7 +430,7 @@ def main():
     total = 4 * W + K + seq_steps + E + min(K, 2048)
     tokens = (total + R - 1) // R + 2
     kern = {"auto": 0, "persistent": 1, "cluster": 2}[args.kernel]
-    st = Stack(cfg, R, tokens, dev, seed_off=rank_seed_offset(rank), kernel=kern)
+    st = Stack(cfg, R, tokens, dev, seed_off=rank_seed_offset(rank), kernel=kern, policy=1 if args.retain else 0)
     if args.cluster:
         st.ctx.set_option(st.prr.OPT_CLUSTER, args.cluster)
     if args.subtile:

@@ -66,6 +66,7 @@ struct RowArgs {
   uint32_t* ctl; unsigned long long* stats; unsigned long long* tl;
   int B, Hq, Hkv, G, MB, MBw, bs, K, Bud, retain, spec, cut;
   int recompute;  // ablation S1: any miss in the row -> the speculative result is discarded, all of A is fetched
+  int BudMax;  // the largest run-time budget among the launch's sequences (sizes the parking slots)
   int CS, NBUF, NSLOT, UCAP, HL, SLMAX, NBH, BudSel;  // BudSel <= Bud: the run-time budget of the NEXT prediction
   // dynamic shared memory offsets (bytes)
   int o_keys, o_pkeys, o_hist, o_plist, o_pmask, o_amask, o_offs, o_tslice, o_sc, o_units, o_cand, o_red,
@@ -979,7 +980,9 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
             const int bi = pos % NBUF;
             if (pos >= NBUF) {  // the buffer's previous tenant must be consumed
               const uint32_t par = ((pos / NBUF) - 1) & 1;
-              bool free_ = mbar_try_wait_cl(&sh.empty[bi], par);
+              // (try_wait may suspend the thread for a system-dependent time: while A is still unknown the probe must
+              // not block, or the repair units -- the critical path -- are issued late)
+              bool free_ = nrep < 0 ? mbar_test_wait(&sh.empty[bi], par) : mbar_try_wait_cl(&sh.empty[bi], par);
               if (!free_ && nrep < 0) {  // keep an eye on A while waiting
                 while (!(free_ = mbar_test_wait(&sh.empty[bi], par)) && !sh.sel_done)
                   if ((++itw & 1023u) == 0 && (long long)(gtime() - t0w) > (long long)WAIT_NS) { wait_fail(err, 3); break; }
@@ -1649,7 +1652,8 @@ static cudaError_t plan_and_launch(prr_ctx* c, RowArgs& a, cudaStream_t s) {
   // a slot per speculative unit of a CTA if they fit (a unit whose fate is unknown and that finds no slot
   // holds its warp until A is known); then the deepest ring; a ring of at least four tenants comes first
   // (the sequential path parks nothing: its shared memory goes to the ring)
-  a.NSLOT = a.spec ? std::max(1, std::min(16, ((a.Bud + CS - 1) / CS) * ((a.bs + ST - 1) / ST))) : 1;
+  // (and a small run-time budget parks few: a.BudMax is the largest budget in force among the launch's sequences)
+  a.NSLOT = a.spec ? std::max(1, std::min(16, ((std::min(a.Bud, a.BudMax) + CS - 1) / CS) * ((a.bs + ST - 1) / ST))) : 1;
   const int min_ring = 4;
   const int budget = c->row_dyn[key];
   int NBUF = NBMAX;
@@ -1768,6 +1772,11 @@ int launch_step_cluster(prr_ctx* c, const prr_paged_kv* kv, const void* q, const
   a.tl = c->tl_on ? c->tl : nullptr;
   a.B = kv->batch; a.Hq = c->Hq; a.Hkv = c->Hkv; a.G = c->G; a.MB = c->MB; a.MBw = (c->MB + 31) / 32 + 1;
   a.bs = c->bs; a.K = c->K; a.Bud = c->Bud; a.NBH = c->MB; a.BudSel = c->bud_eff[kv->layer];
+  a.BudMax = a.BudSel;
+  for (int b = 0; b < kv->batch; ++b) {
+    const int v = c->bud_seq_h[(size_t)kv->layer * c->maxB + b];
+    if (v > 0) a.BudMax = std::max(a.BudMax, v - 1);
+  }
   a.bud_seq = c->bud_seq + (size_t)kv->layer * c->maxB;
   a.retain = c->lay.overpredict_policy == PRR_RETAIN;
   a.spec = (spec && c->Bud > 0) ? 1 : 0;
