@@ -1381,11 +1381,18 @@ __global__ void __launch_bounds__(NTHR, 1) k_row(const __grid_constant__ RowArgs
           g.sync();
           all_rep = sh.miss_cnt > 0;
         }
-        for (int i = s0 + g.tid; i < min(s1, nb); i += g.nt) {
-          const uint32_t bit = 1u << (i & 31);
-          if ((amask[i >> 5] & bit) && (all_rep || !(pmask[i >> 5] & bit))) {
-            const int pos = atomicAdd(&sh.rep_cnt, 1);
-            units[UREP0 + pos] = make_int2(i, tslice[i - s0]);
+        {  // one shared-memory atomic per warp and trip (same-address atomics serialise: 64 of them cost ~1 us)
+          const int lim = min(s1, nb);
+#pragma unroll 1
+          for (int i0 = s0 + g.wid * 32; i0 < lim; i0 += g.nt) {
+            const int i = i0 + lane;
+            const uint32_t bit = 1u << (i & 31);
+            const bool rep_i = i < lim && (amask[i >> 5] & bit) && (all_rep || !(pmask[i >> 5] & bit));
+            const uint32_t bal = __ballot_sync(FULL, rep_i);
+            int base = 0;
+            if (lane == 0 && bal) base = atomicAdd(&sh.rep_cnt, __popc(bal));
+            base = __shfl_sync(FULL, base, 0);
+            if (rep_i) units[UREP0 + base + __popc(bal & ((1u << lane) - 1u))] = make_int2(i, tslice[i - s0]);
           }
         }
         g.sync();
